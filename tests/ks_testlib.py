@@ -1,0 +1,73 @@
+"""Helpers for the tests: golden-file parser and two independent restatements of the clearing
+definition (brute force over all ticks; greedy unit matching).  These live in the test tree, not
+in oracle/: they are what the oracle is pinned AGAINST."""
+import os
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLDEN = os.path.join(ROOT, "tests", "golden")
+
+
+def read_golden(name):
+    """Parse a tests/golden/*.txt fixture: '#' lines are comments (citations), blank lines
+    separate records, 'key: v v v' lines are fields.  -> list of dict(key -> list of str)."""
+    recs, cur = [], {}
+    with open(os.path.join(GOLDEN, name)) as f:
+        for line in f:
+            line = line.rstrip("\n")
+            if line.startswith("#"):
+                continue
+            if not line.strip():
+                if cur:
+                    recs.append(cur)
+                    cur = {}
+                continue
+            k, v = line.split(":", 1)
+            cur[k.strip()] = v.split()
+    if cur:
+        recs.append(cur)
+    return recs
+
+
+
+
+def ints(rec, key):
+    return np.array([int(x) for x in rec[key]], dtype=np.int64)
+
+
+def brute_force_price(bid, ask):
+    """Eq.1-2 evaluated literally, O(L^2): for every p sum the bids at q >= p
+    and the asks at q <= p; the price is the lowest p attaining the largest min(D, S).
+    -> (pstar or -1, vmax, D, S)."""
+    L = len(bid)
+    D = [sum(int(bid[q]) for q in range(L) if q >= p) for p in range(L)]
+    S = [sum(int(ask[q]) for q in range(L) if q <= p) for p in range(L)]
+    V = [min(D[p], S[p]) for p in range(L)]
+    vmax = max(V)
+    pstar = V.index(vmax) if vmax > 0 else -1
+    return pstar, vmax, D, S
+
+
+def greedy_match(bid, ask):
+    """Price-priority matching one lot at a time: repeatedly take the highest
+    outstanding bid and the lowest outstanding ask; while bid tick >= ask tick, trade
+    min(remaining) lots.  Stops when the book is uncrossed.  -> (volume, new_bid, new_ask).
+    Knows nothing of cumulative profiles or of p*."""
+    b = [int(x) for x in bid]
+    a = [int(x) for x in ask]
+    L = len(b)
+    vol = 0
+    hi, lo = L - 1, 0
+    while True:
+        while hi >= 0 and b[hi] == 0:
+            hi -= 1
+        while lo < L and a[lo] == 0:
+            lo += 1
+        if hi < 0 or lo >= L or hi < lo:
+            break
+        x = min(b[hi], a[lo])
+        b[hi] -= x
+        a[lo] -= x
+        vol += x
+    return vol, np.array(b, dtype=np.int64), np.array(a, dtype=np.int64)
