@@ -1,0 +1,171 @@
+/*
+ * kineticsim.h -- C ABI of the B200-native (sm_100a) call-auction clearing library.
+ *
+ * The library runs the hot path of KineticSim (arxiv/paper_2606_21784; citations are PAPER.md
+ * line numbers): M independent limit-order-book markets, each with L price ticks and A agents,
+ * advanced S steps by ONE launch of a persistent kernel that keeps every market's book in shared
+ * memory for all S steps (Alg.1; SIII-A/B) and touches HBM
+ * once to load and once to store the state (Eq.6).  Per step and market:
+ *   1. every agent a draws one Philox4x32-10 block keyed by (seed, market, step, agent) and turns
+ *      it into a limit order (side, tick, integer quantity)       (SIII-C)
+ *   2. orders are added to the int32 bid/ask depth per tick with shared-memory atomics
+ *                                                          (Alg.1 l.10-13)
+ *   3. D[p] = sum_{q>=p} bid[q], S[p] = sum_{q<=p} ask[q]              (Eq.1)
+ *   4. p* = lowest p maximising V[p] = min(D[p], S[p]), Vmax = V[p*]   (Eq.2; ties
+ *      to the lowest tick)
+ *   5. price-priority allocation; the unfilled remainder rests for the next step:
+ *      bid[p] <- min(bid[p], max(0, D[p]-Vmax)), ask[p] <- min(ask[p], max(0, S[p]-Vmax));
+ *      nothing changes when Vmax = 0            (SIV-C)
+ *   6. prev <- last; last <- p* if Vmax > 0; int64 statistics accumulate
+ *
+ * Conventions.  No C++ types, exceptions or torch types cross this boundary.  Every pointer
+ * argument says whether it is a HOST or a DEVICE pointer.  `stream` is a cudaStream_t passed as
+ * void* (NULL = the legacy default stream).  Unless stated otherwise a call only ENQUEUES work on
+ * `stream` and returns; the caller synchronises, and calls on one ks_sim must be stream-ordered
+ * by the caller.  On an error return nothing has been enqueued.  There is no CPU fallback: with
+ * no CUDA device every call that needs one returns KS_ERR_CUDA.
+ */
+#ifndef KINETICSIM_H_
+#define KINETICSIM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define KS_API __attribute__((visibility("default")))
+#else
+#define KS_API
+#endif
+
+typedef struct ks_sim ks_sim; /* opaque host-side handle, owned by the library */
+
+typedef enum {
+  KS_OK = 0,
+  KS_ERR_INVALID_ARG = -1, /* NULL pointer, M < 1, A < 0, S < 0, L not a power of two or < 32, bad params */
+  KS_ERR_UNSUPPORTED = -2, /* L above the single-CTA limit (16384) -- see DESIGN.md "out of scope"        */
+  KS_ERR_OVERFLOW = -3,    /* a per-side depth sum or a statistic could leave its integer type            */
+  KS_ERR_CUDA = -4,        /* a CUDA call failed; text in ks_last_error()                                 */
+  KS_ERR_NOMEM = -5        /* host allocation failed                                                      */
+} ks_status;
+
+typedef enum {
+  KS_MODEL_ZI = 0,  /* every agent is a zero-intelligence noise trader (BASELINE.json configs[0..3]) */
+  KS_MODEL_MIX3 = 1 /* agent a: a%3 = 0 noise, 1 market maker, 2 momentum (BASELINE.json configs[4]) */
+} ks_model;
+
+/*
+ * Agent rules (SIII-C, in the integer form BASELINE.json fixes).  With
+ * w0..w3 = Philox4x32-10(ctr = (agent, step, market, 0), key = (seed lo, seed hi)),
+ * mulhi(w, n) = (uint64(w) * n) >> 32, clamp(x) = min(max(x, 0), L-1), and last / prev the last
+ * two clearing prices as they were at the START of the step:
+ *   noise     buy = w0 >> 31; o = mulhi(w1, 2*noise_delta+1) - noise_delta; q = 1 + mulhi(w2, noise_qmax)
+ *             tick = buy ? clamp(last - o) : clamp(last + o)
+ *   maker     s = 1 + mulhi(w1, maker_spread_max); bid maker_qty @ clamp(last - s) AND ask
+ *             maker_qty @ clamp(last + s) (one agent event, two orders)
+ *   momentum  dp = last - prev; buy = dp > 0 ? 1 : dp < 0 ? 0 : w0 >> 31; o = mulhi(w1, mom_delta+1)
+ *             q = 1 + mulhi(w2, mom_qmax); tick = buy ? clamp(last + o) : clamp(last - o)
+ * Ranges: 0 <= noise_delta, mom_delta, maker_spread_max-1 < L; 1 <= qmax, qty <= 2^20.
+ */
+typedef struct {
+  int32_t model;            /* ks_model                                             */
+  int32_t noise_delta;      /* noise offset uniform in [-noise_delta, +noise_delta] */
+  int32_t noise_qmax;       /* noise quantity uniform in 1..noise_qmax              */
+  int32_t maker_spread_max; /* maker spread uniform in 1..maker_spread_max          */
+  int32_t maker_qty;        /* maker quantity posted on each side                   */
+  int32_t mom_delta;        /* momentum offset uniform in [0, mom_delta]            */
+  int32_t mom_qmax;         /* momentum quantity uniform in 1..mom_qmax             */
+  int32_t init_price;       /* opening last = prev; < 0 means L/2                   */
+} ks_agent_params;
+
+/*
+ * Per-market statistics record, 128 bytes, integer sums only ("clearing statistics",
+ * PAPER.md:302).  r = last_after - last_before of a step (0 on a no-trade step).
+ *   f[0] steps       f[1] n_trades (steps with Vmax > 0)   f[2] sum Vmax       f[3] sum p*
+ *   f[4] sum p*^2    f[5] sum p* * Vmax                    f[6] sum r          f[7] sum r^2
+ *   f[8] sum r^3     f[9] sum r^4      f[10] submitted bid quantity   f[11] submitted ask quantity
+ *   f[12] last       f[13] prev        f[14] trajectory hash (uint64) f[15] number of orders
+ * Trajectory hash: h0 = 0xcbf29ce484222325; per step x = Vmax > 0 ? (uint64(Vmax) << 16 | p*) :
+ * 0xFFFF; h = (h ^ x) * 0x100000001b3 mod 2^64 -- it pins every step's (p*, Vmax).
+ */
+typedef struct { int64_t f[16]; } ks_market_stats;
+
+/* fp64 statistics derived on the HOST from one record by ks_derive_stats:
+ *   d[0] mean clearing price = f3/f1        d[1] VWAP = f5/f2          d[2] volume per step = f2/f0
+ *   d[3] mean return mu = f6/f0             d[4] return variance = f7/f0 - mu^2
+ *   d[5] excess kurtosis = m4/var^2 - 3, m4 = (f9 - 4 mu f8 + 6 mu^2 f7)/f0 - 3 mu^4
+ * A quantity with a zero denominator is NaN. */
+typedef struct { double d[6]; } ks_derived_stats;
+
+/* Bytes of the caller-owned DEVICE state buffer: int32 books[M][2][L] (side 0 = bid, 1 = ask),
+ * then ks_market_stats rec[M], then 256 bytes of library scratch.  = M*(8*L+128) + 256.
+ * Returns 0 for arguments ks_create would reject. */
+KS_API size_t ks_state_bytes(int32_t M, int32_t L);
+
+/*
+ * Create a simulation of M markets x L ticks x A agents (Alg.1 "Require").
+ *   out      HOST: receives the handle (freed by ks_destroy).
+ *   p        HOST: agent parameters, copied.
+ *   seed     Philox key.
+ *   d_state  DEVICE: caller-owned buffer of ks_state_bytes(M, L) bytes, 16-byte aligned; the
+ *            library never allocates or frees device memory and never frees d_state.  It IS the
+ *            checkpoint: books, prices, step counter and accumulators live there between calls.
+ * Enqueues the initialisation on `stream`: empty books, last = prev = init price, zero sums
+ * (Alg.1 l.2-3; opening quotes per BASELINE.json: empty book, price L/2).
+ * ks_create_ex additionally takes the global id of this shard's first market: Philox is keyed by
+ * market_base + local index, so a market's trajectory does not depend on how the market range is
+ * partitioned across GPUs.  ks_create(...) == ks_create_ex(..., market_base = 0, ...).
+ */
+KS_API ks_status ks_create(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p,
+                           uint64_t seed, void* d_state, void* stream);
+KS_API ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p,
+                              uint64_t seed, uint32_t market_base, void* d_state, void* stream);
+
+/*
+ * Advance every market by S steps with ONE launch of the persistent kernel,
+ * continuing from the state in d_state: the Philox step index is steps_done + i, so
+ * ks_run(S1); ks_run(S2) leaves the same bytes as ks_run(S1+S2).  S = 0 is a no-op.
+ * KS_ERR_OVERFLOW (nothing enqueued) when (steps_done+S) x per-step per-side inflow bound, plus
+ * the depth injected by ks_write_books, could reach 2^31, or (L-1)^4 x (steps_done+S) >= 2^63.
+ * After a ks_write_books this call first waits (host-side) for that call's depth check.
+ */
+KS_API ks_status ks_run(ks_sim* s, int64_t S, void* stream);
+
+/* Copy the books / the records out of d_state.  dst: HOST or DEVICE pointer (cudaMemcpyDefault),
+ * int32 [M][2][L] resp. ks_market_stats [M]; a host destination must stay valid until the stream
+ * work is done (pinned memory makes the copy asynchronous).  Alg.1 "Ensure". */
+KS_API ks_status ks_read_books(ks_sim* s, int32_t* dst, void* stream);
+KS_API ks_status ks_read_stats(ks_sim* s, ks_market_stats* dst, void* stream);
+
+/* Replace the resting books (test / checkpoint-restore hook: "seeds the opening quotes",
+ * PAPER.md:126).  src: HOST or DEVICE pointer, int32 [M][2][L], every entry >= 0.  Records are
+ * left as they are.  Also enqueues a depth check whose result the next ks_run waits for. */
+KS_API ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream);
+
+/* Tuning / ablation switches; none of them changes a single output byte.  Returns
+ * KS_ERR_INVALID_ARG for an unknown option or value. */
+typedef enum {
+  KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 64..1024, multiple of 32          */
+  KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
+  KS_OPT_CLEAR_PATH = 2     /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
+} ks_option;
+KS_API ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value);
+
+/* HOST-only helper: derive the fp64 statistics of n records. */
+KS_API void ks_derive_stats(const ks_market_stats* rec, ks_derived_stats* out, int64_t n);
+
+KS_API void ks_destroy(ks_sim* s);
+
+/* Text of the last error on this thread; never NULL. */
+KS_API const char* ks_last_error(void);
+
+/* Number of kernels this library has launched in this process (all handles). */
+KS_API int64_t ks_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KINETICSIM_H_ */

@@ -1,0 +1,324 @@
+// ks_api.cu -- host side of the C ABI declared in include/kineticsim.h.
+#include "../../include/kineticsim.h"
+#include "../../include/kineticsim_bench.h"
+#include "ks_kernel.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+
+void set_err(const char* fmt, const char* a = "", const char* b = "") {
+  snprintf(g_err, sizeof(g_err), fmt, a, b);
+}
+
+#define KS_CUDA(call)                                                 \
+  do {                                                                \
+    cudaError_t e_ = (call);                                          \
+    if (e_ != cudaSuccess) {                                          \
+      set_err("%s failed: %s", #call, cudaGetErrorString(e_));        \
+      return KS_ERR_CUDA;                                             \
+    }                                                                 \
+  } while (0)
+
+bool is_pow2(int32_t x) { return x > 0 && (x & (x - 1)) == 0; }
+
+constexpr int32_t kMaxL = 16384;          // 8*L = 128 KB of the 227 KB a CTA may own
+constexpr int32_t kMaxQty = 1 << 20;
+
+}  // namespace
+
+struct ks_sim {
+  int32_t M, L, A;
+  ks_agent_params p;
+  uint64_t seed;
+  uint32_t market_base;
+  void* d_state;
+  int64_t steps_done;
+  int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books
+  int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
+  int32_t opt_threads, opt_atomic, opt_clear;
+  int32_t n_noise, n_maker, n_mom;
+  int64_t inflow_per_step;    // per-side bound on the quantity one step can add
+  // ks_write_books depth check
+  unsigned long long* h_bound;   // pinned host
+  cudaEvent_t bound_event;
+  int32_t bound_pending;
+  int32_t dev_smem_optin;
+  int32_t num_sms;
+};
+
+static int32_t* books_ptr(const ks_sim* s) { return reinterpret_cast<int32_t*>(s->d_state); }
+static long long* recs_ptr(const ks_sim* s) {
+  return reinterpret_cast<long long*>(reinterpret_cast<char*>(s->d_state) + (size_t)s->M * 8 * (size_t)s->L);
+}
+static unsigned long long* scratch_ptr(const ks_sim* s) {
+  return reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(s->d_state) +
+                                               (size_t)s->M * (8 * (size_t)s->L + 128));
+}
+
+static bool shape_ok(int32_t M, int32_t L) { return M >= 1 && is_pow2(L) && L >= 32 && L <= 32768; }
+
+extern "C" {
+
+size_t ks_state_bytes(int32_t M, int32_t L) {
+  if (!shape_ok(M, L)) return 0;
+  return (size_t)M * (8 * (size_t)L + 128) + 256;
+}
+
+const char* ks_last_error(void) { return g_err; }
+int64_t ks_launch_count(void) { return g_launches.load(); }
+
+ks_status ks_create(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
+                    void* d_state, void* stream) {
+  return ks_create_ex(out, M, L, A, p, seed, 0u, d_state, stream);
+}
+
+ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
+                       uint32_t market_base, void* d_state, void* stream) {
+  if (!out || !p || !d_state) { set_err("ks_create: NULL argument"); return KS_ERR_INVALID_ARG; }
+  *out = nullptr;
+  if (!shape_ok(M, L) || A < 0) { set_err("ks_create: need M >= 1, A >= 0, L a power of two in [32, 32768]"); return KS_ERR_INVALID_ARG; }
+  if ((reinterpret_cast<uintptr_t>(d_state) & 15) != 0) { set_err("ks_create: d_state must be 16-byte aligned"); return KS_ERR_INVALID_ARG; }
+  if (p->model != KS_MODEL_ZI && p->model != KS_MODEL_MIX3) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
+  if (p->noise_delta < 0 || p->noise_delta >= L || p->noise_qmax < 1 || p->noise_qmax > kMaxQty || p->init_price >= L) {
+    set_err("ks_create: bad noise parameters or init_price"); return KS_ERR_INVALID_ARG;
+  }
+  if (p->model == KS_MODEL_MIX3 &&
+      (p->maker_spread_max < 1 || p->maker_spread_max > L || p->maker_qty < 1 || p->maker_qty > kMaxQty ||
+       p->mom_delta < 0 || p->mom_delta >= L || p->mom_qmax < 1 || p->mom_qmax > kMaxQty)) {
+    set_err("ks_create: bad maker/momentum parameters"); return KS_ERR_INVALID_ARG;
+  }
+  if ((uint64_t)market_base + (uint64_t)M > 0x100000000ull) { set_err("ks_create: market ids exceed 32 bits"); return KS_ERR_INVALID_ARG; }
+  if (L > kMaxL) { set_err("ks_create: L > 16384 needs the cluster/DSMEM path, which is not built"); return KS_ERR_UNSUPPORTED; }
+
+  int dev = 0, optin = 0, sms = 0;
+  KS_CUDA(cudaGetDevice(&dev));
+  KS_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  KS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if ((size_t)8 * L + 2048 > (size_t)optin) { set_err("ks_create: book does not fit this device's shared memory"); return KS_ERR_UNSUPPORTED; }
+
+  ks_sim* s = new (std::nothrow) ks_sim();
+  if (!s) { set_err("ks_create: out of host memory"); return KS_ERR_NOMEM; }
+  s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
+  s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = 1;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0;
+  s->dev_smem_optin = optin; s->num_sms = sms;
+  s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
+  if (p->model == KS_MODEL_ZI) {
+    s->n_noise = A; s->n_maker = 0; s->n_mom = 0;
+    s->inflow_per_step = (int64_t)A * p->noise_qmax;
+  } else {
+    s->n_noise = (A + 2) / 3; s->n_maker = (A + 1) / 3; s->n_mom = A / 3;
+    s->inflow_per_step = (int64_t)s->n_noise * p->noise_qmax + (int64_t)s->n_maker * p->maker_qty +
+                         (int64_t)s->n_mom * p->mom_qmax;
+  }
+  if (s->p.init_price < 0) s->p.init_price = L / 2;
+
+  cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&s->h_bound), sizeof(unsigned long long), cudaHostAllocDefault);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->bound_event, cudaEventDisableTiming);
+  if (e != cudaSuccess) {
+    set_err("ks_create: %s", cudaGetErrorString(e));
+    if (s->h_bound) cudaFreeHost(s->h_bound);
+    delete s;
+    return KS_ERR_CUDA;
+  }
+  *s->h_bound = 0;
+
+  size_t nvec = (size_t)M * 2 * (size_t)L / 4;
+  int blocks = (int)((nvec + 255) / 256);
+  if (blocks > sms * 16) blocks = sms * 16;
+  if (blocks < 1) blocks = 1;
+  ks::ks_init_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<int4*>(books_ptr(s)), nvec, recs_ptr(s), M,
+                                                              s->p.init_price);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    set_err("ks_create: init launch failed: %s", cudaGetErrorString(e));
+    cudaFreeHost(s->h_bound); cudaEventDestroy(s->bound_event); delete s;
+    return KS_ERR_CUDA;
+  }
+  g_launches++;
+  *out = s;
+  return KS_OK;
+}
+
+void ks_destroy(ks_sim* s) {
+  if (!s) return;
+  if (s->h_bound) cudaFreeHost(s->h_bound);
+  if (s->bound_event) cudaEventDestroy(s->bound_event);
+  delete s;
+}
+
+ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
+  if (!s) { set_err("ks_set_option: NULL handle"); return KS_ERR_INVALID_ARG; }
+  switch (option) {
+    case KS_OPT_BLOCK_THREADS:
+      if (value != 0 && (value < 32 || value > 1024 || value % 32 != 0)) break;
+      s->opt_threads = value; return KS_OK;
+    case KS_OPT_ATOMIC_MODE:
+      if (value != 0 && value != 1) break;
+      s->opt_atomic = value; return KS_OK;
+    case KS_OPT_CLEAR_PATH:
+      if (value != 0 && value != 1) break;
+      s->opt_clear = value; return KS_OK;
+    default: break;
+  }
+  set_err("ks_set_option: unknown option or value");
+  return KS_ERR_INVALID_ARG;
+}
+
+}  // extern "C"
+
+// Threads per CTA.  Throughput regime (M CTAs oversubscribe the GPU): small CTAs so that many
+// markets are co-resident and one market's barrier/clearing phase hides behind another's
+// generation.  Few markets: widen the CTA so the whole GPU is used, but never beyond the agents.
+static int pick_threads(const ks_sim* s) {
+  if (s->opt_threads) return s->opt_threads;
+  const long long resident_threads = (long long)s->num_sms * 2048;
+  int T = 128;
+  while (T < 1024 && (long long)s->M * (T * 2) <= resident_threads && T * 2 <= s->A) T *= 2;
+  // the book must leave room for several CTAs per SM; with a large book prefer wider CTAs
+  const long long smem_per_cta = 8LL * s->L + 1536;
+  long long ctas_by_smem = (228LL * 1024) / smem_per_cta;
+  if (ctas_by_smem < 1) ctas_by_smem = 1;
+  while (T < 1024 && ctas_by_smem * T < 1536 && T * 2 <= (s->A > 32 ? s->A : 32)) T *= 2;
+  return T;
+}
+
+template <int MODEL, int ATOM>
+static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
+  auto kern = ks::ks_persistent_kernel<MODEL, ATOM>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e != cudaSuccess) return e;
+  kern<<<P.M, T, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
+  if (!s) { set_err("%s: NULL handle", who); return KS_ERR_INVALID_ARG; }
+  if (S < 0) { set_err("%s: S < 0", who); return KS_ERR_INVALID_ARG; }
+  if (S == 0) return KS_OK;
+  if (s->bound_pending) {
+    KS_CUDA(cudaEventSynchronize(s->bound_event));
+    s->bound_pending = 0;
+    if (*s->h_bound == 0xffffffffffffffffull) { set_err("%s: ks_write_books stored a negative depth", who); return KS_ERR_INVALID_ARG; }
+    s->resting_bound = (int64_t)*s->h_bound;
+  }
+  const long double total_steps = (long double)s->steps_done + (long double)S;
+  if ((long double)s->resting_bound + total_steps * (long double)s->inflow_per_step >= 2147483648.0L) {
+    set_err("%s: per-side depth could reach 2^31", who); return KS_ERR_OVERFLOW;
+  }
+  const long double lm1 = (long double)(s->L - 1);
+  if (lm1 * lm1 * lm1 * lm1 * total_steps >= 9223372036854775808.0L || total_steps >= 4294967296.0L) {
+    set_err("%s: a statistic or the step counter could overflow", who); return KS_ERR_OVERFLOW;
+  }
+
+  ks::KernelParams P;
+  memset(&P, 0, sizeof(P));
+  P.books = books_ptr(s);
+  P.recs = recs_ptr(s);
+  uint32_t k0 = (uint32_t)(s->seed & 0xffffffffu), k1 = (uint32_t)(s->seed >> 32);
+  for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += ks::kPhiloxW0; k1 += ks::kPhiloxW1; }
+  P.M = s->M; P.L = s->L; P.A = s->A; P.market_base = s->market_base;
+  P.noise_delta = s->p.noise_delta; P.noise_n = 2 * s->p.noise_delta + 1; P.noise_qmax = s->p.noise_qmax;
+  P.maker_spread_max = s->p.maker_spread_max; P.maker_qty = s->p.maker_qty;
+  P.mom_n = s->p.mom_delta + 1; P.mom_qmax = s->p.mom_qmax;
+  P.dmax = s->p.noise_delta;
+  if (s->p.model == KS_MODEL_MIX3) {
+    if (s->p.maker_spread_max > P.dmax) P.dmax = s->p.maker_spread_max;
+    if (s->p.mom_delta > P.dmax) P.dmax = s->p.mom_delta;
+  }
+  P.fresh = s->fresh;
+  P.force_generic = s->opt_clear;
+  P.S = S;
+  P.orders_per_step = (long long)s->A + s->n_maker;
+
+  const int T = pick_threads(s);
+  const size_t smem = (size_t)8 * s->L;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e;
+  if (s->p.model == KS_MODEL_ZI)
+    e = s->opt_atomic ? launch_persistent<0, 1>(P, T, smem, st) : launch_persistent<0, 0>(P, T, smem, st);
+  else
+    e = s->opt_atomic ? launch_persistent<1, 1>(P, T, smem, st) : launch_persistent<1, 0>(P, T, smem, st);
+  if (e != cudaSuccess) { set_err("%s: launch failed: %s", who, cudaGetErrorString(e)); return KS_ERR_CUDA; }
+  g_launches++;
+  s->steps_done += S;
+  s->fresh = 0;
+  return KS_OK;
+}
+
+extern "C" {
+
+ks_status ks_run(ks_sim* s, int64_t S, void* stream) { return run_impl(s, S, stream, "ks_run"); }
+
+// a8 ablation: the same kernel, one launch per step, book through HBM between launches.
+ks_status ks_run_stepwise(ks_sim* s, int64_t S, void* stream) {
+  if (!s) { set_err("ks_run_stepwise: NULL handle"); return KS_ERR_INVALID_ARG; }
+  if (S < 0) { set_err("ks_run_stepwise: S < 0"); return KS_ERR_INVALID_ARG; }
+  for (int64_t i = 0; i < S; ++i) {
+    ks_status r = run_impl(s, 1, stream, "ks_run_stepwise");
+    if (r != KS_OK) return r;
+  }
+  return KS_OK;
+}
+
+ks_status ks_read_books(ks_sim* s, int32_t* dst, void* stream) {
+  if (!s || !dst) { set_err("ks_read_books: NULL argument"); return KS_ERR_INVALID_ARG; }
+  KS_CUDA(cudaMemcpyAsync(dst, books_ptr(s), (size_t)s->M * 8 * (size_t)s->L, cudaMemcpyDefault, (cudaStream_t)stream));
+  return KS_OK;
+}
+
+ks_status ks_read_stats(ks_sim* s, ks_market_stats* dst, void* stream) {
+  if (!s || !dst) { set_err("ks_read_stats: NULL argument"); return KS_ERR_INVALID_ARG; }
+  KS_CUDA(cudaMemcpyAsync(dst, recs_ptr(s), (size_t)s->M * 128, cudaMemcpyDefault, (cudaStream_t)stream));
+  return KS_OK;
+}
+
+ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream) {
+  if (!s || !src) { set_err("ks_write_books: NULL argument"); return KS_ERR_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)stream;
+  KS_CUDA(cudaMemcpyAsync(books_ptr(s), src, (size_t)s->M * 8 * (size_t)s->L, cudaMemcpyDefault, st));
+  KS_CUDA(cudaMemsetAsync(scratch_ptr(s), 0, sizeof(unsigned long long), st));
+  ks::ks_depth_bound_kernel<<<2 * s->M, 128, 0, st>>>(books_ptr(s), s->L, scratch_ptr(s));
+  KS_CUDA(cudaGetLastError());
+  g_launches++;
+  KS_CUDA(cudaMemcpyAsync(s->h_bound, scratch_ptr(s), sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  KS_CUDA(cudaEventRecord(s->bound_event, st));
+  s->bound_pending = 1;
+  s->fresh = 0;
+  return KS_OK;
+}
+
+void ks_derive_stats(const ks_market_stats* rec, ks_derived_stats* out, int64_t n) {
+  const double nan = std::nan("");
+  for (int64_t i = 0; i < n; ++i) {
+    const int64_t* f = rec[i].f;
+    double* d = out[i].d;
+    const double steps = (double)f[0], ntr = (double)f[1], vol = (double)f[2];
+    d[0] = f[1] > 0 ? (double)f[3] / ntr : nan;
+    d[1] = f[2] > 0 ? (double)f[5] / vol : nan;
+    d[2] = f[0] > 0 ? vol / steps : nan;
+    if (f[0] > 0) {
+      const double mu = (double)f[6] / steps;
+      const double var = (double)f[7] / steps - mu * mu;
+      const double m4 = ((double)f[9] - 4.0 * mu * (double)f[8] + 6.0 * mu * mu * (double)f[7]) / steps -
+                        3.0 * mu * mu * mu * mu;
+      d[3] = mu; d[4] = var;
+      d[5] = var > 0 ? m4 / (var * var) - 3.0 : nan;
+    } else {
+      d[3] = d[4] = d[5] = nan;
+    }
+  }
+}
+
+}  // extern "C"

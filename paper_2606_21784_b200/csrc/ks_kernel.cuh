@@ -1,0 +1,203 @@
+// ks_kernel.cuh -- the persistent kernel (a0-a7) and the state-initialisation kernel.
+#pragma once
+#include "ks_device.cuh"
+
+namespace ks {
+
+// Block-wide reduction of (sum, sum, max, min) used once at load and once at write-back.
+struct BookTotals { long long sum_bid, sum_ask; int bmax, amin; };
+
+__device__ __forceinline__ BookTotals block_reduce_totals(long long sb, long long sa, int bmax, int amin,
+                                                          long long* s_red64, int* s_red32) {
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    sb += __shfl_xor_sync(FULL, sb, d);
+    sa += __shfl_xor_sync(FULL, sa, d);
+  }
+  bmax = __reduce_max_sync(FULL, bmax);
+  amin = __reduce_min_sync(FULL, amin);
+  __syncthreads();                      // protect s_red* against a previous use
+  if (lane == 0) { s_red64[2 * warp] = sb; s_red64[2 * warp + 1] = sa; s_red32[2 * warp] = bmax; s_red32[2 * warp + 1] = amin; }
+  __syncthreads();
+  BookTotals r; r.sum_bid = 0; r.sum_ask = 0; r.bmax = -1; r.amin = 0x7fffffff;
+  for (int w = 0; w < nwarps; ++w) {
+    r.sum_bid += s_red64[2 * w]; r.sum_ask += s_red64[2 * w + 1];
+    r.bmax = max(r.bmax, s_red32[2 * w]); r.amin = min(r.amin, s_red32[2 * w + 1]);
+  }
+  return r;
+}
+
+// a6: price state, statistics and trajectory hash -- executed by lane 0 of warp 0 on the
+// shared-memory copy of the record (include/kineticsim.h, ks_market_stats).
+__device__ __forceinline__ void update_record(long long* rec, int last, int vmax, int pstar, int& new_last) {
+  long long before = last;
+  unsigned long long x;
+  new_last = last;
+  if (vmax > 0) {
+    new_last = pstar;
+    rec[F_NTRADES] += 1;
+    rec[F_SUMVOL] += vmax;
+    rec[F_SUMPX] += pstar;
+    rec[F_SUMPX2] += (long long)pstar * pstar;
+    rec[F_SUMPXVOL] += (long long)pstar * vmax;
+    x = ((unsigned long long)(unsigned)vmax << 16) | (unsigned long long)(unsigned)pstar;
+  } else {
+    x = 0xFFFFull;
+  }
+  long long r = (long long)new_last - before;
+  long long r2 = r * r;
+  rec[F_SUMRET] += r;
+  rec[F_SUMRET2] += r2;
+  rec[F_SUMRET3] += r2 * r;
+  rec[F_SUMRET4] += r2 * r2;
+  rec[F_HASH] = (long long)(((unsigned long long)rec[F_HASH] ^ x) * kHashPrime);
+  rec[F_STEPS] += 1;
+  rec[F_PREV] = before;
+  rec[F_LAST] = new_last;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
+// dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
+// ---------------------------------------------------------------------------------------------
+template <int MODEL, int ATOM>
+__global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
+  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
+  __shared__ long long s_rec[16];
+  __shared__ long long s_red64[64];
+  __shared__ int s_red32[64];
+  __shared__ int s_ctl[4];                            // last, prev
+
+  const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
+  const int L = P.L;
+  const uint32_t market = P.market_base + blockIdx.x;
+  int32_t* gbook = P.books + (size_t)blockIdx.x * 2 * (size_t)L;
+  long long* grec = P.recs + (size_t)blockIdx.x * 16;
+
+  // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
+  long long sb0 = 0, sa0 = 0;
+  int bmax = -1, amin = 0x7fffffff;
+  {
+    const int nvec = L / 2;                            // int4 vectors in the whole book
+    int4* sbook4 = reinterpret_cast<int4*>(book);
+    if (P.fresh) {
+      for (int i = tid; i < nvec; i += T) sbook4[i] = make_int4(0, 0, 0, 0);
+    } else {
+      const int4* gbook4 = reinterpret_cast<const int4*>(gbook);
+      const int nside = L / 4;
+      for (int i = tid; i < nvec; i += T) {
+        int4 v = __ldg(gbook4 + i);
+        sbook4[i] = v;
+        int vals[4] = {v.x, v.y, v.z, v.w};
+        if (i < nside) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) { sb0 += vals[j]; if (vals[j] > 0) bmax = max(bmax, 4 * i + j); }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) { sa0 += vals[j]; if (vals[j] > 0) amin = min(amin, 4 * (i - nside) + j); }
+        }
+      }
+    }
+    if (tid < 16) s_rec[tid] = grec[tid];
+  }
+  BookTotals tot0 = block_reduce_totals(sb0, sa0, bmax, amin, s_red64, s_red32);   // has barriers
+  bmax = tot0.bmax;                       // only warp 0 keeps these up to date below
+  amin = min(tot0.amin, L);
+  int last = (int)s_rec[F_LAST], prev = (int)s_rec[F_PREV];
+  const uint32_t t0 = (uint32_t)s_rec[F_STEPS];
+  const long long vol0 = s_rec[F_SUMVOL];
+
+  int sink = 0;                           // only used by the ATOM == 2 microbenchmark variant
+  // ---- S steps, all on-chip
+  for (long long s = 0; s < P.S; ++s) {
+    const uint32_t t = t0 + (uint32_t)s;
+    const StepUniform u = step_uniform(P, market, t);
+    // a1 + a2: order generation and aggregation
+    generate_step<MODEL, ATOM>(P, book, u, last, prev, tid, T, sink);
+    __syncthreads();                                   // B1: the combined book is complete
+
+    // a3-a6: clearing by warp 0 on the active window
+    if (warp == 0) {
+      int lo = max(0, min(amin, last - P.dmax));
+      int hi = min(L - 1, max(bmax, last + P.dmax));
+      int vmax, pstar, nb, na;
+      int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
+      if (P.force_generic || width8 > 256) clear_generic(book, L, lo & ~3, hi, lane, vmax, pstar, nb, na);
+      else if (width4 <= 128)              clear_window<4>(book, L, lo & ~3, lane, vmax, pstar, nb, na);
+      else                                 clear_window<8>(book, L, lo & ~7, lane, vmax, pstar, nb, na);
+      bmax = nb; amin = na;
+      if (lane == 0) {
+        int new_last;
+        update_record(s_rec, last, vmax, pstar, new_last);
+        s_ctl[0] = new_last;
+      }
+    }
+    __syncthreads();                                   // B2: residual book and new price visible
+    prev = last;
+    last = s_ctl[0];
+  }
+
+  // ---- a7: write-back (shared -> HBM), 16-byte vectors, plus the totals for sub_buy/sub_sell
+  long long sb1 = 0, sa1 = 0;
+  {
+    const int nvec = L / 2, nside = L / 4;
+    const int4* sbook4 = reinterpret_cast<const int4*>(book);
+    int4* gbook4 = reinterpret_cast<int4*>(gbook);
+    for (int i = tid; i < nvec; i += T) {
+      int4 v = sbook4[i];
+      gbook4[i] = v;
+      long long sum = (long long)v.x + v.y + v.z + v.w;
+      if (i < nside) sb1 += sum; else sa1 += sum;
+    }
+  }
+  BookTotals tot1 = block_reduce_totals(sb1, sa1, -1, 0x7fffffff, s_red64, s_red32);
+  if (tid == 0) {
+    // submitted = (resting after - resting before) + executed during this run (conservation;
+    // the oracle counts the same quantity order by order)
+    long long dvol = s_rec[F_SUMVOL] - vol0;
+    s_rec[F_SUBBUY] += (tot1.sum_bid - tot0.sum_bid) + dvol;
+    s_rec[F_SUBSELL] += (tot1.sum_ask - tot0.sum_ask) + dvol;
+    s_rec[F_NORDERS] += P.S * P.orders_per_step;
+  }
+  __syncthreads();
+  if (tid < 16) grec[tid] = s_rec[tid];
+}
+
+// ks_create: empty books, opening price, zero accumulators (Alg.1 l.2-3).
+__global__ void ks_init_kernel(int4* books4, size_t nvec, long long* recs, int M, int init_price) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t v = i; v < nvec; v += stride) books4[v] = make_int4(0, 0, 0, 0);
+  for (size_t r = i; r < (size_t)M * 16; r += stride) {
+    int f = (int)(r & 15);
+    long long val = 0;
+    if (f == F_LAST || f == F_PREV) val = init_price;
+    if (f == F_HASH) val = (long long)kHashBasis;
+    recs[r] = val;
+  }
+}
+
+// ks_write_books depth check: max over markets and sides of the total depth -> *out (atomicMax).
+__global__ void ks_depth_bound_kernel(const int32_t* books, int L, unsigned long long* out) {
+  const int32_t* side = books + (size_t)blockIdx.x * (size_t)L;      // grid = 2*M sides
+  long long sum = 0; int neg = 0;
+  for (int i = threadIdx.x; i < L; i += blockDim.x) { int v = side[i]; sum += v; neg |= (v < 0); }
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  neg = __any_sync(0xffffffffu, neg);
+  __shared__ long long s[32];
+  __shared__ int sneg;
+  if (threadIdx.x == 0) sneg = 0;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) { s[threadIdx.x >> 5] = sum; if (neg) sneg = 1; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    long long tot = 0;
+    for (int w = 0; w < (int)((blockDim.x + 31) >> 5); ++w) tot += s[w];
+    unsigned long long v = sneg ? 0xffffffffffffffffull : (unsigned long long)tot;
+    atomicMax(out, v);
+  }
+}
+
+}  // namespace ks

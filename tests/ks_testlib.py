@@ -71,3 +71,42 @@ def greedy_match(bid, ask):
         a[lo] -= x
         vol += x
     return vol, np.array(b, dtype=np.int64), np.array(a, dtype=np.int64)
+
+
+def oracle_rows(oracle, params, L, A, seed, ids, S, books=None, recs=None, threads=None):
+    """Run the (single-threaded) oracle on the markets `ids`, one independent oracle call per
+    host thread over disjoint id ranges (markets are independent; ctypes releases the GIL)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    ids = np.asarray(ids, dtype=np.uint32)
+    n = len(ids)
+    threads = max(1, min(threads or (os.cpu_count() or 1), n))
+    cuts = np.linspace(0, n, threads + 1).astype(int)
+
+    def job(k):
+        lo, hi = cuts[k], cuts[k + 1]
+        if lo == hi:
+            return None
+        b = None if books is None else books[lo:hi]
+        r = None if recs is None else recs[lo:hi]
+        return oracle.run_markets(params, L, A, seed, ids[lo:hi], S, b, r)
+
+    with ThreadPoolExecutor(threads) as ex:
+        parts = [p for p in ex.map(job, range(threads)) if p is not None]
+    return np.concatenate([p[0] for p in parts]), np.concatenate([p[1] for p in parts])
+
+
+def assert_rows_equal(gpu_books, gpu_recs, ids, exp_books, exp_recs, what=""):
+    """Bit-exact comparison of the sampled rows: books, prices, every integer sum and the hash."""
+    ids = np.asarray(ids, dtype=np.int64)
+    gb, gr = gpu_books[ids], gpu_recs[ids]
+    if not np.array_equal(gr, exp_recs):
+        bad = np.argwhere(gr != exp_recs)
+        i, f = bad[0]
+        raise AssertionError("%s: record mismatch at market %d field %d: gpu %d oracle %d (%d mismatches)"
+                             % (what, ids[i], f, gr[i, f], exp_recs[i, f], len(bad)))
+    if not np.array_equal(gb, exp_books):
+        bad = np.argwhere(gb != exp_books)
+        i, s, p = bad[0]
+        raise AssertionError("%s: book mismatch at market %d side %d tick %d: gpu %d oracle %d (%d mismatches)"
+                             % (what, ids[i], s, p, gb[i, s, p], exp_books[i, s, p], len(bad)))

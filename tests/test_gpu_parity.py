@@ -1,0 +1,192 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on
+the same seeded configurations -- bit-exact on books, clearing prices (trajectory hash), every
+integer sum; derived fp64 statistics within 1e-12 relative (north_star)."""
+import numpy as np
+import pytest
+
+from ks_testlib import assert_rows_equal, ints, oracle_rows, read_golden
+from paper_2606_21784_b200.workloads import (CONFIGS, mix3_params, random_books, sampled_markets, zi_params)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ks():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_21784_b200 import binding
+    binding.load()          # raises if the CUDA library is not built: no fallback
+    return binding
+
+
+def _gpu(ks, M, L, A, params, seed, S, *, opts=(), market_base=0, books=None, split=None, stepwise=False):
+    import torch
+    sim = ks.KsSim(M, L, A, params, seed, market_base=market_base)
+    for o, v in opts:
+        sim.ks_set_option(o, v)
+    if books is not None:
+        sim.ks_write_books(torch.from_numpy(np.ascontiguousarray(books)).cuda())
+    for s in (split or [S]):
+        (sim.ks_run_stepwise if stepwise else sim.ks_run)(s)
+    b, r = sim.books_to_host(), sim.stats_to_host()
+    sim.ks_destroy()
+    return b, r
+
+
+def _check_derived(ks, oracle, recs):
+    got = ks.ks_derive_stats(recs)
+    exp = np.stack([oracle.derived(r) for r in recs])
+    assert np.array_equal(np.isnan(got), np.isnan(exp))
+    m = ~np.isnan(exp)
+    assert np.all(np.abs(got[m] - exp[m]) <= 1e-12 * np.abs(exp[m]))
+
+
+# ------------------------------------------------------------------ the five BASELINE configs
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+def test_config_all_markets(ks, oracle, name):
+    """C1-C3 at full size, every market (C2 is ~1e9 agent events for the oracle)."""
+    c = CONFIGS[name]
+    b, r = _gpu(ks, c.M, c.L, c.A, c.params, c.seed, c.S)
+    ids = np.arange(c.M)
+    eb, er = oracle_rows(oracle, c.params, c.L, c.A, c.seed, ids, c.S)
+    assert_rows_equal(b, r, ids, eb, er, name)
+    _check_derived(ks, oracle, r)
+
+
+@pytest.mark.parametrize("name", ["C4", "C5"])
+def test_config_sampled_markets(ks, oracle, name):
+    """C4/C5 at BASELINE.json's full size in the launch configuration bench.py times; the oracle
+    runs the 64 seeded sampled markets (ids 0, M-1 and 62 SplitMix64 draws)."""
+    c = CONFIGS[name]
+    b, r = _gpu(ks, c.M, c.L, c.A, c.params, c.seed, c.S)
+    ids = sampled_markets(c.M, c.seed, 64)
+    eb, er = oracle_rows(oracle, c.params, c.L, c.A, c.seed, ids, c.S)
+    assert_rows_equal(b, r, ids, eb, er, name)
+    _check_derived(ks, oracle, r[ids.astype(np.int64)])
+    # properties that hold for every market at any size
+    r64 = r.astype(np.int64)
+    assert (r64[:, 0] == c.S).all() and (r64[:, 1] <= c.S).all()
+    assert (b >= 0).all()
+    tot = b.astype(np.int64).sum(axis=2)
+    assert (r64[:, 10] == r64[:, 2] + tot[:, 0]).all() and (r64[:, 11] == r64[:, 2] + tot[:, 1]).all()
+
+
+# ------------------------------------------------------------------ equivalences
+@pytest.mark.parametrize("model", ["zi", "mix3"])
+def test_block_sizes_atomic_modes_and_clear_paths_give_identical_bytes(ks, oracle, model):
+    """Integer quantities make accumulation order irrelevant: any block size, the
+    warp-aggregated atomics and the chunked general scan must give the same bytes as the oracle.
+    Ragged sizes: A is not a multiple of the block size or of 3."""
+    if model == "zi":
+        M, L, A, S, seed, p = 37, 256, 1000, 120, 9, zi_params(16, 100)
+    else:
+        M, L, A, S, seed, p = 21, 1024, 1541, 90, 4, mix3_params()
+    ids = np.arange(M)
+    eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+    for T in (32, 64, 96, 128, 256, 512, 1024):
+        for atom in (0, 1):
+            for clear in (0, 1):
+                if T not in (96, 256) and (atom or clear):
+                    continue
+                b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T),
+                                                            (ks.KS_OPT_ATOMIC_MODE, atom),
+                                                            (ks.KS_OPT_CLEAR_PATH, clear)])
+                assert_rows_equal(b, r, ids, eb, er, "T=%d atom=%d clear=%d" % (T, atom, clear))
+
+
+def test_split_run_and_stepwise_ablation_are_bit_identical(ks, oracle):
+    """ks_run(S1); ks_run(S2) == ks_run(S1+S2); the launch-per-step ablation (a8) == persistent."""
+    c = CONFIGS["C3"]
+    S = 300
+    ids = np.arange(c.M)
+    eb, er = oracle_rows(oracle, c.params, c.L, c.A, c.seed, ids, S)
+    b1, r1 = _gpu(ks, c.M, c.L, c.A, c.params, c.seed, S)
+    b2, r2 = _gpu(ks, c.M, c.L, c.A, c.params, c.seed, S, split=[1, 99, 200])
+    b3, r3 = _gpu(ks, c.M, c.L, c.A, c.params, c.seed, S, stepwise=True)
+    for b, r, what in [(b1, r1, "one run"), (b2, r2, "split"), (b3, r3, "stepwise")]:
+        assert_rows_equal(b, r, ids, eb, er, what)
+    m = mix3_params()
+    eb, er = oracle_rows(oracle, m, 512, 700, 4, np.arange(5), 64)
+    b, r = _gpu(ks, 5, 512, 700, m, 4, 64, split=[7, 57])
+    assert_rows_equal(b, r, np.arange(5), eb, er, "mix3 split")
+    b, r = _gpu(ks, 5, 512, 700, m, 4, 64, stepwise=True)
+    assert_rows_equal(b, r, np.arange(5), eb, er, "mix3 stepwise")
+
+
+def test_market_base_shards_reproduce_the_global_run(ks, oracle):
+    """S8(e): a shard created with market_base = b computes markets b..b+M-1 of the global run."""
+    c = CONFIGS["C2"]
+    S = 40
+    bg, rg = _gpu(ks, 64, c.L, c.A, c.params, c.seed, S)
+    b0, r0 = _gpu(ks, 24, c.L, c.A, c.params, c.seed, S)
+    b1, r1 = _gpu(ks, 40, c.L, c.A, c.params, c.seed, S, market_base=24)
+    assert np.array_equal(np.concatenate([b0, b1]), bg) and np.array_equal(np.concatenate([r0, r1]), rg)
+    eb, er = oracle_rows(oracle, c.params, c.L, c.A, c.seed, np.arange(24, 64), S)
+    assert_rows_equal(b1, r1, np.arange(40), eb, er, "shard with market_base")
+
+
+# ------------------------------------------------------------------ book injection / edge cases
+def test_paper_worked_example_through_the_library(ks):
+    """PAPER.md:315-354 (Eq.11-18) embedded at ticks 10..14 of an L=32 grid, A = 0: zero padding
+    leaves p*, Vmax and the residual books unchanged."""
+    ex = read_golden("paper_worked_example.txt")[0]
+    books = np.zeros((3, 2, 32), dtype=np.int32)
+    books[1, 0, 10:15] = ints(ex, "BUY"); books[1, 1, 10:15] = ints(ex, "SELL")
+    b, r = _gpu(ks, 3, 32, 0, zi_params(1, 1), 0, 1, books=books)
+    assert list(b[1, 0, 10:15]) == list(ints(ex, "new_bid")) and list(b[1, 1, 10:15]) == list(ints(ex, "new_ask"))
+    assert b[1].sum() == ints(ex, "new_bid").sum() + ints(ex, "new_ask").sum()
+    assert r[1, 12] == 10 + int(ex["pstar"][0]) and r[1, 2] == int(ex["vmax"][0]) and r[1, 1] == 1
+    assert r[0, 1] == 0 and r[0, 12] == 16 and (b[0] == 0).all()          # empty market: no trade
+
+
+@pytest.mark.parametrize("L,A,model", [(32, 0, "zi"), (64, 77, "zi"), (2048, 300, "mix3"), (4096, 0, "zi")])
+def test_random_injected_books(ks, oracle, L, A, model):
+    """Arbitrary (crossed, wide) resting books written with ks_write_books: the first step clears a
+    window as wide as the grid (chunked general scan), later steps the narrow one."""
+    M, S, seed = 9, 6, 12
+    p = zi_params(min(8, L // 4), 10) if model == "zi" else mix3_params()
+    books = random_books(M, L, seed=L + A, max_qty=40, fill=0.3)
+    books[0] = 0                                   # empty market
+    books[1, 1] = 0                                # one-sided market
+    books[2] = random_books(1, L, seed=1, crossed=False)[0]
+    eb0, er0 = oracle.init_state(M, L, -1)
+    eb, er = oracle_rows(oracle, p, L, A, seed, np.arange(M), S, books=books, recs=er0)
+    for clear in (0, 1):
+        b, r = _gpu(ks, M, L, A, p, seed, S, books=books, opts=[(ks.KS_OPT_CLEAR_PATH, clear)])
+        assert_rows_equal(b, r, np.arange(M), eb, er, "injected L=%d clear=%d" % (L, clear))
+
+
+def test_price_pinned_to_grid_edge(ks, oracle):
+    """init_price at the edges: clamped orders pile on ticks 0 / L-1 (A15) and the clamp path of
+    the generator is exercised."""
+    for init in (0, 63, 3):
+        p = zi_params(8, 10, init_price=init)
+        eb, er = oracle_rows(oracle, p, 64, 200, 5, np.arange(4), 50)
+        b, r = _gpu(ks, 4, 64, 200, p, 5, 50)
+        assert_rows_equal(b, r, np.arange(4), eb, er, "init_price=%d" % init)
+    p = mix3_params(init_price=1)
+    eb, er = oracle_rows(oracle, p, 128, 333, 6, np.arange(3), 40)
+    b, r = _gpu(ks, 3, 128, 333, p, 6, 40)
+    assert_rows_equal(b, r, np.arange(3), eb, er, "mix3 at the edge")
+
+
+def test_max_grid_and_overflow_guards(ks, oracle):
+    """L = 16384 (the single-CTA maximum); KS_ERR_OVERFLOW before a run that could pass 2^31."""
+    p = zi_params(300, 7)
+    eb, er = oracle_rows(oracle, p, 16384, 500, 3, np.arange(2), 12)
+    b, r = _gpu(ks, 2, 16384, 500, p, 3, 12)
+    assert_rows_equal(b, r, np.arange(2), eb, er, "L=16384")
+    sim = ks.KsSim(1, 64, 4096, zi_params(8, 1 << 20), 0)
+    with pytest.raises(ks.KsError) as e:
+        sim.ks_run(1)
+    assert e.value.status == ks.KS_ERR_OVERFLOW
+    sim.ks_run(0)
+    assert sim.stats_to_host()[0, 0] == 0
+    sim.ks_destroy()
+
+
+def test_run_to_run_determinism(ks):
+    c = CONFIGS["C2"]
+    a = _gpu(ks, 256, c.L, c.A, c.params, c.seed, 50)
+    b = _gpu(ks, 256, c.L, c.A, c.params, c.seed, 50)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])

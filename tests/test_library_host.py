@@ -1,0 +1,109 @@
+"""Host-side checks of the C-ABI library that need no GPU: it builds for sm_100a, loads, exports
+every symbol the headers declare (and nothing else), validates arguments before touching CUDA,
+fails loudly without a device, and its fp64 derivation agrees with the oracle's on equal integers."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_2606_21784_b200 import binding, build
+from paper_2606_21784_b200.workloads import CONFIGS, zi_params
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load()
+
+
+def _declared():
+    names = []
+    for h in ("kineticsim.h", "kineticsim_bench.h"):
+        src = open(os.path.join(ROOT, "include", h)).read()
+        names += re.findall(r"KS_API\s+[\w\s\*]+?\b(ks_\w+)\s*\(", src)
+    return names
+
+
+def test_headers_declare_what_the_binding_lists():
+    assert sorted(_declared()) == sorted(binding.EXPORTS)
+
+
+def test_library_exports_every_declared_symbol(lib):
+    out = subprocess.check_output(["nm", "-D", "--defined-only", binding.LIB_PATH]).decode()
+    exported = {l.split()[-1] for l in out.splitlines() if " T " in l}
+    ks = {s for s in exported if s.startswith("ks_")}
+    assert ks == set(_declared())
+    for n in _declared():
+        assert getattr(lib, n) is not None
+
+
+def test_library_is_sm100a_with_shared_atomics():
+    """The cubin inside the library targets sm_100a and the persistent kernel uses ATOMS (shared
+    atomics) and REDUX (warp reductions) -- i.e. the hot path is in the kernel, not on the host."""
+    out = subprocess.check_output(["cuobjdump", "-sass", binding.LIB_PATH]).decode()
+    assert "sm_100a" in out
+    body = out.split("ks_persistent_kernel")[1]
+    assert "ATOMS" in body and "REDUX" in body and "IMAD.WIDE.U32" in body
+
+
+def test_state_bytes(lib):
+    assert binding.ks_state_bytes(1, 64) == 1 * (8 * 64 + 128) + 256
+    assert binding.ks_state_bytes(65536, 512) == 65536 * (8 * 512 + 128) + 256
+    for M, L in [(0, 64), (1, 48), (1, 16), (-3, 64), (1, 65536)]:
+        assert binding.ks_state_bytes(M, L) == 0
+
+
+def test_argument_validation_precedes_cuda(lib):
+    h = C.c_void_p(None)
+    P = binding._params(zi_params(8, 10))
+    fake = 0x1000   # never dereferenced: every call below must fail before any CUDA work
+    assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(P), 0, None, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_create(None, 1, 64, 256, C.byref(P), 0, fake, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_create(C.byref(h), 1, 48, 256, C.byref(P), 0, fake, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_create(C.byref(h), 0, 64, 256, C.byref(P), 0, fake, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_create(C.byref(h), 1, 64, -1, C.byref(P), 0, fake, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(P), 0, fake + 4, None) == binding.KS_ERR_INVALID_ARG
+    bad = binding._params(zi_params(8, 0))
+    assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(bad), 0, fake, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_create(C.byref(h), 1, 32768, 256, C.byref(P), 0, fake, None) == binding.KS_ERR_UNSUPPORTED
+    assert h.value is None
+    assert lib.ks_run(None, 1, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_read_books(None, None, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_set_option(None, 0, 0) == binding.KS_ERR_INVALID_ARG
+    assert b"NULL" in lib.ks_last_error()
+    lib.ks_destroy(None)
+
+
+def test_no_cpu_fallback_without_a_device(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = C.c_void_p(None)
+    P = binding._params(zi_params(8, 10))
+    assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(P), 0, 0x1000, None) == binding.KS_ERR_CUDA
+    assert h.value is None and len(lib.ks_last_error()) > 0
+    ops, sec = C.c_double(0), C.c_double(0)
+    assert lib.ks_bench_int_pipe(0, 256, 1, 1, 0, 1, None, C.byref(ops), C.byref(sec)) == binding.KS_ERR_CUDA
+
+
+def test_derive_stats_matches_oracle_on_equal_integers(lib, oracle):
+    c = CONFIGS["C1"]
+    _, recs = oracle.run_markets(c.params, c.L, c.A, c.seed, [0, 1, 2], 80)
+    recs = np.vstack([recs, oracle.init_state(1, 64)[1]])       # a record with zero steps -> NaNs
+    got = binding.ks_derive_stats(recs)
+    exp = np.stack([oracle.derived(r) for r in recs])
+    assert np.array_equal(np.isnan(got), np.isnan(exp)) and np.isnan(got[-1]).all()
+    m = ~np.isnan(exp)
+    assert np.all(np.abs(got[m] - exp[m]) <= 1e-12 * np.abs(exp[m]))
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libkineticsim.so")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.load()
