@@ -44,7 +44,7 @@ struct ks_sim {
   int64_t steps_done;
   int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear;
+  int32_t opt_threads, opt_atomic, opt_clear, opt_table;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
   // ks_write_books depth check
@@ -109,7 +109,7 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   if (!s) { set_err("ks_create: out of host memory"); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
   s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_table = -1;
   s->dev_smem_optin = optin; s->num_sms = sms;
   s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_ZI) {
@@ -168,6 +168,9 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_CLEAR_PATH:
       if (value != 0 && value != 1) break;
       s->opt_clear = value; return KS_OK;
+    case KS_OPT_TABLE_AGENTS:
+      if (value < -1) break;
+      s->opt_table = value; return KS_OK;
     default: break;
   }
   set_err("ks_set_option: unknown option or value");
@@ -176,20 +179,55 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 
 }  // extern "C"
 
-// Threads per CTA.  Throughput regime (M CTAs oversubscribe the GPU): small CTAs so that many
-// markets are co-resident and one market's barrier/clearing phase hides behind another's
-// generation.  Few markets: widen the CTA so the whole GPU is used, but never beyond the agents.
-static int pick_threads(const ks_sim* s) {
-  if (s->opt_threads) return s->opt_threads;
-  const long long resident_threads = (long long)s->num_sms * 2048;
+// Launch plan: threads per CTA, agents covered by the shared-memory Philox table, dynamic
+// shared memory.  An SM has 228 KB of shared memory; each resident CTA costs its dynamic + static
+// allocation + 1 KB of system reserve.
+//  * Table: all A agents when that still leaves >= 3 CTAs per SM (or as many as the grid can
+//    give an SM); otherwise the largest table that keeps 2 CTAs per SM, so that one market's
+//    clearing phase (one warp) hides behind another market's generation; a book too large for
+//    that runs 1 CTA per SM.
+//  * Threads: few markets -> widen the CTA so the whole GPU is used, but never beyond the
+//    agents; many markets -> at least ~1024 resident threads per SM.
+struct LaunchPlan { int T; int n_tab; size_t smem; };
+
+static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
+
+static LaunchPlan plan_launch(const ks_sim* s) {
+  LaunchPlan pl;
+  const long long book = 8LL * s->L;
+  const long long max_cta = (long long)s->dev_smem_optin - 1024;       // static shared memory
+  auto ctas_for = [&](long long dyn) { return (int)(kSmemPerSM / (dyn + kSmemCtaOverhead)); };
+  auto tab_for = [&](int k) {                                            // largest table with k CTAs per SM
+    long long dyn = kSmemPerSM / k - kSmemCtaOverhead;
+    if (dyn > max_cta) dyn = max_cta;
+    long long n = (dyn - book) / 12;
+    return (int)(n < 0 ? 0 : (n > s->A ? s->A : n));
+  };
+  const int per_sm = (s->M + s->num_sms - 1) / s->num_sms;              // CTAs the grid can give one SM
+  int n_tab;
+  if (s->opt_table >= 0) {
+    n_tab = s->opt_table < tab_for(1) ? s->opt_table : tab_for(1);
+  } else {
+    const int want = per_sm < 3 ? per_sm : 3;
+    if (book + 12LL * s->A <= max_cta && ctas_for(book + 12LL * s->A) >= want) n_tab = s->A;
+    else if (ctas_for(book) >= 2) n_tab = tab_for(2);
+    else n_tab = tab_for(1);
+  }
+  pl.n_tab = n_tab;
+  pl.smem = (size_t)(book + 12LL * n_tab);
+  const int k = ctas_for((long long)pl.smem) < 1 ? 1 : ctas_for((long long)pl.smem);
+
   int T = 128;
-  while (T < 1024 && (long long)s->M * (T * 2) <= resident_threads && T * 2 <= s->A) T *= 2;
-  // the book must leave room for several CTAs per SM; with a large book prefer wider CTAs
-  const long long smem_per_cta = 8LL * s->L + 1536;
-  long long ctas_by_smem = (228LL * 1024) / smem_per_cta;
-  if (ctas_by_smem < 1) ctas_by_smem = 1;
-  while (T < 1024 && ctas_by_smem * T < 1536 && T * 2 <= (s->A > 32 ? s->A : 32)) T *= 2;
-  return T;
+  if (s->opt_threads) {
+    T = s->opt_threads;
+  } else {
+    const long long resident_threads = (long long)s->num_sms * 2048;
+    const int a_cap = s->A > 32 ? s->A : 32;
+    while (T < 1024 && (long long)s->M * (T * 2) <= resident_threads && T * 2 <= a_cap) T *= 2;
+    while (T < 1024 && (long long)k * T < 1024 && T * 2 <= a_cap) T *= 2;
+  }
+  pl.T = T;
+  return pl;
 }
 
 template <int MODEL, int ATOM>
@@ -230,6 +268,7 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += ks::kPhiloxW0; k1 += ks::kPhiloxW1; }
   P.M = s->M; P.L = s->L; P.A = s->A; P.market_base = s->market_base;
   P.noise_delta = s->p.noise_delta; P.noise_n = 2 * s->p.noise_delta + 1; P.noise_qmax = s->p.noise_qmax;
+  P.noise_n4 = 4 * P.noise_n; P.q_addend = 1ull << 32;
   P.maker_spread_max = s->p.maker_spread_max; P.maker_qty = s->p.maker_qty;
   P.mom_n = s->p.mom_delta + 1; P.mom_qmax = s->p.mom_qmax;
   P.dmax = s->p.noise_delta;
@@ -242,8 +281,10 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   P.S = S;
   P.orders_per_step = (long long)s->A + s->n_maker;
 
-  const int T = pick_threads(s);
-  const size_t smem = (size_t)8 * s->L;
+  const LaunchPlan pl = plan_launch(s);
+  const int T = pl.T;
+  const size_t smem = pl.smem;
+  P.n_tab = pl.n_tab;
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
   if (s->p.model == KS_MODEL_ZI)

@@ -38,11 +38,14 @@ struct KernelParams {
   int32_t M, L, A;
   uint32_t market_base;
   int32_t noise_delta, noise_n, noise_qmax;      // noise_n = 2*delta+1
+  int32_t noise_n4;                               // 4*noise_n
+  unsigned long long q_addend;                    // 2^32: the "+1" of q = 1 + mulhi(w, qmax), as an IMAD addend
   int32_t maker_spread_max, maker_qty;
   int32_t mom_n, mom_qmax;                        // mom_n = mom_delta+1
   int32_t dmax;                                   // largest |tick - last| any rule can produce
   int32_t fresh;                                  // books are known to be all zero: skip the load
   int32_t force_generic;                          // ablation/test: always use the chunked scan
+  int32_t n_tab;                                  // agents [0, n_tab) start from the shared-memory table
   long long S;                                    // steps to run
   long long orders_per_step;                      // A + number of makers
 };
@@ -50,41 +53,74 @@ struct KernelParams {
 __device__ __forceinline__ uint32_t hi32(uint64_t x) { return (uint32_t)(x >> 32); }
 __device__ __forceinline__ uint32_t lo32(uint64_t x) { return (uint32_t)x; }
 
-// Values of the first two Philox rounds that do not depend on the agent.
-// Round 0 on ctr = (a, t, m, 0):  n0 = hi(M1*m) ^ t ^ k0[0], n1 = lo(M1*m)      (uniform)
-//                                 n2 = hi(M0*a) ^ k1[0],     n3 = lo(M0*a)      (per agent)
-// Round 1 on (n0, n1, n2, n3):    d0 = hi(M1*n2) ^ n1 ^ k0[1], d1 = lo(M1*n2)   (per agent)
-//                                 d2 = hi(M0*n0) ^ n3 ^ k1[1], d3 = lo(M0*n0)   (d3 uniform)
-struct StepUniform {
-  uint32_t n1k;   // n1 ^ k0[1]
-  uint32_t d2x;   // hi(M0*n0) ^ k1[1]
-  uint32_t d3;    // lo(M0*n0)
+// ---------------------------------------------------------------------------------------------
+// a1: Philox4x32-10 on ctr = (agent a, step t, market m, 0), with everything that does not
+// depend on all three of (a, t, m) hoisted out of the per-event work.
+//   round 0:  n0 = hi(M1*m) ^ t ^ k0[0]        (m, t)      n1 = lo(M1*m)              (m)
+//             n2 = hi(M0*a) ^ k1[0]            (a)         n3 = lo(M0*a)              (a)
+//   round 1:  c0 = hi(M1*n2) ^ n1 ^ k0[1]      (a, m)      c1 = lo(M1*n2)             (a)
+//             c2 = hi(M0*n0) ^ n3 ^ k1[1]      (a, m, t)   c3 = lo(M0*n0)             (m, t)
+// so per (market, agent) the triple (c0, c1, n3) is constant over all S steps: it is computed
+// once per launch into a shared-memory table (AgentTable) and each event starts at round 2 with
+// one LDS.64 + one LDS.32 + one LOP3 instead of two 32x32->64 multiplies.  The multiplies are
+// what bounds the kernel (IMAD.WIDE runs at a quarter of the LOP3/IADD rate), so per event the
+// path issues 15 IMAD.WIDE + 1 IMAD.HI for rounds 2..9 and 2 IMAD.HI for the agent rule.
+// ---------------------------------------------------------------------------------------------
+struct MarketUniform {   // depends on the market only
+  uint32_t hm;     // hi(M1*m)
+  uint32_t n1k;    // lo(M1*m) ^ k0[1]
+};
+struct StepUniform {     // depends on (market, step)
+  uint32_t d2x;    // hi(M0*n0) ^ k1[1]
+  uint32_t d3;     // lo(M0*n0)
+  uint32_t d3k;    // d3 ^ k1[2]: round 2 xors two uniform words into hi(M0*c0); pre-xored here
 };
 
-__device__ __forceinline__ StepUniform step_uniform(const KernelParams& P, uint32_t market, uint32_t t) {
+__device__ __forceinline__ MarketUniform market_uniform(const KernelParams& P, uint32_t market) {
   uint64_t pm = (uint64_t)kPhiloxM1 * market;
-  uint32_t n0 = hi32(pm) ^ t ^ P.k0[0];
+  MarketUniform mu;
+  mu.hm = hi32(pm);
+  mu.n1k = lo32(pm) ^ P.k0[1];
+  return mu;
+}
+
+__device__ __forceinline__ StepUniform step_uniform(const KernelParams& P, const MarketUniform& mu, uint32_t t) {
+  uint32_t n0 = mu.hm ^ t ^ P.k0[0];
   uint64_t q0 = (uint64_t)kPhiloxM0 * n0;
   StepUniform u;
-  u.n1k = lo32(pm) ^ P.k0[1];
   u.d2x = hi32(q0) ^ P.k1[1];
   u.d3 = lo32(q0);
+  u.d3k = u.d3 ^ P.k1[2];
   return u;
 }
 
-// Philox4x32-10 block of agent a; returns output words w0, w1, w2 (w3 is reserved, unused).
-__device__ __forceinline__ void philox_agent(const KernelParams& P, const StepUniform& u, uint32_t a,
-                                             uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+// (c0, c1, n3) of agent a in market mu -- the table entry, also used directly for agents beyond
+// the table.
+__device__ __forceinline__ void agent_rounds01(const KernelParams& P, const MarketUniform& mu, uint32_t a,
+                                               uint32_t& c0, uint32_t& c1, uint32_t& n3) {
   uint64_t p0 = (uint64_t)kPhiloxM0 * a;
   uint32_t n2 = hi32(p0) ^ P.k1[0];
-  uint32_t n3 = lo32(p0);
+  n3 = lo32(p0);
   uint64_t p1 = (uint64_t)kPhiloxM1 * n2;
-  uint32_t c0 = hi32(p1) ^ u.n1k;
-  uint32_t c1 = lo32(p1);
-  uint32_t c2 = u.d2x ^ n3;
-  uint32_t c3 = u.d3;
+  c0 = hi32(p1) ^ mu.n1k;
+  c1 = lo32(p1);
+}
+
+// Rounds 2..9 from (c0, c1, c2, c3 = u.d3).  Outputs w0, w1, w2 (w3 is reserved and never
+// computed).  NEED02 = false skips the last round's M0 product (the maker rule reads w1 only).
+template <bool NEED02>
+__device__ __forceinline__ void philox_rounds(const KernelParams& P, const StepUniform& u, uint32_t c0, uint32_t c1,
+                                              uint32_t c2, uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+  uint32_t c3;
+  {                                       // round 2: c3 = d3 is uniform, d3 ^ k1[2] was pre-xored
+    uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
+    uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
+    uint32_t t0 = hi32(a1) ^ c1 ^ P.k0[2];
+    uint32_t t2 = hi32(a0) ^ u.d3k;
+    c1 = lo32(a1); c3 = lo32(a0); c0 = t0; c2 = t2;
+  }
 #pragma unroll
-  for (int r = 2; r < 10; ++r) {
+  for (int r = 3; r < 9; ++r) {
     uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
     uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
     uint32_t t0 = hi32(a1) ^ c1 ^ P.k0[r];
@@ -94,105 +130,178 @@ __device__ __forceinline__ void philox_agent(const KernelParams& P, const StepUn
     c0 = t0;
     c2 = t2;
   }
-  w0 = c0; w1 = c1; w2 = c2;
+  uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
+  w1 = lo32(a1);
+  if (NEED02) {
+    w0 = hi32(a1) ^ c1 ^ P.k0[9];
+    w2 = __umulhi(kPhiloxM0, c0) ^ c3 ^ P.k1[9];
+  } else {
+    w0 = 0; w2 = 0;
+  }
 }
 
-// a2: add one order to the shared-memory book.  ATOM 0: plain atomicAdd (ATOMS.ADD, result
-// unused).  ATOM 1: warp-aggregated -- lanes with the same address elect a leader that adds the
-// group's sum (north_star (3)); kept as an ablation switch.
+// The per-CTA agent table in shared memory: three arrays of n_tab words, c0[], c1[], n3[], for
+// agents [0, n_tab) -- one base register plus uniform offsets addresses all three, and a warp's
+// loads are conflict-free.
+struct AgentTable {
+  uint32_t* w;         // c0 at w[a], c1 at w[n_tab + a], n3 at w[2*n_tab + a]
+  uint32_t n_tab;
+};
+
+__device__ __forceinline__ void table_fill(const KernelParams& P, const MarketUniform& mu, const AgentTable& tab) {
+  for (uint32_t a = threadIdx.x; a < tab.n_tab; a += blockDim.x) {
+    uint32_t c0, c1, n3;
+    agent_rounds01(P, mu, a, c0, c1, n3);
+    tab.w[a] = c0; tab.w[tab.n_tab + a] = c1; tab.w[2 * tab.n_tab + a] = n3;
+  }
+}
+
+template <bool NEED02>
+__device__ __forceinline__ void philox_agent(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
+                                             const AgentTable& tab, bool tabled, uint32_t a,
+                                             uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+  uint32_t c0, c1, n3;
+  if (tabled) { c0 = tab.w[a]; c1 = tab.w[tab.n_tab + a]; n3 = tab.w[2 * tab.n_tab + a]; }
+  else        agent_rounds01(P, mu, a, c0, c1, n3);
+  philox_rounds<NEED02>(P, u, c0, c1, u.d2x ^ n3, w0, w1, w2);
+}
+
+// a2: add one order to the shared-memory book at byte offset `off` from the start of the book.
+// ATOM 0: plain shared-memory reduction (ATOMS.ADD, result unused).  ATOM 1: warp-aggregated --
+// lanes with the same address elect a leader that adds the group's sum (north_star (3)); kept as
+// an ablation switch.  ATOM 2: microbenchmark only, no memory access.
+struct BookRef {
+  int32_t* ptr;        // generic pointer to the book
+  uint32_t saddr;      // its 32-bit shared-window address
+};
+
 template <int ATOM>
-__device__ __forceinline__ void book_add(int32_t* book, int idx, int q, int& sink) {
+__device__ __forceinline__ void book_add_at(const BookRef& book, uint32_t saddr, int q, int& sink) {
   if (ATOM == 0) {
-    atomicAdd(&book[idx], q);
+    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(saddr), "r"(q) : "memory");
   } else if (ATOM == 2) {
-    sink ^= idx * 131 + q;               // microbenchmark only: no memory access (ks_bench_generate_only)
+    sink ^= (int)saddr * 131 + q;        // no memory access (ks_bench_generate_only)
   } else {
     unsigned act = __activemask();
-    unsigned peers = __match_any_sync(act, idx);
+    unsigned peers = __match_any_sync(act, saddr);
     int sum = __reduce_add_sync(peers, q);
-    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&book[idx], sum);
+    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(book.ptr + ((saddr - book.saddr) >> 2), sum);
   }
+}
+
+template <int ATOM>
+__device__ __forceinline__ void book_add(const BookRef& book, uint32_t off, int q, int& sink) {
+  book_add_at<ATOM>(book, book.saddr + off, q, sink);
 }
 
 __device__ __forceinline__ int clamp_tick(int x, int L) { return min(max(x, 0), L - 1); }
 
-// a1 noise rule.  CLAMP = false is the fast path used when last-delta >= 0 and last+delta <= L-1
-// (a per-step uniform test), where the clamp is the identity.
-template <int ATOM, bool CLAMP>
-__device__ __forceinline__ void noise_order(const KernelParams& P, int32_t* book, int last,
-                                            uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
-  int o = (int)__umulhi(w1, (uint32_t)P.noise_n);
-  int q = 1 + (int)__umulhi(w2, (uint32_t)P.noise_qmax);
-  bool buy = (int32_t)w0 < 0;
-  // buy: last - (o - delta) = (last + delta) - o ; sell: last + (o - delta) = (last - delta) + o
-  int tick = buy ? (last + P.noise_delta) - o : (last - P.noise_delta) + o;
-  if (CLAMP) tick = clamp_tick(tick, P.L);
-  book_add<ATOM>(book, buy ? tick : tick + P.L, q, sink);
-}
+// Per-step values of the rules that are uniform over the CTA.  bid_hi / ask_lo are absolute
+// shared addresses, published once per step by the clearing warp (ks_kernel.cuh, StepCtl) so that
+// no thread recomputes them per order.
+struct RuleCtx {
+  int last, dp, L;
+  bool noclamp;          // last - noise_delta >= 0 and last + noise_delta <= L-1: the noise clamp is the identity
+  uint32_t bid_hi;       // shared address of bid[last + noise_delta]
+  uint32_t ask_lo;       // shared address of ask[last - noise_delta]
+};
 
+// a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; buy tick = last - (o - delta) = (last + delta) - o,
+// sell tick = (last - delta) + o.  4*o is taken as mulhi(w1, 4n) & ~3 (floor(4y) = 4 floor(y) +
+// floor(4 frac(y))), which saves the separate address scaling.  q = 1 + mulhi(w2, qmax) is the
+// high word of w2*qmax + P.q_addend (= 2^32): one IMAD with the +1 folded into its addend.
 template <int ATOM, bool CLAMP>
-__device__ __forceinline__ void generate_noise(const KernelParams& P, int32_t* book, const StepUniform& u,
-                                               int last, uint32_t first, uint32_t a_end, uint32_t a_step,
-                                               int& sink) {
-  // agents first, first+a_step, ... < a_end
-#pragma unroll 4
-  for (uint32_t a = first; a < a_end; a += a_step) {
-    uint32_t w0, w1, w2;
-    philox_agent(P, u, a, w0, w1, w2);
-    noise_order<ATOM, CLAMP>(P, book, last, w0, w1, w2, sink);
+__device__ __forceinline__ void noise_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                            uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
+  const int q = (int)hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend);
+  const bool buy = (int32_t)w0 < 0;
+  if (!CLAMP) {
+    const uint32_t o4 = __umulhi(w1, (uint32_t)P.noise_n4) & ~3u;
+    book_add_at<ATOM>(book, buy ? rc.bid_hi - o4 : rc.ask_lo + o4, q, sink);
+  } else {
+    const int o = (int)__umulhi(w1, (uint32_t)P.noise_n);
+    const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - o : (rc.last - P.noise_delta) + o, rc.L);
+    book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
   }
 }
 
 // a1 maker rule: both sides, fixed quantity; only w1 is used.
 template <int ATOM>
-__device__ __forceinline__ void generate_maker(const KernelParams& P, int32_t* book, const StepUniform& u,
-                                               int last, uint32_t first, uint32_t a_end, uint32_t a_step,
-                                               int& sink) {
-#pragma unroll 2
-  for (uint32_t a = first; a < a_end; a += a_step) {
-    uint32_t w0, w1, w2;
-    philox_agent(P, u, a, w0, w1, w2);
-    int s = 1 + (int)__umulhi(w1, (uint32_t)P.maker_spread_max);
-    book_add<ATOM>(book, clamp_tick(last - s, P.L), P.maker_qty, sink);
-    book_add<ATOM>(book, clamp_tick(last + s, P.L) + P.L, P.maker_qty, sink);
-  }
+__device__ __forceinline__ void maker_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                            uint32_t w1, int& sink) {
+  const int s = 1 + (int)__umulhi(w1, (uint32_t)P.maker_spread_max);
+  book_add<ATOM>(book, 4u * (uint32_t)clamp_tick(rc.last - s, rc.L), P.maker_qty, sink);
+  book_add<ATOM>(book, 4u * (uint32_t)(clamp_tick(rc.last + s, rc.L) + rc.L), P.maker_qty, sink);
 }
 
 // a1 momentum rule: dp = last - prev is uniform over the market-step.
 template <int ATOM>
-__device__ __forceinline__ void generate_momentum(const KernelParams& P, int32_t* book, const StepUniform& u,
-                                                  int last, int dp, uint32_t first, uint32_t a_end,
-                                                  uint32_t a_step, int& sink) {
-#pragma unroll 2
-  for (uint32_t a = first; a < a_end; a += a_step) {
+__device__ __forceinline__ void momentum_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                               uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
+  const bool buy = rc.dp > 0 ? true : (rc.dp < 0 ? false : ((int32_t)w0 < 0));
+  const int o = (int)__umulhi(w1, (uint32_t)P.mom_n);
+  const int q = 1 + (int)__umulhi(w2, (uint32_t)P.mom_qmax);
+  const int tick = clamp_tick(buy ? rc.last + o : rc.last - o, rc.L);
+  book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
+}
+
+// One agent class of one market-step: agents first, first + a_step, ... < a_end, rule KIND
+// (0 noise, 1 maker, 2 momentum).  Agents below tab.n_tab start from the table; the loop over
+// them has a uniform trip count (no per-agent bound check) plus one ragged tail.
+template <int ATOM, int KIND, bool CLAMP>
+__device__ __forceinline__ void generate_class(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                               const StepUniform& u, const AgentTable& tab, const RuleCtx& rc,
+                                               uint32_t first, uint32_t a_end, uint32_t a_step, int& sink) {
+  auto one = [&](uint32_t a, bool tabled) {
     uint32_t w0, w1, w2;
-    philox_agent(P, u, a, w0, w1, w2);
-    bool buy = dp > 0 ? true : (dp < 0 ? false : ((int32_t)w0 < 0));
-    int o = (int)__umulhi(w1, (uint32_t)P.mom_n);
-    int q = 1 + (int)__umulhi(w2, (uint32_t)P.mom_qmax);
-    int tick = clamp_tick(buy ? last + o : last - o, P.L);
-    book_add<ATOM>(book, buy ? tick : tick + P.L, q, sink);
+    philox_agent<KIND != 1>(P, mu, u, tab, tabled, a, w0, w1, w2);
+    if (KIND == 0)      noise_order<ATOM, CLAMP>(P, book, rc, w0, w1, w2, sink);
+    else if (KIND == 1) maker_order<ATOM>(P, book, rc, w1, sink);
+    else                momentum_order<ATOM>(P, book, rc, w0, w1, w2, sink);
+  };
+  const uint32_t t_end = min(a_end, tab.n_tab);
+  uint32_t a = first;
+  if (t_end > first) {
+    // full groups: every thread of the CTA has an agent (first <= first of the last thread)
+    const uint32_t last_first = first - (uint32_t)threadIdx.x * (a_step / blockDim.x) +
+                                (blockDim.x - 1) * (a_step / blockDim.x);
+    const uint32_t nfull = t_end > last_first ? (t_end - last_first + a_step - 1) / a_step : 0u;
+#pragma unroll 2
+    for (uint32_t k = 0; k < nfull; ++k, a += a_step) one(a, true);
+    if (a < t_end) { one(a, true); a += a_step; }
   }
+#pragma unroll 2
+  for (; a < a_end; a += a_step) one(a, false);
 }
 
 // a1 + a2 for one market-step: every thread of the CTA generates the orders of its agents.
 // MODEL 1: agent a = 3j + c has type c; each class runs in its own warp-uniform loop (integer
 // atomics commute, so the agent -> thread mapping cannot change a byte of the result).
 template <int MODEL, int ATOM>
-__device__ __forceinline__ void generate_step(const KernelParams& P, int32_t* book, const StepUniform& u,
-                                              int last, int prev, int tid, int T, int& sink) {
+__device__ __forceinline__ void generate_step(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                              const StepUniform& u, const AgentTable& tab, const RuleCtx& rc,
+                                              int tid, int T, int& sink) {
   const uint32_t A = (uint32_t)P.A;
-  const bool noclamp = (last - P.noise_delta >= 0) && (last + P.noise_delta <= P.L - 1);
   if (MODEL == 0) {
-    if (noclamp) generate_noise<ATOM, false>(P, book, u, last, (uint32_t)tid, A, (uint32_t)T, sink);
-    else         generate_noise<ATOM, true >(P, book, u, last, (uint32_t)tid, A, (uint32_t)T, sink);
+    if (rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, tab, rc, (uint32_t)tid, A, (uint32_t)T, sink);
+    else            generate_class<ATOM, 0, true >(P, book, mu, u, tab, rc, (uint32_t)tid, A, (uint32_t)T, sink);
   } else {
     const uint32_t st = 3u * (uint32_t)T;
-    if (noclamp) generate_noise<ATOM, false>(P, book, u, last, 3u * tid, A, st, sink);
-    else         generate_noise<ATOM, true >(P, book, u, last, 3u * tid, A, st, sink);
-    generate_maker<ATOM>(P, book, u, last, 3u * tid + 1u, A, st, sink);
-    generate_momentum<ATOM>(P, book, u, last, last - prev, 3u * tid + 2u, A, st, sink);
+    if (rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, tab, rc, 3u * tid, A, st, sink);
+    else            generate_class<ATOM, 0, true >(P, book, mu, u, tab, rc, 3u * tid, A, st, sink);
+    generate_class<ATOM, 1, true>(P, book, mu, u, tab, rc, 3u * tid + 1u, A, st, sink);
+    generate_class<ATOM, 2, true>(P, book, mu, u, tab, rc, 3u * tid + 2u, A, st, sink);
   }
+}
+
+// The rule context of a step from the market state (every thread computes the same values).
+__device__ __forceinline__ RuleCtx rule_ctx(const KernelParams& P, const BookRef& book, int last, int prev) {
+  RuleCtx rc;
+  rc.last = last; rc.dp = last - prev; rc.L = P.L;
+  rc.noclamp = (last - P.noise_delta >= 0) && (last + P.noise_delta <= P.L - 1);
+  rc.bid_hi = book.saddr + 4u * (uint32_t)(last + P.noise_delta);
+  rc.ask_lo = book.saddr + 4u * (uint32_t)(P.L + last - P.noise_delta);
+  return rc;
 }
 
 // ---------------------------------------------------------------------------------------------

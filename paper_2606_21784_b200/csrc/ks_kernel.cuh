@@ -60,21 +60,28 @@ __device__ __forceinline__ void update_record(long long* rec, int last, int vmax
 
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
-// dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
+// dynamic shared memory = 8*L bytes (the book) + 12*n_tab bytes (the agent table of
+// ks_device.cuh, n_tab = P.n_tab agents).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
 // ---------------------------------------------------------------------------------------------
 template <int MODEL, int ATOM>
 __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
-  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
+  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then the agent table
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
   __shared__ int s_red32[64];
-  __shared__ int s_ctl[4];                            // last, prev
+  __shared__ __align__(16) int s_ctl[4];              // per-step broadcast: last, &bid[last+delta], &ask[last-delta], noclamp
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
   const int L = P.L;
   const uint32_t market = P.market_base + blockIdx.x;
   int32_t* gbook = P.books + (size_t)blockIdx.x * 2 * (size_t)L;
   long long* grec = P.recs + (size_t)blockIdx.x * 16;
+  const MarketUniform mu = market_uniform(P, market);
+
+  // ---- agent table: rounds 0-1 of Philox for agents [0, n_tab), constant over the S steps
+  AgentTable tab; tab.w = reinterpret_cast<uint32_t*>(book + 2 * L); tab.n_tab = (uint32_t)P.n_tab;
+  table_fill(P, mu, tab);
+  BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
 
   // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
   long long sb0 = 0, sa0 = 0;
@@ -110,12 +117,23 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   const long long vol0 = s_rec[F_SUMVOL];
 
   int sink = 0;                           // only used by the ATOM == 2 microbenchmark variant
+  auto publish = [&](int new_last) {      // one thread: the rule context of the next step
+    RuleCtx rc = rule_ctx(P, bref, new_last, new_last);
+    *reinterpret_cast<int4*>(s_ctl) = make_int4(new_last, (int)rc.bid_hi, (int)rc.ask_lo, rc.noclamp ? 1 : 0);
+  };
+  if (tid == 0) publish(last);
+  __syncthreads();
   // ---- S steps, all on-chip
   for (long long s = 0; s < P.S; ++s) {
     const uint32_t t = t0 + (uint32_t)s;
-    const StepUniform u = step_uniform(P, market, t);
+    const StepUniform u = step_uniform(P, mu, t);
+    const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
+    last = ctl.x;
+    RuleCtx rc;
+    rc.last = last; rc.dp = last - prev; rc.L = L;
+    rc.bid_hi = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
     // a1 + a2: order generation and aggregation
-    generate_step<MODEL, ATOM>(P, book, u, last, prev, tid, T, sink);
+    generate_step<MODEL, ATOM>(P, bref, mu, u, tab, rc, tid, T, sink);
     __syncthreads();                                   // B1: the combined book is complete
 
     // a3-a6: clearing by warp 0 on the active window
@@ -131,12 +149,11 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
       if (lane == 0) {
         int new_last;
         update_record(s_rec, last, vmax, pstar, new_last);
-        s_ctl[0] = new_last;
+        publish(new_last);
       }
     }
     __syncthreads();                                   // B2: residual book and new price visible
     prev = last;
-    last = s_ctl[0];
   }
 
   // ---- a7: write-back (shared -> HBM), 16-byte vectors, plus the totals for sub_buy/sub_sell

@@ -17,6 +17,7 @@ __global__ void smem_atomic_kernel(int L, int delta, int iters, int* out) {
   for (int i = threadIdx.x; i < 2 * L; i += blockDim.x) sbook[i] = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31;
+  ks::BookRef bref; bref.ptr = sbook; bref.saddr = (uint32_t)__cvta_generic_to_shared(sbook);
   const uint32_t n = 2u * (uint32_t)delta + 1u;
   uint32_t x = (blockIdx.x * 1024u + threadIdx.x) * 2654435761u + 12345u;
   int sink = 0;
@@ -33,8 +34,8 @@ __global__ void smem_atomic_kernel(int L, int delta, int iters, int* out) {
         uint32_t o = __umulhi(x, n);
         idx = (int)((x & 1u) * (uint32_t)L) + L / 2 - delta + (int)o;
       }
-      if (MODE == 2) ks::book_add<1>(sbook, idx, 1, sink);
-      else           ks::book_add<0>(sbook, idx, 1, sink);
+      if (MODE == 2) ks::book_add<1>(bref, 4u * (uint32_t)idx, 1, sink);
+      else           ks::book_add<0>(bref, 4u * (uint32_t)idx, 1, sink);
     }
   }
   __syncthreads();
@@ -44,13 +45,20 @@ __global__ void smem_atomic_kernel(int L, int delta, int iters, int* out) {
 // ---- (2) generation only ---------------------------------------------------------------------
 template <int MODEL>
 __global__ void generate_only_kernel(const __grid_constant__ ks::KernelParams P, int* out) {
+  extern __shared__ __align__(16) int32_t gsm[];          // the agent table only (no book)
   const int tid = threadIdx.x, T = blockDim.x;
   const uint32_t market = P.market_base + blockIdx.x;
+  const ks::MarketUniform mu = ks::market_uniform(P, market);
+  ks::AgentTable tab; tab.w = reinterpret_cast<uint32_t*>(gsm); tab.n_tab = (uint32_t)P.n_tab;
+  ks::table_fill(P, mu, tab);
+  __syncthreads();
+  ks::BookRef bref; bref.ptr = nullptr; bref.saddr = 0;
   int sink = 0;
   int last = P.L / 2, prev = P.L / 2;
   for (long long s = 0; s < P.S; ++s) {
-    const ks::StepUniform u = ks::step_uniform(P, market, (uint32_t)s);
-    ks::generate_step<MODEL, 2>(P, nullptr, u, last, prev, tid, T, sink);
+    const ks::StepUniform u = ks::step_uniform(P, mu, (uint32_t)s);
+    const ks::RuleCtx rc = ks::rule_ctx(P, bref, last, prev);
+    ks::generate_step<MODEL, 2>(P, bref, mu, u, tab, rc, tid, T, sink);
   }
   if (sink == 0x12345678) out[0] = sink;
 }
@@ -150,7 +158,7 @@ ks_status ks_bench_smem_atomic(int32_t mode, int32_t delta, int32_t L, int32_t t
 }
 
 ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L, int32_t A, int64_t S, int32_t threads,
-                                 int32_t warmup, int32_t reps, void* stream, double* events_per_s, double* seconds) {
+                                 int32_t table_agents, int32_t warmup, int32_t reps, void* stream, double* events_per_s, double* seconds) {
   if (!p || !events_per_s || !seconds || M < 1 || L < 32 || (L & (L - 1)) || A < 0 || S < 1 || threads < 32 ||
       threads > 1024 || threads % 32 || reps < 1)
     return KS_ERR_INVALID_ARG;
@@ -160,15 +168,21 @@ ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L,
   for (int r = 0; r < 10; ++r) { P.k0[r] = k0; P.k1[r] = k1; k0 += ks::kPhiloxW0; k1 += ks::kPhiloxW1; }
   P.M = M; P.L = L; P.A = A; P.S = S;
   P.noise_delta = p->noise_delta; P.noise_n = 2 * p->noise_delta + 1; P.noise_qmax = p->noise_qmax;
+  P.noise_n4 = 4 * P.noise_n; P.q_addend = 1ull << 32;
   P.maker_spread_max = p->maker_spread_max; P.maker_qty = p->maker_qty;
   P.mom_n = p->mom_delta + 1; P.mom_qmax = p->mom_qmax;
+  P.n_tab = table_agents < 0 ? 0 : (table_agents > A ? A : table_agents);
+  const size_t smem = (size_t)12 * P.n_tab;
+  if (smem > 200 * 1024) return KS_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   int* d_out = nullptr;
   if (cudaMalloc(&d_out, 64) != cudaSuccess) return KS_ERR_CUDA;
   const int model = p->model;
+  cudaFuncSetAttribute(generate_only_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(generate_only_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   auto launch = [&]() {
-    if (model == KS_MODEL_ZI) generate_only_kernel<0><<<M, threads, 0, st>>>(P, d_out);
-    else                      generate_only_kernel<1><<<M, threads, 0, st>>>(P, d_out);
+    if (model == KS_MODEL_ZI) generate_only_kernel<0><<<M, threads, smem, st>>>(P, d_out);
+    else                      generate_only_kernel<1><<<M, threads, smem, st>>>(P, d_out);
   };
   ks_status rc = time_best(launch, warmup, reps, st, seconds);
   cudaFree(d_out);
