@@ -27,14 +27,15 @@ if ROOT not in sys.path:
 
 from paper_2606_21784_b200.workloads import CONFIGS, KS_MODEL_ZI, sampled_markets  # noqa: E402
 
-# Algorithmic integer operations per agent event: 18 u32xu32->u64
-# multiplies + 19 three-input xors of Philox4x32-10 after hoisting what is uniform per
-# market-step, 2 mulhi, 7 rule operations (side test, offset add/sub, select, +1, address) and
-# 1 shared-memory atomic.  MIX3: weighted over the three rules (maker uses fewer words but two
-# atomics).
-ALG_OPS_PER_EVENT = {"zi": 47.0, "mix3": 47.0}
-# issue-limited peak: SMs x 4 schedulers x 32 lanes x 1 warp-instruction/clk x max SM clock
-LANES_PER_SM_PER_CLK = 4 * 32
+# Roofline of ks_persistent_kernel: the fmaheavy pipe that executes the 32x32->64
+# multiplies.  Algorithmic multiplies per agent event: 20 of Philox4x32-10 + the
+# mulhi draws of the rule (noise/momentum: offset and quantity; maker: spread only).
+ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0}
+# Multiplies the kernel actually issues per event (IMAD.WIDE.U32 + IMAD.HI.U32 in the hot loop,
+# from cuobjdump -sass): hoisting of (market, step)-uniform products, w3 never computed.
+EXEC_MULTS_PER_EVENT = {"zi": 21.0, "mix3": (21.0 + 19.0 + 21.0) / 3.0}
+# a 32-lane IMAD.WIDE/IMAD.HI occupies an SMSP's fmaheavy pipe for 4 cycles -> 8 lanes/clk/SMSP
+WIDE_MUL_LANES_PER_SM_PER_CLK = 4 * 8
 
 
 class ClockSampler(threading.Thread):
@@ -279,17 +280,19 @@ def main():
         pass
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
-    peak_tops = sms * LANES_PER_SM_PER_CLK * sm_max_mhz * 1e6 / 1e12
-    achieved_tops = ALG_OPS_PER_EVENT[model] * events_per_step / avg_kern_s / 1e12
-    roofline = {"bound": "alu", "kernel": "ks_persistent_kernel", "achieved": achieved_tops, "peak": peak_tops,
-                "unit": "Tera integer thread-ops/s", "frac": achieved_tops / peak_tops,
+    peak = sms * WIDE_MUL_LANES_PER_SM_PER_CLK * sm_max_mhz * 1e6 / 1e12
+    achieved = ALG_MULTS_PER_EVENT[model] * events_per_step / avg_kern_s / 1e12
+    executed = EXEC_MULTS_PER_EVENT[model] * events_per_step / avg_kern_s / 1e12
+    roofline = {"bound": "alu", "kernel": "ks_persistent_kernel", "achieved": achieved, "peak": peak,
+                "unit": "T 32x32->64-bit integer multiplies/s", "frac": achieved / peak,
                 "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name),
-                "ops_per_event": ALG_OPS_PER_EVENT[model], "avg_launch_ms": avg_kern_s * 1e3,
-                "peak_source": "derived: %d SMs x 4 schedulers x 32 lanes x %.0f MHz (%s)"
+                "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "avg_launch_ms": avg_kern_s * 1e3,
+                "executed_mults_per_event": EXEC_MULTS_PER_EVENT[model], "fmaheavy_pipe_frac_from_executed": executed / peak,
+                "peak_source": "derived (DESIGN.md 7.2): %d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
                                % (sms, sm_max_mhz, "MEASURED_PEAKS.json sm_max_mhz" if peaks else "NVML max clock"),
                 "hbm": {"algorithmic_bytes": M * (8 * L + 128), "achieved_GBps": M * (8 * L + 128) / avg_kern_s / 1e9,
                         "peak_GBps": peaks.get("hbm_gbs", 6650.0),
-                        "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback (B200_PROFILING.md)"}}
+                        "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback (B200_PROFILING.md)"}}
 
     line = {
         "metric": "agent_events_per_s", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
@@ -317,7 +320,7 @@ def main():
         one_ops, _ = ks.ks_bench_smem_atomic(3, delta, Lb, thr, 8, 500)
         gen_M = min(M, sms * 16 * 4)
         gen_S = max(1, min(S, int(2e10 / (gen_M * A))))
-        gen_ev, _ = ks.ks_bench_generate_only(cfg.params, gen_M, L, A, gen_S, args.threads or 128)
+        gen_ev, _ = ks.ks_bench_generate_only(cfg.params, gen_M, L, A, gen_S, args.threads or 128, 0)
         wide, _ = ks.ks_bench_int_pipe(0)
         lop, _ = ks.ks_bench_int_pipe(1)
         mix, _ = ks.ks_bench_int_pipe(2)
@@ -360,7 +363,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {}
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 27806208 + 244404992}   # profiles/r1a_persistent_full.md
 
 if __name__ == "__main__":
     main()

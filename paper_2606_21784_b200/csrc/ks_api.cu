@@ -191,6 +191,7 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 struct LaunchPlan { int T; int n_tab; size_t smem; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
+static const bool kAutoTable = false;   // the table does not pay on B200 in its present form
 
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
@@ -207,6 +208,8 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   int n_tab;
   if (s->opt_table >= 0) {
     n_tab = s->opt_table < tab_for(1) ? s->opt_table : tab_for(1);
+  } else if (!kAutoTable) {
+    n_tab = 0;
   } else {
     const int want = per_sm < 3 ? per_sm : 3;
     if (book + 12LL * s->A <= max_cta && ctas_for(book + 12LL * s->A) >= want) n_tab = s->A;
