@@ -150,9 +150,7 @@ KS_API ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream);
 typedef enum {
   KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 64..1024, multiple of 32          */
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
-  KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
-  KS_OPT_TABLE_AGENTS = 3   /* agents whose Philox rounds 0-1 are kept in a shared-memory table across the
-                               S steps: -1 = automatic, else 0..A (capped to what fits one CTA)            */
+  KS_OPT_CLEAR_PATH = 2     /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
 } ks_option;
 KS_API ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value);
 

@@ -35,11 +35,10 @@ KS_API ks_status ks_bench_smem_atomic(int32_t mode, int32_t delta, int32_t L, in
 
 /* Integer-ALU ceiling for this RNG contract: the library's own generation code (Philox4x32-10 +
  * agent rule, same templates as the persistent kernel) with the shared-memory atomic replaced by
- * a register fold.  Runs M CTAs x `threads` threads, S steps of A agents with a fixed price;
- * the first `table_agents` agents start from the shared-memory table of rounds 0-1.
+ * a register fold.  Runs M CTAs x `threads` threads, S steps of A agents with a fixed price.
  * *events_per_s receives agent events per second. */
 KS_API ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L, int32_t A, int64_t S,
-                                        int32_t threads, int32_t table_agents, int32_t warmup, int32_t reps,
+                                        int32_t threads, int32_t warmup, int32_t reps,
                                         void* stream, double* events_per_s, double* seconds);
 
 /* Raw issue rates of the two instructions Philox is made of.  kind 0: IMAD.WIDE.U32 (u32 x u32 ->

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libkineticsim.so")
 
 KS_OK, KS_ERR_INVALID_ARG, KS_ERR_UNSUPPORTED, KS_ERR_OVERFLOW, KS_ERR_CUDA, KS_ERR_NOMEM = 0, -1, -2, -3, -4, -5
-KS_OPT_BLOCK_THREADS, KS_OPT_ATOMIC_MODE, KS_OPT_CLEAR_PATH, KS_OPT_TABLE_AGENTS = 0, 1, 2, 3
+KS_OPT_BLOCK_THREADS, KS_OPT_ATOMIC_MODE, KS_OPT_CLEAR_PATH = 0, 1, 2
 
 PARAM_FIELDS = ("model", "noise_delta", "noise_qmax", "maker_spread_max", "maker_qty", "mom_delta",
                 "mom_qmax", "init_price")
@@ -70,7 +70,7 @@ def load():
     pd = C.POINTER(dbl)
     L.ks_bench_smem_atomic.argtypes = [i32, i32, i32, i32, i32, i32, i32, i32, vp, pd, pd]
     L.ks_bench_smem_atomic.restype = i32
-    L.ks_bench_generate_only.argtypes = [pp, i32, i32, i32, i64, i32, i32, i32, i32, vp, pd, pd]
+    L.ks_bench_generate_only.argtypes = [pp, i32, i32, i32, i64, i32, i32, i32, vp, pd, pd]
     L.ks_bench_generate_only.restype = i32
     L.ks_bench_int_pipe.argtypes = [i32, i32, i32, i32, i32, i32, vp, pd, pd]
     L.ks_bench_int_pipe.restype = i32
@@ -199,10 +199,10 @@ def ks_bench_smem_atomic(mode, delta, L, threads=256, ctas_per_sm=8, iters=2000,
     return ops.value, sec.value
 
 
-def ks_bench_generate_only(params: dict, M, L, A, S, threads=256, table_agents=0, warmup=1, reps=3, stream=None):
+def ks_bench_generate_only(params: dict, M, L, A, S, threads=256, warmup=1, reps=3, stream=None):
     ev, sec = C.c_double(0), C.c_double(0)
     P = _params(params)
-    _check(load().ks_bench_generate_only(C.byref(P), M, L, A, S, threads, table_agents, warmup, reps, _stream_ptr(stream),
+    _check(load().ks_bench_generate_only(C.byref(P), M, L, A, S, threads, warmup, reps, _stream_ptr(stream),
                                          C.byref(ev), C.byref(sec)))
     return ev.value, sec.value
 

@@ -44,7 +44,7 @@ struct ks_sim {
   int64_t steps_done;
   int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear, opt_table;
+  int32_t opt_threads, opt_atomic, opt_clear;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
   // ks_write_books depth check
@@ -109,7 +109,7 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   if (!s) { set_err("ks_create: out of host memory"); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
   s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_table = -1;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0;
   s->dev_smem_optin = optin; s->num_sms = sms;
   s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_ZI) {
@@ -168,9 +168,6 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_CLEAR_PATH:
       if (value != 0 && value != 1) break;
       s->opt_clear = value; return KS_OK;
-    case KS_OPT_TABLE_AGENTS:
-      if (value < -1) break;
-      s->opt_table = value; return KS_OK;
     default: break;
   }
   set_err("ks_set_option: unknown option or value");
@@ -179,47 +176,20 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 
 }  // extern "C"
 
-// Launch plan: threads per CTA, agents covered by the shared-memory Philox table, dynamic
-// shared memory.  An SM has 228 KB of shared memory; each resident CTA costs its dynamic + static
-// allocation + 1 KB of system reserve.
-//  * Table: all A agents when that still leaves >= 3 CTAs per SM (or as many as the grid can
-//    give an SM); otherwise the largest table that keeps 2 CTAs per SM, so that one market's
-//    clearing phase (one warp) hides behind another market's generation; a book too large for
-//    that runs 1 CTA per SM.
-//  * Threads: few markets -> widen the CTA so the whole GPU is used, but never beyond the
-//    agents; many markets -> at least ~1024 resident threads per SM.
-struct LaunchPlan { int T; int n_tab; size_t smem; };
+// Launch plan: threads per CTA and dynamic shared memory (the book).  An SM has 228 KB of shared
+// memory; each resident CTA costs its dynamic + static allocation + 1 KB of system reserve.
+// Threads: few markets -> widen the CTA so the whole GPU is used, but never beyond the agents;
+// many markets -> 128 threads, so that ~9-16 resident CTAs per SM hide one market's clearing
+// phase (one warp) behind other markets' generation.
+struct LaunchPlan { int T; size_t smem; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
-static const bool kAutoTable = false;   // the table does not pay on B200 in its present form
 
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
-  const long long book = 8LL * s->L;
-  const long long max_cta = (long long)s->dev_smem_optin - 1024;       // static shared memory
-  auto ctas_for = [&](long long dyn) { return (int)(kSmemPerSM / (dyn + kSmemCtaOverhead)); };
-  auto tab_for = [&](int k) {                                            // largest table with k CTAs per SM
-    long long dyn = kSmemPerSM / k - kSmemCtaOverhead;
-    if (dyn > max_cta) dyn = max_cta;
-    long long n = (dyn - book) / 12;
-    return (int)(n < 0 ? 0 : (n > s->A ? s->A : n));
-  };
-  const int per_sm = (s->M + s->num_sms - 1) / s->num_sms;              // CTAs the grid can give one SM
-  int n_tab;
-  if (s->opt_table >= 0) {
-    n_tab = s->opt_table < tab_for(1) ? s->opt_table : tab_for(1);
-  } else if (!kAutoTable) {
-    n_tab = 0;
-  } else {
-    const int want = per_sm < 3 ? per_sm : 3;
-    if (book + 12LL * s->A <= max_cta && ctas_for(book + 12LL * s->A) >= want) n_tab = s->A;
-    else if (ctas_for(book) >= 2) n_tab = tab_for(2);
-    else n_tab = tab_for(1);
-  }
-  pl.n_tab = n_tab;
-  pl.smem = (size_t)(book + 12LL * n_tab);
-  const int k = ctas_for((long long)pl.smem) < 1 ? 1 : ctas_for((long long)pl.smem);
-
+  pl.smem = (size_t)8 * (size_t)s->L;
+  int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
+  if (k < 1) k = 1;
   int T = 128;
   if (s->opt_threads) {
     T = s->opt_threads;
@@ -287,7 +257,6 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   const LaunchPlan pl = plan_launch(s);
   const int T = pl.T;
   const size_t smem = pl.smem;
-  P.n_tab = pl.n_tab;
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
   if (s->p.model == KS_MODEL_ZI)

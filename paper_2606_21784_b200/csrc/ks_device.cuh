@@ -45,7 +45,6 @@ struct KernelParams {
   int32_t dmax;                                   // largest |tick - last| any rule can produce
   int32_t fresh;                                  // books are known to be all zero: skip the load
   int32_t force_generic;                          // ablation/test: always use the chunked scan
-  int32_t n_tab;                                  // agents [0, n_tab) start from the shared-memory table
   long long S;                                    // steps to run
   long long orders_per_step;                      // A + number of makers
 };
@@ -60,11 +59,12 @@ __device__ __forceinline__ uint32_t lo32(uint64_t x) { return (uint32_t)x; }
 //             n2 = hi(M0*a) ^ k1[0]            (a)         n3 = lo(M0*a)              (a)
 //   round 1:  c0 = hi(M1*n2) ^ n1 ^ k0[1]      (a, m)      c1 = lo(M1*n2)             (a)
 //             c2 = hi(M0*n0) ^ n3 ^ k1[1]      (a, m, t)   c3 = lo(M0*n0)             (m, t)
-// so per (market, agent) the triple (c0, c1, n3) is constant over all S steps: it is computed
-// once per launch into a shared-memory table (AgentTable) and each event starts at round 2 with
-// one LDS.64 + one LDS.32 + one LOP3 instead of two 32x32->64 multiplies.  The multiplies are
-// what bounds the kernel (IMAD.WIDE runs at a quarter of the LOP3/IADD rate), so per event the
-// path issues 15 IMAD.WIDE + 1 IMAD.HI for rounds 2..9 and 2 IMAD.HI for the agent rule.
+// M1*m is computed once per CTA, M0*n0 once per thread and step.  A thread visits agents
+// a, a + a_step, a + 2*a_step, ... so the 64-bit product M0*a is carried as a running sum
+// (p0 += M0*a_step: two ALU adds with carry instead of a multiply -- exact, the product of two
+// 32-bit numbers never overflows 64 bits).  The 32x32->64 multiplies are what bounds the kernel
+// (IMAD.WIDE/IMAD.HI hold an SMSP's fmaheavy pipe for 4 cycles per warp), so per
+// event the path issues 16 IMAD.WIDE + 1 IMAD.HI for rounds 1..9 and 2 IMAD.HI for the agent rule.
 // ---------------------------------------------------------------------------------------------
 struct MarketUniform {   // depends on the market only
   uint32_t hm;     // hi(M1*m)
@@ -94,24 +94,20 @@ __device__ __forceinline__ StepUniform step_uniform(const KernelParams& P, const
   return u;
 }
 
-// (c0, c1, n3) of agent a in market mu -- the table entry, also used directly for agents beyond
-// the table.
-__device__ __forceinline__ void agent_rounds01(const KernelParams& P, const MarketUniform& mu, uint32_t a,
-                                               uint32_t& c0, uint32_t& c1, uint32_t& n3) {
-  uint64_t p0 = (uint64_t)kPhiloxM0 * a;
-  uint32_t n2 = hi32(p0) ^ P.k1[0];
-  n3 = lo32(p0);
-  uint64_t p1 = (uint64_t)kPhiloxM1 * n2;
-  c0 = hi32(p1) ^ mu.n1k;
-  c1 = lo32(p1);
-}
-
-// Rounds 2..9 from (c0, c1, c2, c3 = u.d3).  Outputs w0, w1, w2 (w3 is reserved and never
-// computed).  NEED02 = false skips the last round's M0 product (the maker rule reads w1 only).
+// Philox4x32-10 of agent a from p0 = M0*a (round 0's product).  Outputs w0, w1, w2 (w3 is
+// reserved and never computed).  NEED02 = false skips the last round's M0 product and w0 (the
+// maker rule reads w1 only).
 template <bool NEED02>
-__device__ __forceinline__ void philox_rounds(const KernelParams& P, const StepUniform& u, uint32_t c0, uint32_t c1,
-                                              uint32_t c2, uint32_t& w0, uint32_t& w1, uint32_t& w2) {
-  uint32_t c3;
+__device__ __forceinline__ void philox_from_p0(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
+                                               uint64_t p0, uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+  uint32_t c0, c1, c2, c3;
+  {                                       // rounds 0-1
+    const uint32_t n2 = hi32(p0) ^ P.k1[0];
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * n2;
+    c0 = hi32(p1) ^ mu.n1k;
+    c1 = lo32(p1);
+    c2 = u.d2x ^ lo32(p0);
+  }
   {                                       // round 2: c3 = d3 is uniform, d3 ^ k1[2] was pre-xored
     uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
     uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
@@ -138,32 +134,6 @@ __device__ __forceinline__ void philox_rounds(const KernelParams& P, const StepU
   } else {
     w0 = 0; w2 = 0;
   }
-}
-
-// The per-CTA agent table in shared memory: three arrays of n_tab words, c0[], c1[], n3[], for
-// agents [0, n_tab) -- one base register plus uniform offsets addresses all three, and a warp's
-// loads are conflict-free.
-struct AgentTable {
-  uint32_t* w;         // c0 at w[a], c1 at w[n_tab + a], n3 at w[2*n_tab + a]
-  uint32_t n_tab;
-};
-
-__device__ __forceinline__ void table_fill(const KernelParams& P, const MarketUniform& mu, const AgentTable& tab) {
-  for (uint32_t a = threadIdx.x; a < tab.n_tab; a += blockDim.x) {
-    uint32_t c0, c1, n3;
-    agent_rounds01(P, mu, a, c0, c1, n3);
-    tab.w[a] = c0; tab.w[tab.n_tab + a] = c1; tab.w[2 * tab.n_tab + a] = n3;
-  }
-}
-
-template <bool NEED02>
-__device__ __forceinline__ void philox_agent(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
-                                             const AgentTable& tab, bool tabled, uint32_t a,
-                                             uint32_t& w0, uint32_t& w1, uint32_t& w2) {
-  uint32_t c0, c1, n3;
-  if (tabled) { c0 = tab.w[a]; c1 = tab.w[tab.n_tab + a]; n3 = tab.w[2 * tab.n_tab + a]; }
-  else        agent_rounds01(P, mu, a, c0, c1, n3);
-  philox_rounds<NEED02>(P, u, c0, c1, u.d2x ^ n3, w0, w1, w2);
 }
 
 // a2: add one order to the shared-memory book at byte offset `off` from the start of the book.
@@ -196,29 +166,40 @@ __device__ __forceinline__ void book_add(const BookRef& book, uint32_t off, int 
 
 __device__ __forceinline__ int clamp_tick(int x, int L) { return min(max(x, 0), L - 1); }
 
-// Per-step values of the rules that are uniform over the CTA.  bid_hi / ask_lo are absolute
-// shared addresses, published once per step by the clearing warp (ks_kernel.cuh, StepCtl) so that
+// Per-step values of the rules that are uniform over the CTA.  bid_lo / ask_lo are absolute
+// shared addresses, published once per step by the clearing warp (ks_kernel.cuh, s_ctl) so that
 // no thread recomputes them per order.
 struct RuleCtx {
   int last, dp, L;
   bool noclamp;          // last - noise_delta >= 0 and last + noise_delta <= L-1: the noise clamp is the identity
-  uint32_t bid_hi;       // shared address of bid[last + noise_delta]
+  uint32_t bid_lo;       // shared address of bid[last - noise_delta]
   uint32_t ask_lo;       // shared address of ask[last - noise_delta]
 };
 
-// a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; buy tick = last - (o - delta) = (last + delta) - o,
-// sell tick = (last - delta) + o.  4*o is taken as mulhi(w1, 4n) & ~3 (floor(4y) = 4 floor(y) +
-// floor(4 frac(y))), which saves the separate address scaling.  q = 1 + mulhi(w2, qmax) is the
-// high word of w2*qmax + P.q_addend (= 2^32): one IMAD with the +1 folded into its addend.
+// a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; sell tick = (last - delta) + o, buy tick =
+// last - (o - delta) = (last - delta) + (n-1-o).  q = 1 + mulhi(w2, qmax) is the high word of
+// w2*qmax + 2^32: one IMAD.HI with the +1 folded into its 64-bit addend.
+// No-clamp path: the whole address comes out of ONE IMAD.HI, because the fma pipe that executes
+// the multiplies is the bound and every IMAD.IADD the compiler would emit for an address add
+// costs it two more cycles:
+//   sell:  hi(w1*4n + {hi: &ask[last-delta], lo: 0})       = &ask[last-delta] + 4o + r,  r in 0..3
+//   buy:   hi(~w1*4n + {hi: &bid[last-delta], lo: 4n-1})   = &bid[last-delta] + 4(n-1-o) + (3-r)
+// (floor(4y) = 4 floor(y) + r; and with w*4n = H*2^32 + Lo, (2^32-1-w)*4n + 4n-1 =
+// (4n-1-H)*2^32 + (2^32-1-Lo), so the high word is exactly 4n-1-H), then & ~3 drops r.
+// m = w0 >> 31 (arithmetic) is all-ones for a buy: x = w1 ^ m, addend = {ask_lo ^ (m & (ask_lo ^
+// bid_lo)), m & (4n-1)} -- alu-pipe instructions only.
 template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                             uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
   const int q = (int)hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend);
-  const bool buy = (int32_t)w0 < 0;
   if (!CLAMP) {
-    const uint32_t o4 = __umulhi(w1, (uint32_t)P.noise_n4) & ~3u;
-    book_add_at<ATOM>(book, buy ? rc.bid_hi - o4 : rc.ask_lo + o4, q, sink);
+    const uint32_t m = (uint32_t)((int32_t)w0 >> 31);
+    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ rc.bid_lo));
+    const uint64_t addend = ((uint64_t)base << 32) | (m & (uint32_t)(P.noise_n4 - 1));
+    const uint32_t addr = hi32((uint64_t)(w1 ^ m) * (uint32_t)P.noise_n4 + addend) & ~3u;
+    book_add_at<ATOM>(book, addr, q, sink);
   } else {
+    const bool buy = (int32_t)w0 < 0;
     const int o = (int)__umulhi(w1, (uint32_t)P.noise_n);
     const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - o : (rc.last - P.noise_delta) + o, rc.L);
     book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
@@ -245,52 +226,91 @@ __device__ __forceinline__ void momentum_order(const KernelParams& P, const Book
   book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
 }
 
-// One agent class of one market-step: agents first, first + a_step, ... < a_end, rule KIND
-// (0 noise, 1 maker, 2 momentum).  Agents below tab.n_tab start from the table; the loop over
-// them has a uniform trip count (no per-agent bound check) plus one ragged tail.
+// The agents of one class that a thread visits: first, first + a_step, ... < a_end.  p0 = M0*first;
+// n_uniform trips are made by every thread of the CTA (a uniform loop, no per-agent bound
+// check), `extra` marks the threads that own one agent more (ragged tail).
+struct ClassPlan {
+  uint64_t p0;
+  uint32_t n_uniform;
+  bool extra;
+};
+
+__device__ __forceinline__ ClassPlan class_plan(uint32_t first, uint32_t first_of_last_thread, uint32_t a_end,
+                                                uint32_t a_step) {
+  auto trips = [&](uint32_t f) { return f < a_end ? (a_end - f + a_step - 1u) / a_step : 0u; };
+  ClassPlan pl;
+  pl.p0 = (uint64_t)kPhiloxM0 * first;
+  pl.n_uniform = trips(first_of_last_thread);
+  pl.extra = trips(first) > pl.n_uniform;
+  return pl;
+}
+
+// p + inc as an explicit carry chain, so that it stays one IADD3 + one IADD3.X on the alu pipe and
+// is neither turned back into a multiply nor duplicated per unrolled copy.
+__device__ __forceinline__ uint64_t add64_alu(uint64_t p, uint64_t inc) {
+  uint32_t lo, hi;
+  asm volatile("add.cc.u32 %0, %2, %4;\n\taddc.u32 %1, %3, %5;"
+               : "=r"(lo), "=r"(hi)
+               : "r"(lo32(p)), "r"(hi32(p)), "r"(lo32(inc)), "r"(hi32(inc)));
+  return ((uint64_t)hi << 32) | lo;
+}
+
+// One agent class of one market-step, rule KIND (0 noise, 1 maker, 2 momentum).
 template <int ATOM, int KIND, bool CLAMP>
 __device__ __forceinline__ void generate_class(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
-                                               const StepUniform& u, const AgentTable& tab, const RuleCtx& rc,
-                                               uint32_t first, uint32_t a_end, uint32_t a_step, int& sink) {
-  auto one = [&](uint32_t a, bool tabled) {
+                                               const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
+                                               uint64_t p0_inc, int& sink) {
+  auto one = [&](uint64_t p0) {
     uint32_t w0, w1, w2;
-    philox_agent<KIND != 1>(P, mu, u, tab, tabled, a, w0, w1, w2);
+    philox_from_p0<KIND != 1>(P, mu, u, p0, w0, w1, w2);
     if (KIND == 0)      noise_order<ATOM, CLAMP>(P, book, rc, w0, w1, w2, sink);
     else if (KIND == 1) maker_order<ATOM>(P, book, rc, w1, sink);
     else                momentum_order<ATOM>(P, book, rc, w0, w1, w2, sink);
   };
-  const uint32_t t_end = min(a_end, tab.n_tab);
-  uint32_t a = first;
-  if (t_end > first) {
-    // full groups: every thread of the CTA has an agent (first <= first of the last thread)
-    const uint32_t last_first = first - (uint32_t)threadIdx.x * (a_step / blockDim.x) +
-                                (blockDim.x - 1) * (a_step / blockDim.x);
-    const uint32_t nfull = t_end > last_first ? (t_end - last_first + a_step - 1) / a_step : 0u;
+  uint64_t p0 = pl.p0;
 #pragma unroll 2
-    for (uint32_t k = 0; k < nfull; ++k, a += a_step) one(a, true);
-    if (a < t_end) { one(a, true); a += a_step; }
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
+  if (pl.extra) one(p0);
+}
+
+// The per-thread plans of a launch: MODEL 0 one class (a = tid + k*T), MODEL 1 three classes
+// (agent a = 3j + c has type c, j = tid + k*T; each class runs in its own warp-uniform loop --
+// integer atomics commute, so the agent -> thread mapping cannot change a byte of the result).
+template <int MODEL>
+struct GenPlan {
+  ClassPlan cls[MODEL == 0 ? 1 : 3];
+  uint64_t p0_inc;       // M0 * a_step
+};
+
+template <int MODEL>
+__device__ __forceinline__ GenPlan<MODEL> gen_plan(const KernelParams& P, int tid, int T) {
+  GenPlan<MODEL> g;
+  const uint32_t A = (uint32_t)P.A;
+  if (MODEL == 0) {
+    g.p0_inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
+    g.cls[0] = class_plan((uint32_t)tid, (uint32_t)(T - 1), A, (uint32_t)T);
+  } else {
+    const uint32_t st = 3u * (uint32_t)T;
+    g.p0_inc = (uint64_t)kPhiloxM0 * st;
+#pragma unroll
+    for (int c = 0; c < (MODEL == 0 ? 1 : 3); ++c)
+      g.cls[c] = class_plan(3u * (uint32_t)tid + (uint32_t)c, 3u * (uint32_t)(T - 1) + (uint32_t)c, A, st);
   }
-#pragma unroll 2
-  for (; a < a_end; a += a_step) one(a, false);
+  // hide that p0_inc is a product: otherwise p0 += p0_inc is turned back into IMAD.WIDE(M0, a_step, p0)
+  asm volatile("" : "+l"(g.p0_inc));
+  return g;
 }
 
 // a1 + a2 for one market-step: every thread of the CTA generates the orders of its agents.
-// MODEL 1: agent a = 3j + c has type c; each class runs in its own warp-uniform loop (integer
-// atomics commute, so the agent -> thread mapping cannot change a byte of the result).
 template <int MODEL, int ATOM>
 __device__ __forceinline__ void generate_step(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
-                                              const StepUniform& u, const AgentTable& tab, const RuleCtx& rc,
-                                              int tid, int T, int& sink) {
-  const uint32_t A = (uint32_t)P.A;
-  if (MODEL == 0) {
-    if (rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, tab, rc, (uint32_t)tid, A, (uint32_t)T, sink);
-    else            generate_class<ATOM, 0, true >(P, book, mu, u, tab, rc, (uint32_t)tid, A, (uint32_t)T, sink);
-  } else {
-    const uint32_t st = 3u * (uint32_t)T;
-    if (rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, tab, rc, 3u * tid, A, st, sink);
-    else            generate_class<ATOM, 0, true >(P, book, mu, u, tab, rc, 3u * tid, A, st, sink);
-    generate_class<ATOM, 1, true>(P, book, mu, u, tab, rc, 3u * tid + 1u, A, st, sink);
-    generate_class<ATOM, 2, true>(P, book, mu, u, tab, rc, 3u * tid + 2u, A, st, sink);
+                                              const StepUniform& u, const RuleCtx& rc, const GenPlan<MODEL>& g,
+                                              int& sink) {
+  if (rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+  else            generate_class<ATOM, 0, true >(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+  if (MODEL == 1) {
+    generate_class<ATOM, 1, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 1], g.p0_inc, sink);
+    generate_class<ATOM, 2, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 2], g.p0_inc, sink);
   }
 }
 
@@ -299,7 +319,7 @@ __device__ __forceinline__ RuleCtx rule_ctx(const KernelParams& P, const BookRef
   RuleCtx rc;
   rc.last = last; rc.dp = last - prev; rc.L = P.L;
   rc.noclamp = (last - P.noise_delta >= 0) && (last + P.noise_delta <= P.L - 1);
-  rc.bid_hi = book.saddr + 4u * (uint32_t)(last + P.noise_delta);
+  rc.bid_lo = book.saddr + 4u * (uint32_t)(last - P.noise_delta);
   rc.ask_lo = book.saddr + 4u * (uint32_t)(P.L + last - P.noise_delta);
   return rc;
 }

@@ -60,16 +60,15 @@ __device__ __forceinline__ void update_record(long long* rec, int last, int vmax
 
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
-// dynamic shared memory = 8*L bytes (the book) + 12*n_tab bytes (the agent table of
-// ks_device.cuh, n_tab = P.n_tab agents).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
+// dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
 // ---------------------------------------------------------------------------------------------
 template <int MODEL, int ATOM>
 __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
-  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then the agent table
+  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
   __shared__ int s_red32[64];
-  __shared__ __align__(16) int s_ctl[4];              // per-step broadcast: last, &bid[last+delta], &ask[last-delta], noclamp
+  __shared__ __align__(16) int s_ctl[4];              // per-step broadcast: last, &bid[last-delta], &ask[last-delta], noclamp
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
   const int L = P.L;
@@ -78,9 +77,7 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   long long* grec = P.recs + (size_t)blockIdx.x * 16;
   const MarketUniform mu = market_uniform(P, market);
 
-  // ---- agent table: rounds 0-1 of Philox for agents [0, n_tab), constant over the S steps
-  AgentTable tab; tab.w = reinterpret_cast<uint32_t*>(book + 2 * L); tab.n_tab = (uint32_t)P.n_tab;
-  table_fill(P, mu, tab);
+  const GenPlan<MODEL> gplan = gen_plan<MODEL>(P, tid, T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
 
   // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
@@ -119,7 +116,7 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   int sink = 0;                           // only used by the ATOM == 2 microbenchmark variant
   auto publish = [&](int new_last) {      // one thread: the rule context of the next step
     RuleCtx rc = rule_ctx(P, bref, new_last, new_last);
-    *reinterpret_cast<int4*>(s_ctl) = make_int4(new_last, (int)rc.bid_hi, (int)rc.ask_lo, rc.noclamp ? 1 : 0);
+    *reinterpret_cast<int4*>(s_ctl) = make_int4(new_last, (int)rc.bid_lo, (int)rc.ask_lo, rc.noclamp ? 1 : 0);
   };
   if (tid == 0) publish(last);
   __syncthreads();
@@ -131,9 +128,9 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
     last = ctl.x;
     RuleCtx rc;
     rc.last = last; rc.dp = last - prev; rc.L = L;
-    rc.bid_hi = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
+    rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
     // a1 + a2: order generation and aggregation
-    generate_step<MODEL, ATOM>(P, bref, mu, u, tab, rc, tid, T, sink);
+    generate_step<MODEL, ATOM>(P, bref, mu, u, rc, gplan, sink);
     __syncthreads();                                   // B1: the combined book is complete
 
     // a3-a6: clearing by warp 0 on the active window

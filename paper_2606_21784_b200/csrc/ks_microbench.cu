@@ -45,20 +45,17 @@ __global__ void smem_atomic_kernel(int L, int delta, int iters, int* out) {
 // ---- (2) generation only ---------------------------------------------------------------------
 template <int MODEL>
 __global__ void generate_only_kernel(const __grid_constant__ ks::KernelParams P, int* out) {
-  extern __shared__ __align__(16) int32_t gsm[];          // the agent table only (no book)
   const int tid = threadIdx.x, T = blockDim.x;
   const uint32_t market = P.market_base + blockIdx.x;
   const ks::MarketUniform mu = ks::market_uniform(P, market);
-  ks::AgentTable tab; tab.w = reinterpret_cast<uint32_t*>(gsm); tab.n_tab = (uint32_t)P.n_tab;
-  ks::table_fill(P, mu, tab);
-  __syncthreads();
+  const ks::GenPlan<MODEL> gplan = ks::gen_plan<MODEL>(P, tid, T);
   ks::BookRef bref; bref.ptr = nullptr; bref.saddr = 0;
   int sink = 0;
   int last = P.L / 2, prev = P.L / 2;
   for (long long s = 0; s < P.S; ++s) {
     const ks::StepUniform u = ks::step_uniform(P, mu, (uint32_t)s);
     const ks::RuleCtx rc = ks::rule_ctx(P, bref, last, prev);
-    ks::generate_step<MODEL, 2>(P, bref, mu, u, tab, rc, tid, T, sink);
+    ks::generate_step<MODEL, 2>(P, bref, mu, u, rc, gplan, sink);
   }
   if (sink == 0x12345678) out[0] = sink;
 }
@@ -158,7 +155,7 @@ ks_status ks_bench_smem_atomic(int32_t mode, int32_t delta, int32_t L, int32_t t
 }
 
 ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L, int32_t A, int64_t S, int32_t threads,
-                                 int32_t table_agents, int32_t warmup, int32_t reps, void* stream, double* events_per_s, double* seconds) {
+                                 int32_t warmup, int32_t reps, void* stream, double* events_per_s, double* seconds) {
   if (!p || !events_per_s || !seconds || M < 1 || L < 32 || (L & (L - 1)) || A < 0 || S < 1 || threads < 32 ||
       threads > 1024 || threads % 32 || reps < 1)
     return KS_ERR_INVALID_ARG;
@@ -171,15 +168,11 @@ ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L,
   P.noise_n4 = 4 * P.noise_n; P.q_addend = 1ull << 32;
   P.maker_spread_max = p->maker_spread_max; P.maker_qty = p->maker_qty;
   P.mom_n = p->mom_delta + 1; P.mom_qmax = p->mom_qmax;
-  P.n_tab = table_agents < 0 ? 0 : (table_agents > A ? A : table_agents);
-  const size_t smem = (size_t)12 * P.n_tab;
-  if (smem > 200 * 1024) return KS_ERR_INVALID_ARG;
+  const size_t smem = 0;
   cudaStream_t st = (cudaStream_t)stream;
   int* d_out = nullptr;
   if (cudaMalloc(&d_out, 64) != cudaSuccess) return KS_ERR_CUDA;
   const int model = p->model;
-  cudaFuncSetAttribute(generate_only_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(generate_only_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   auto launch = [&]() {
     if (model == KS_MODEL_ZI) generate_only_kernel<0><<<M, threads, smem, st>>>(P, d_out);
     else                      generate_only_kernel<1><<<M, threads, smem, st>>>(P, d_out);
