@@ -177,10 +177,14 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 }  // extern "C"
 
 // Launch plan: threads per CTA and dynamic shared memory (the book).  An SM has 228 KB of shared
-// memory; each resident CTA costs its dynamic + static allocation + 1 KB of system reserve.
-// Threads: few markets -> widen the CTA so the whole GPU is used, but never beyond the agents;
-// many markets -> 128 threads, so that ~9-16 resident CTAs per SM hide one market's clearing
-// phase (one warp) behind other markets' generation.
+// memory; each resident CTA costs its dynamic + static allocation + 1 KB of system reserve, and an
+// SM holds at most 32 CTAs.
+// Threads: many markets and a small book -> ONE WARP per market (T = 32, 32 CTAs per SM): no warp
+// ever waits at a barrier for another warp's generation or for the clearing warp, and the eight
+// markets resident on a scheduler hide each other's clearing (measured on B200, DESIGN.md 7.4:
+// T = 32 beats 64/128 on C4).  A book so large that 32-thread CTAs would leave the SM short of
+// warps -> widen until ~1024 threads are resident; few markets -> widen so the whole GPU is used,
+// but never beyond the agents.
 struct LaunchPlan { int T; size_t smem; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
@@ -190,7 +194,8 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   pl.smem = (size_t)8 * (size_t)s->L;
   int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
   if (k < 1) k = 1;
-  int T = 128;
+  if (k > 32) k = 32;
+  int T = 32;
   if (s->opt_threads) {
     T = s->opt_threads;
   } else {

@@ -17,8 +17,13 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#ifndef KS_GEN_UNROLL
+#define KS_GEN_UNROLL 2      // independent Philox chains per thread in the generation loop
+#endif
+
 namespace ks {
 
+constexpr int kGenUnroll = KS_GEN_UNROLL;
 constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
 constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;
 constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;
@@ -268,7 +273,7 @@ __device__ __forceinline__ void generate_class(const KernelParams& P, const Book
     else                momentum_order<ATOM>(P, book, rc, w0, w1, w2, sink);
   };
   uint64_t p0 = pl.p0;
-#pragma unroll 2
+#pragma unroll kGenUnroll
   for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
   if (pl.extra) one(p0);
 }
