@@ -321,7 +321,7 @@ def main():
         one_ops, _ = ks.ks_bench_smem_atomic(3, delta, Lb, thr, 8, 500)
         gen_M = min(M, sms * 16 * 4)
         gen_S = max(1, min(S, int(2e10 / (gen_M * A))))
-        gen_ev, _ = ks.ks_bench_generate_only(cfg.params, gen_M, L, A, gen_S, args.threads or 128)
+        gen_ev, _ = ks.ks_bench_generate_only(cfg.params, gen_M, L, A, gen_S, args.threads or 32)
         wide, _ = ks.ks_bench_int_pipe(0)
         lop, _ = ks.ks_bench_int_pipe(1)
         mix, _ = ks.ks_bench_int_pipe(2)
@@ -350,6 +350,22 @@ def main():
                 ts.append(a.elapsed_time(b)); sim.ks_destroy()
             extra[name] = {"ms_median_of_3": float(np.median(ts[1:])), "events_per_s": c.events / (float(np.median(ts[1:])) * 1e-3)}
         line["all_configs"] = extra
+        # a8 ablation on C2: one launch per step, book through HBM every step
+        c = CONFIGS["C2"]
+        st = torch.empty(ks.ks_state_bytes(c.M, c.L), dtype=torch.uint8, device=dev)
+        ts = []
+        for i in range(3):
+            sim = ks.KsSim(c.M, c.L, c.A, c.params, c.seed, state=st)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); sim.ks_run_stepwise(c.S); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b)); sim.ks_destroy()
+        ms = float(np.median(ts[1:]))
+        hbm_bytes = float(c.S) * c.M * 2 * (8 * c.L + 128)          # load + store of book and record, every step
+        line["ablation_launch_per_step_C2"] = {
+            "ms": ms, "events_per_s": c.events / (ms * 1e-3), "launches": c.S,
+            "slowdown_vs_persistent": ms / extra["C2"]["ms_median_of_3"],
+            "algorithmic_hbm_bytes": hbm_bytes, "hbm_GBps": hbm_bytes / (ms * 1e-3) / 1e9,
+            "persistent_hbm_bytes": float(c.M) * (8 * c.L + 128)}
 
     if not args.no_cpu_baseline and world == 1:
         n_mk = min(cfg.M, 64)
@@ -364,7 +380,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 27806208 + 244404992}   # profiles/r1a_persistent_full.md
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 25957888 + 239323648}   # profiles/r1c_persistent_full.md
 
 if __name__ == "__main__":
     main()

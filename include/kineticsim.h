@@ -46,7 +46,9 @@ typedef struct ks_sim ks_sim; /* opaque host-side handle, owned by the library *
 typedef enum {
   KS_OK = 0,
   KS_ERR_INVALID_ARG = -1, /* NULL pointer, M < 1, A < 0, S < 0, L not a power of two or < 32, bad params */
-  KS_ERR_UNSUPPORTED = -2, /* L above the single-CTA limit (16384) -- see DESIGN.md "out of scope"        */
+  KS_ERR_UNSUPPORTED = -2, /* L > 32768 (p* must fit the 16-bit field of the trajectory hash), or a book
+                              that does not fit this device's shared memory.  16384 < L <= 32768 runs on a
+                              thread-block cluster (DSMEM), see KS_OPT_CLUSTER_SIZE                        */
   KS_ERR_OVERFLOW = -3,    /* a per-side depth sum or a statistic could leave its integer type            */
   KS_ERR_CUDA = -4,        /* a CUDA call failed; text in ks_last_error()                                 */
   KS_ERR_NOMEM = -5        /* host allocation failed                                                      */
@@ -150,7 +152,11 @@ KS_API ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream);
 typedef enum {
   KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 64..1024, multiple of 32          */
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
-  KS_OPT_CLEAR_PATH = 2     /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
+  KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
+  KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
+                               i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
+                               book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and
+                               KS_OPT_ATOMIC_MODE 0                                                          */
 } ks_option;
 KS_API ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value);
 

@@ -1,7 +1,7 @@
 // ks_api.cu -- host side of the C ABI declared in include/kineticsim.h.
 #include "../../include/kineticsim.h"
 #include "../../include/kineticsim_bench.h"
-#include "ks_kernel.cuh"
+#include "ks_cluster.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -30,7 +30,8 @@ void set_err(const char* fmt, const char* a = "", const char* b = "") {
 
 bool is_pow2(int32_t x) { return x > 0 && (x & (x - 1)) == 0; }
 
-constexpr int32_t kMaxL = 16384;          // 8*L = 128 KB of the 227 KB a CTA may own
+constexpr int32_t kMaxLPerCta = 16384;    // 8*Lc = 128 KB of the 227 KB a CTA may own
+constexpr int32_t kMaxL = 32768;          // p* must fit the 16-bit field of the trajectory hash
 constexpr int32_t kMaxQty = 1 << 20;
 
 }  // namespace
@@ -44,7 +45,7 @@ struct ks_sim {
   int64_t steps_done;
   int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear;
+  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
   // ks_write_books depth check
@@ -85,7 +86,8 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
                        uint32_t market_base, void* d_state, void* stream) {
   if (!out || !p || !d_state) { set_err("ks_create: NULL argument"); return KS_ERR_INVALID_ARG; }
   *out = nullptr;
-  if (!shape_ok(M, L) || A < 0) { set_err("ks_create: need M >= 1, A >= 0, L a power of two in [32, 32768]"); return KS_ERR_INVALID_ARG; }
+  if (M < 1 || A < 0 || !is_pow2(L) || L < 32) { set_err("ks_create: need M >= 1, A >= 0, L a power of two >= 32"); return KS_ERR_INVALID_ARG; }
+  if (L > kMaxL) { set_err("ks_create: L > 32768 is not supported (p* must fit 16 bits of the trajectory hash)"); return KS_ERR_UNSUPPORTED; }
   if ((reinterpret_cast<uintptr_t>(d_state) & 15) != 0) { set_err("ks_create: d_state must be 16-byte aligned"); return KS_ERR_INVALID_ARG; }
   if (p->model != KS_MODEL_ZI && p->model != KS_MODEL_MIX3) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
   if (p->noise_delta < 0 || p->noise_delta >= L || p->noise_qmax < 1 || p->noise_qmax > kMaxQty || p->init_price >= L) {
@@ -97,19 +99,21 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
     set_err("ks_create: bad maker/momentum parameters"); return KS_ERR_INVALID_ARG;
   }
   if ((uint64_t)market_base + (uint64_t)M > 0x100000000ull) { set_err("ks_create: market ids exceed 32 bits"); return KS_ERR_INVALID_ARG; }
-  if (L > kMaxL) { set_err("ks_create: L > 16384 needs the cluster/DSMEM path, which is not built"); return KS_ERR_UNSUPPORTED; }
 
   int dev = 0, optin = 0, sms = 0;
   KS_CUDA(cudaGetDevice(&dev));
   KS_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   KS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  if ((size_t)8 * L + 2048 > (size_t)optin) { set_err("ks_create: book does not fit this device's shared memory"); return KS_ERR_UNSUPPORTED; }
+  {
+    const int32_t Lc = L > kMaxLPerCta ? kMaxLPerCta : L;           // larger books are split across a cluster
+    if ((size_t)8 * Lc + 2048 > (size_t)optin) { set_err("ks_create: book does not fit this device's shared memory"); return KS_ERR_UNSUPPORTED; }
+  }
 
   ks_sim* s = new (std::nothrow) ks_sim();
   if (!s) { set_err("ks_create: out of host memory"); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
   s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0;
   s->dev_smem_optin = optin; s->num_sms = sms;
   s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_ZI) {
@@ -164,10 +168,16 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
       s->opt_threads = value; return KS_OK;
     case KS_OPT_ATOMIC_MODE:
       if (value != 0 && value != 1) break;
+      if (value == 1 && (s->opt_cluster > 1 || s->L > kMaxLPerCta)) break;   // the cluster kernel has plain atomics only
       s->opt_atomic = value; return KS_OK;
     case KS_OPT_CLEAR_PATH:
       if (value != 0 && value != 1) break;
       s->opt_clear = value; return KS_OK;
+    case KS_OPT_CLUSTER_SIZE:
+      if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break;
+      if (value > 1 && (s->L / value < 32 || s->opt_atomic)) break;
+      if (value == 1 && s->L > kMaxLPerCta) break;
+      s->opt_cluster = value; return KS_OK;
     default: break;
   }
   set_err("ks_set_option: unknown option or value");
@@ -219,6 +229,27 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
   return cudaGetLastError();
 }
 
+// Cluster launch: grid = M*C CTAs in clusters of C (cluster <-> market), 8*L/C bytes of shared
+// memory per CTA.
+template <int MODEL>
+static cudaError_t launch_cluster(const ks::KernelParams& P, int C, int T, cudaStream_t st) {
+  auto kern = ks::ks_cluster_kernel<MODEL>;
+  const size_t smem = (size_t)8 * (size_t)(P.L / C);
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3((unsigned)P.M * (unsigned)C, 1, 1);
+  cfg.blockDim = dim3((unsigned)T, 1, 1);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, P);
+}
+
 static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   if (!s) { set_err("%s: NULL handle", who); return KS_ERR_INVALID_ARG; }
   if (S < 0) { set_err("%s: S < 0", who); return KS_ERR_INVALID_ARG; }
@@ -259,15 +290,26 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   P.S = S;
   P.orders_per_step = (long long)s->A + s->n_maker;
 
-  const LaunchPlan pl = plan_launch(s);
-  const int T = pl.T;
-  const size_t smem = pl.smem;
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
-  if (s->p.model == KS_MODEL_ZI)
-    e = s->opt_atomic ? launch_persistent<0, 1>(P, T, smem, st) : launch_persistent<0, 0>(P, T, smem, st);
-  else
-    e = s->opt_atomic ? launch_persistent<1, 1>(P, T, smem, st) : launch_persistent<1, 0>(P, T, smem, st);
+  int C = s->opt_cluster;
+  if (C == 0) C = s->L > kMaxLPerCta ? s->L / kMaxLPerCta : 1;
+  if (C > 1) {
+    // cluster path: the C*T threads of a cluster share the agents
+    int T = s->opt_threads ? s->opt_threads : 256;
+    while (!s->opt_threads && T > 32 && (long long)C * (T / 2) >= s->A) T /= 2;
+    int log2C = 0;
+    while ((1 << log2C) < C) ++log2C;
+    P.log2C = log2C;
+    if ((long long)s->M * C > 0x7fffffffLL) { set_err("%s: M * cluster size exceeds the grid limit", who); return KS_ERR_UNSUPPORTED; }
+    e = s->p.model == KS_MODEL_ZI ? launch_cluster<0>(P, C, T, st) : launch_cluster<1>(P, C, T, st);
+  } else {
+    const LaunchPlan pl = plan_launch(s);
+    if (s->p.model == KS_MODEL_ZI)
+      e = s->opt_atomic ? launch_persistent<0, 1>(P, pl.T, pl.smem, st) : launch_persistent<0, 0>(P, pl.T, pl.smem, st);
+    else
+      e = s->opt_atomic ? launch_persistent<1, 1>(P, pl.T, pl.smem, st) : launch_persistent<1, 0>(P, pl.T, pl.smem, st);
+  }
   if (e != cudaSuccess) { set_err("%s: launch failed: %s", who, cudaGetErrorString(e)); return KS_ERR_CUDA; }
   g_launches++;
   s->steps_done += S;

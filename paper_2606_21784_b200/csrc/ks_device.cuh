@@ -50,6 +50,7 @@ struct KernelParams {
   int32_t dmax;                                   // largest |tick - last| any rule can produce
   int32_t fresh;                                  // books are known to be all zero: skip the load
   int32_t force_generic;                          // ablation/test: always use the chunked scan
+  int32_t log2C;                                  // cluster kernel only: CTAs per market = 1 << log2C
   long long S;                                    // steps to run
   long long orders_per_step;                      // A + number of makers
 };
@@ -141,13 +142,15 @@ __device__ __forceinline__ void philox_from_p0(const KernelParams& P, const Mark
   }
 }
 
-// a2: add one order to the shared-memory book at byte offset `off` from the start of the book.
-// ATOM 0: plain shared-memory reduction (ATOMS.ADD, result unused).  ATOM 1: warp-aggregated --
-// lanes with the same address elect a leader that adds the group's sum (north_star (3)); kept as
-// an ablation switch.  ATOM 2: microbenchmark only, no memory access.
+// a2: add one order to the shared-memory book at byte offset `off` from the start of the [2][L]
+// book.  ATOM 0: plain shared-memory reduction (ATOMS.ADD, result unused).  ATOM 1: warp-aggregated
+// -- lanes with the same address elect a leader that adds the group's sum (north_star (3)); kept
+// as an ablation switch.  ATOM 2: microbenchmark only, no memory access.  ATOM 3: the book is
+// split across the CTAs of a cluster (ks_cluster.cuh): remote shared-memory reduction over DSMEM.
 struct BookRef {
   int32_t* ptr;        // generic pointer to the book
   uint32_t saddr;      // its 32-bit shared-window address
+  int log2L, log2Lc;   // ATOM 3 only: L = 1 << log2L ticks, 1 << log2Lc of them per CTA
 };
 
 template <int ATOM>
@@ -166,7 +169,16 @@ __device__ __forceinline__ void book_add_at(const BookRef& book, uint32_t saddr,
 
 template <int ATOM>
 __device__ __forceinline__ void book_add(const BookRef& book, uint32_t off, int q, int& sink) {
-  book_add_at<ATOM>(book, book.saddr + off, q, sink);
+  if (ATOM == 3) {
+    const uint32_t word = off >> 2, side = word >> book.log2L, tick = word & ((1u << book.log2L) - 1u);
+    const uint32_t rank = tick >> book.log2Lc;
+    const uint32_t loc = (side << book.log2Lc) + (tick & ((1u << book.log2Lc) - 1u));
+    uint32_t caddr;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(caddr) : "r"(book.saddr + 4u * loc), "r"(rank));
+    asm volatile("red.shared::cluster.add.s32 [%0], %1;" ::"r"(caddr), "r"(q) : "memory");
+  } else {
+    book_add_at<ATOM>(book, book.saddr + off, q, sink);
+  }
 }
 
 __device__ __forceinline__ int clamp_tick(int x, int L) { return min(max(x, 0), L - 1); }
@@ -311,7 +323,7 @@ template <int MODEL, int ATOM>
 __device__ __forceinline__ void generate_step(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                               const StepUniform& u, const RuleCtx& rc, const GenPlan<MODEL>& g,
                                               int& sink) {
-  if (rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+  if (ATOM != 3 && rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
   else            generate_class<ATOM, 0, true >(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
   if (MODEL == 1) {
     generate_class<ATOM, 1, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 1], g.p0_inc, sink);
@@ -329,6 +341,20 @@ __device__ __forceinline__ RuleCtx rule_ctx(const KernelParams& P, const BookRef
   return rc;
 }
 
+// Book accessors of the clearing code: 16-byte vectors of 4 consecutive ticks of one side
+// (side 0 = bid, 1 = ask), tick a multiple of 4.  LocalBook: the whole [2][L] book in this CTA's
+// shared memory.  ClusterBook (ks_cluster.cuh): the book split across the CTAs of a cluster.
+struct LocalBook {
+  int32_t* book;
+  int L;
+  __device__ __forceinline__ int4 ld4(int side, int tick) const {
+    return *reinterpret_cast<const int4*>((side ? book + L : book) + tick);
+  }
+  __device__ __forceinline__ void st4(int side, int tick, int4 v) const {
+    *reinterpret_cast<int4*>((side ? book + L : book) + tick) = v;
+  }
+};
+
 // ---------------------------------------------------------------------------------------------
 // a3-a5, one warp, window of at most 32*K ticks starting at `base` (a multiple of K).
 // Lane i owns ticks base + i*K .. base + i*K + K-1 in registers.
@@ -339,8 +365,8 @@ __device__ __forceinline__ RuleCtx rule_ctx(const KernelParams& P, const BookRef
 // Also returns conservative bounds of the residual book inside the window (bmax: highest tick
 // with bid depth, else base-1; amin: lowest tick with ask depth, else base+32K).
 // ---------------------------------------------------------------------------------------------
-template <int K>
-__device__ __forceinline__ void clear_window(int32_t* book, int L, int base, int lane,
+template <int K, class IO>
+__device__ __forceinline__ void clear_window(const IO& io, int L, int base, int lane,
                                              int& vmax, int& pstar, int& bmax_new, int& amin_new) {
   static_assert(K % 4 == 0, "K must be a multiple of 4 (16-byte shared-memory vectors)");
   const unsigned FULL = 0xffffffffu;
@@ -351,8 +377,8 @@ __device__ __forceinline__ void clear_window(int32_t* book, int L, int base, int
   for (int v = 0; v < K / 4; ++v) {
     int4 vb = make_int4(0, 0, 0, 0), va = make_int4(0, 0, 0, 0);
     if (in) {
-      vb = *reinterpret_cast<const int4*>(book + tick0 + 4 * v);
-      va = *reinterpret_cast<const int4*>(book + L + tick0 + 4 * v);
+      vb = io.ld4(0, tick0 + 4 * v);
+      va = io.ld4(1, tick0 + 4 * v);
     }
     b[4 * v] = vb.x; b[4 * v + 1] = vb.y; b[4 * v + 2] = vb.z; b[4 * v + 3] = vb.w;
     a[4 * v] = va.x; a[4 * v + 1] = va.y; a[4 * v + 2] = va.z; a[4 * v + 3] = va.w;
@@ -397,8 +423,8 @@ __device__ __forceinline__ void clear_window(int32_t* book, int L, int base, int
     if (in) {
 #pragma unroll
       for (int v = 0; v < K / 4; ++v) {
-        *reinterpret_cast<int4*>(book + tick0 + 4 * v) = make_int4(b[4 * v], b[4 * v + 1], b[4 * v + 2], b[4 * v + 3]);
-        *reinterpret_cast<int4*>(book + L + tick0 + 4 * v) = make_int4(a[4 * v], a[4 * v + 1], a[4 * v + 2], a[4 * v + 3]);
+        io.st4(0, tick0 + 4 * v, make_int4(b[4 * v], b[4 * v + 1], b[4 * v + 2], b[4 * v + 3]));
+        io.st4(1, tick0 + 4 * v, make_int4(a[4 * v], a[4 * v + 1], a[4 * v + 2], a[4 * v + 3]));
       }
     }
   }
@@ -416,14 +442,15 @@ __device__ __forceinline__ void clear_window(int32_t* book, int L, int base, int
 // General window of any width: chunks of 128 ticks, three passes (total bid depth; profiles and
 // arg max; residual and bounds).  Slow path: first step after a ks_write_books, or a window wider
 // than 256 ticks.  Same definitions as clear_window.
-static __device__ __noinline__ void clear_generic(int32_t* book, int L, int base, int top, int lane,
+template <class IO>
+static __device__ __noinline__ void clear_generic(const IO& io, int L, int base, int top, int lane,
                                            int& vmax, int& pstar, int& bmax_new, int& amin_new) {
   const unsigned FULL = 0xffffffffu;
   // pass 0: total bid depth of the window
   int tbsum = 0;
   for (int c = base; c <= top; c += 128) {
     int t = c + lane * 4;
-    if (t < L) { int4 vb = *reinterpret_cast<const int4*>(book + t); tbsum += vb.x + vb.y + vb.z + vb.w; }
+    if (t < L) { int4 vb = io.ld4(0, t); tbsum += vb.x + vb.y + vb.z + vb.w; }
   }
   const int TB = __reduce_add_sync(FULL, tbsum);
   int bestV = 0, bestp = 0x7fffffff;
@@ -435,7 +462,7 @@ static __device__ __noinline__ void clear_generic(int32_t* book, int L, int base
       int t = c + lane * 4;
       bool in = t < L;
       int4 vb = make_int4(0, 0, 0, 0), va = vb;
-      if (in) { vb = *reinterpret_cast<const int4*>(book + t); va = *reinterpret_cast<const int4*>(book + L + t); }
+      if (in) { vb = io.ld4(0, t); va = io.ld4(1, t); }
       int b[4] = {vb.x, vb.y, vb.z, vb.w}, a[4] = {va.x, va.y, va.z, va.w};
       int tb = b[0] + b[1] + b[2] + b[3], ta = a[0] + a[1] + a[2] + a[3];
       int preb = tb, prea = ta;
@@ -463,8 +490,8 @@ static __device__ __noinline__ void clear_generic(int32_t* book, int L, int base
         }
       }
       if (pass == 2 && in && vmax > 0) {
-        *reinterpret_cast<int4*>(book + t) = make_int4(b[0], b[1], b[2], b[3]);
-        *reinterpret_cast<int4*>(book + L + t) = make_int4(a[0], a[1], a[2], a[3]);
+        io.st4(0, t, make_int4(b[0], b[1], b[2], b[3]));
+        io.st4(1, t, make_int4(a[0], a[1], a[2], a[3]));
       }
       carryB += __shfl_sync(FULL, preb, 31);
       carryA += __shfl_sync(FULL, prea, 31);

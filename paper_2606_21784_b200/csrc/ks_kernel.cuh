@@ -139,9 +139,10 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
       int hi = min(L - 1, max(bmax, last + P.dmax));
       int vmax, pstar, nb, na;
       int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
-      if (P.force_generic || width8 > 256) clear_generic(book, L, lo & ~3, hi, lane, vmax, pstar, nb, na);
-      else if (width4 <= 128)              clear_window<4>(book, L, lo & ~3, lane, vmax, pstar, nb, na);
-      else                                 clear_window<8>(book, L, lo & ~7, lane, vmax, pstar, nb, na);
+      const LocalBook io{book, L};
+      if (P.force_generic || width8 > 256) clear_generic(io, L, lo & ~3, hi, lane, vmax, pstar, nb, na);
+      else if (width4 <= 128)              clear_window<4>(io, L, lo & ~3, lane, vmax, pstar, nb, na);
+      else                                 clear_window<8>(io, L, lo & ~7, lane, vmax, pstar, nb, na);
       bmax = nb; amin = na;
       if (lane == 0) {
         int new_last;

@@ -125,6 +125,55 @@ def test_market_base_shards_reproduce_the_global_run(ks, oracle):
     assert_rows_equal(b1, r1, np.arange(40), eb, er, "shard with market_base")
 
 
+# ------------------------------------------------------------------ cluster / DSMEM path
+@pytest.mark.parametrize("model", ["zi", "mix3"])
+def test_cluster_path_gives_identical_bytes(ks, oracle, model):
+    """north_star (2): the book split across the CTAs of a thread-block cluster (remote
+    shared-memory reductions, clearing through ld/st.shared::cluster) must give the bytes of the
+    oracle for every cluster size, block size, clearing path, split run and injected book."""
+    if model == "zi":
+        M, L, A, S, seed, p = 19, 256, 1000, 80, 9, zi_params(16, 100)
+    else:
+        M, L, A, S, seed, p = 11, 1024, 1541, 60, 4, mix3_params()
+    ids = np.arange(M)
+    eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+    for C in (2, 4, 8):
+        for T, clear, split in ((0, 0, None), (32, 1, None), (96, 0, [1, S - 1]), (1024, 0, None)):
+            b, r = _gpu(ks, M, L, A, p, seed, S, split=split,
+                        opts=[(ks.KS_OPT_CLUSTER_SIZE, C), (ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_CLEAR_PATH, clear)])
+            assert_rows_equal(b, r, ids, eb, er, "cluster C=%d T=%d clear=%d" % (C, T, clear))
+    # injected crossed books that span every CTA of the cluster; price pinned near a CTA boundary
+    books = random_books(M, L, seed=77, max_qty=40, fill=0.3)
+    eb0, er0 = oracle.init_state(M, L, -1)
+    eb, er = oracle_rows(oracle, p, L, A, seed, ids, 7, books=books, recs=er0)
+    for C in (2, 8):
+        b, r = _gpu(ks, M, L, A, p, seed, 7, books=books, opts=[(ks.KS_OPT_CLUSTER_SIZE, C)])
+        assert_rows_equal(b, r, ids, eb, er, "cluster injected C=%d" % C)
+
+
+def test_book_larger_than_one_sm(ks, oracle):
+    """L = 32768: 256 KB of book per market, more than one SM's shared memory -> the automatic
+    plan runs a 2-CTA cluster.  Opening price at the CTA boundary (L/2), so orders and the
+    clearing window straddle both CTAs' shared memory.  (The conservative int64 guard on the
+    fourth return moment, (L-1)^4 * steps < 2^63, allows 8 steps per record at this L.)"""
+    M, L, A, S, seed = 6, 32768, 3000, 8, 21
+    p = zi_params(64, 50)
+    ids = np.arange(M)
+    eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+    b, r = _gpu(ks, M, L, A, p, seed, S)
+    assert_rows_equal(b, r, ids, eb, er, "L=32768 auto cluster")
+    pm = mix3_params()
+    books = random_books(M, L, seed=5, max_qty=30, fill=0.05)
+    eb0, er0 = oracle.init_state(M, L, -1)
+    eb, er = oracle_rows(oracle, pm, L, 900, seed, ids, 5, books=books, recs=er0)
+    b, r = _gpu(ks, M, L, 900, pm, seed, 5, books=books, split=[2, 3])
+    assert_rows_equal(b, r, ids, eb, er, "L=32768 mix3 injected")
+    sim = ks.KsSim(1, L, 10, p, 0)
+    with pytest.raises(ks.KsError):
+        sim.ks_run(9)                                  # KS_ERR_OVERFLOW, nothing enqueued
+    sim.ks_destroy()
+
+
 # ------------------------------------------------------------------ book injection / edge cases
 def test_paper_worked_example_through_the_library(ks):
     """PAPER.md:315-354 (Eq.11-18) embedded at ticks 10..14 of an L=32 grid, A = 0: zero padding

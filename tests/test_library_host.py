@@ -70,7 +70,7 @@ def test_argument_validation_precedes_cuda(lib):
     assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(P), 0, fake + 4, None) == binding.KS_ERR_INVALID_ARG
     bad = binding._params(zi_params(8, 0))
     assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(bad), 0, fake, None) == binding.KS_ERR_INVALID_ARG
-    assert lib.ks_create(C.byref(h), 1, 32768, 256, C.byref(P), 0, fake, None) == binding.KS_ERR_UNSUPPORTED
+    assert lib.ks_create(C.byref(h), 1, 65536, 256, C.byref(P), 0, fake, None) == binding.KS_ERR_UNSUPPORTED
     assert h.value is None
     assert lib.ks_run(None, 1, None) == binding.KS_ERR_INVALID_ARG
     assert lib.ks_read_books(None, None, None) == binding.KS_ERR_INVALID_ARG
