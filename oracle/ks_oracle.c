@@ -30,7 +30,9 @@
  * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors,
  * the paper's worked example Eq.11-18, brute-force Eq.1-2 on tiny books, greedy
  * best-bid/best-ask matching, closed forms, per-step invariants, a numpy return
- * series for the derived statistics.  Parity unpinned: the paper's own aggregate
+ * series for the derived statistics; for the PACKED4 draw contract (models 2, 3) the
+ * first four orders by hand from KAT #1 and the exact mixed-radix identity
+ * (tests/test_oracle_packed.py).  Parity unpinned: the paper's own aggregate
  * numbers (Table II, Fig.7) -- its agent parameters and its RNG hash are not given.
  */
 #include <stdint.h>
@@ -43,7 +45,9 @@
 /* The oracle's own parameter block (field order is this file's business; the
  * Python wrapper oracle/ks_oracle.py fills it field by field). */
 typedef struct {
-  int32_t model;            /* 0 = zero-intelligence (all noise), 1 = three types by a mod 3 */
+  int32_t model;            /* 0 = zero-intelligence (all noise), 1 = three types by a mod 3;
+                               2, 3 = the same rules under the PACKED4 draw contract (see
+                               ko_gen_orders)                                                */
   int32_t noise_delta;      /* noise offset uniform in [-delta, +delta]                      */
   int32_t noise_qmax;       /* noise quantity uniform in 1..qmax                             */
   int32_t maker_spread_max; /* maker spread uniform in 1..spread_max                         */
@@ -105,10 +109,62 @@ static int32_t ko_clamp(int64_t x, int32_t L) {
  *   momentum dp = last - prev; buy = dp>0 ? 1 : dp<0 ? 0 : w0>>31; o = mulhi(w1, delta+1);
  *            q = 1 + mulhi(w2, qmax); tick = buy ? clamp(last + o) : clamp(last - o) (A12)
  * Type: model 0 -> all noise; model 1 -> a mod 3 = 0 noise, 1 maker, 2 momentum (A14).
+ *
+ * PACKED4 draw contract (models 2 = ZI rules, 3 = three types, DESIGN.md
+ * reading A22): a separately named contract, NOT the BASELINE.json one.  One Philox block
+ * serves four consecutive agents, w = Philox(ctr = (a >> 2, step, market, 0), key)[a & 3],
+ * and every draw of the agent comes out of that one word by successive multiply-extract
+ * (the high word of x*n is the draw, the low word is the still-unused randomness):
+ *   noise    o = mulhi(w, 2D+1) - D, x1 = lo32(w*(2D+1)); q = 1 + mulhi(x1, qmax),
+ *            x2 = lo32(x1*qmax); buy = x2>>31; tick as above
+ *   maker    s = 1 + mulhi(w, spread_max); orders as above
+ *   momentum o = mulhi(w, delta+1), x1 = lo32(w*(delta+1)); q = 1 + mulhi(x1, qmax),
+ *            x2 = lo32(x1*qmax); buy = dp>0 ? 1 : dp<0 ? 0 : x2>>31; tick as above
+ * Equivalently (exact integers): with N = n*qmax*2, J = floor(w*N / 2^32) and the draws
+ * are J's mixed-radix digits, J = ((o_index*qmax) + (q-1))*2 + buy -- which is how the
+ * pin in tests/test_oracle_packed.py checks them.
  * ---------------------------------------------------------------------------------------- */
+static int32_t ko_gen_orders_packed4(const ko_params* P, int32_t L, int32_t last, int32_t prev,
+                                     uint64_t seed, uint32_t m, uint32_t t, uint32_t a,
+                                     int32_t side[2], int32_t tick[2], int32_t qty[2]) {
+  uint32_t ctr[4] = { a >> 2, t, m, 0u };
+  uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+  uint32_t out[4];
+  ko_philox4x32_10(ctr, key, out);
+  const uint32_t w = out[a & 3u];
+  int type = 0;
+  if (P->model == 3) type = (int)(a % 3u);
+  if (type == 1) {
+    int64_t s = 1 + (int64_t)ko_mulhi(w, (uint32_t)P->maker_spread_max);
+    side[0] = 0; tick[0] = ko_clamp((int64_t)last - s, L); qty[0] = P->maker_qty;
+    side[1] = 1; tick[1] = ko_clamp((int64_t)last + s, L); qty[1] = P->maker_qty;
+    return 2;
+  }
+  const uint32_t n = type == 0 ? (uint32_t)(2 * P->noise_delta + 1) : (uint32_t)(P->mom_delta + 1);
+  const uint32_t qmax = type == 0 ? (uint32_t)P->noise_qmax : (uint32_t)P->mom_qmax;
+  const uint32_t oi = ko_mulhi(w, n);
+  const uint32_t x1 = (uint32_t)((uint64_t)w * (uint64_t)n);
+  const int32_t q = 1 + (int32_t)ko_mulhi(x1, qmax);
+  const uint32_t x2 = (uint32_t)((uint64_t)x1 * (uint64_t)qmax);
+  const int coin = (int)(x2 >> 31);
+  if (type == 0) {
+    int64_t o = (int64_t)oi - (int64_t)P->noise_delta;
+    side[0] = coin ? 0 : 1;
+    tick[0] = coin ? ko_clamp((int64_t)last - o, L) : ko_clamp((int64_t)last + o, L);
+  } else {
+    int64_t dp = (int64_t)last - (int64_t)prev;
+    int buy = dp > 0 ? 1 : (dp < 0 ? 0 : coin);
+    side[0] = buy ? 0 : 1;
+    tick[0] = buy ? ko_clamp((int64_t)last + (int64_t)oi, L) : ko_clamp((int64_t)last - (int64_t)oi, L);
+  }
+  qty[0] = q;
+  return 1;
+}
+
 KO_API int32_t ko_gen_orders(const ko_params* P, int32_t L, int32_t last, int32_t prev,
                              uint64_t seed, uint32_t m, uint32_t t, uint32_t a,
                              int32_t side[2], int32_t tick[2], int32_t qty[2]) {
+  if (P->model >= 2) return ko_gen_orders_packed4(P, L, last, prev, seed, m, t, a, side, tick, qty);
   uint32_t ctr[4] = { a, t, m, 0u };
   uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
   uint32_t w[4];

@@ -14,6 +14,16 @@ import numpy as np
 
 KS_MODEL_ZI = 0
 KS_MODEL_MIX3 = 1
+KS_MODEL_ZI_PACKED4 = 2      # the same rules under the PACKED4 draw contract (A22)
+KS_MODEL_MIX3_PACKED4 = 3
+
+
+def packed4(params: dict) -> dict:
+    """The same agent parameters under the PACKED4 draw contract (one Philox block per four
+    consecutive agents; a separately named contract)."""
+    q = dict(params)
+    q["model"] = {KS_MODEL_ZI: KS_MODEL_ZI_PACKED4, KS_MODEL_MIX3: KS_MODEL_MIX3_PACKED4}[params["model"]]
+    return q
 
 
 def zi_params(delta: int, qmax: int, init_price: int = -1) -> dict:
