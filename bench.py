@@ -25,16 +25,21 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2606_21784_b200.workloads import CONFIGS, KS_MODEL_ZI, sampled_markets  # noqa: E402
+import dataclasses  # noqa: E402
+
+from paper_2606_21784_b200.workloads import CONFIGS, KS_MODEL_ZI, packed4, sampled_markets  # noqa: E402
 
 # Roofline of ks_persistent_kernel: the fmaheavy pipe that executes the 32x32->64
 # multiplies.  Algorithmic multiplies per agent event: 20 of Philox4x32-10 + the
 # mulhi draws of the rule (noise/momentum: offset and quantity; maker: spread only).
-ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0}
+ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0,
+                       # PACKED4 (A22): a Philox block per 4 agents + the rule's multiply-extract draws
+                       "zi_packed4": 20.0 / 4 + 2.0, "mix3_packed4": 20.0 / 4 + (2.0 + 1.0 + 2.0) / 3.0}
 # Multiplies the kernel actually issues per event (IMAD.WIDE.U32 + IMAD.HI.U32 in the hot loop,
 # from cuobjdump -sass): hoisting of (market, step)-uniform products, round 0's M0*agent carried as
 # a running 64-bit sum, w3 never computed.
-EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 17.0 + 19.0) / 3.0}
+EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 17.0 + 19.0) / 3.0,
+                        "zi_packed4": 17.0 / 4 + 2.0, "mix3_packed4": 17.0 / 4 + (2.0 + 1.0 + 2.0) / 3.0}
 # a 32-lane IMAD.WIDE/IMAD.HI occupies an SMSP's fmaheavy pipe for 4 cycles -> 8 lanes/clk/SMSP
 WIDE_MUL_LANES_PER_SM_PER_CLK = 4 * 8
 
@@ -135,7 +140,8 @@ def run_reference(args, cfg, rank: int):
 def workload_config(cfg, n_gpus):
     return {"workload": "%s: BASELINE.json configs[%d] -- M=%d markets/GPU, L=%d ticks, A=%d agents, S=%d steps, seed=%d, %s"
                         % (cfg.name, int(cfg.name[1]) - 1, cfg.M, cfg.L, cfg.A, cfg.S, cfg.seed,
-                           "zero-intelligence" if cfg.params["model"] == KS_MODEL_ZI else "noise/maker/momentum by a%3"),
+                           ("zero-intelligence" if (cfg.params["model"] & 1) == KS_MODEL_ZI else "noise/maker/momentum by a%3")
+                           + (", PACKED4 draw contract (NOT the BASELINE.json one; DESIGN.md A22)" if cfg.params["model"] >= 2 else "")),
             "M_per_gpu": cfg.M, "L": cfg.L, "A": cfg.A, "S": cfg.S, "seed": cfg.seed,
             "parallelism": "markets sharded across %d GPU(s), market_base = rank*M, no collective" % n_gpus,
             "l2": "state buffer %.0f MB per GPU exceeds the 126 MB L2; written once per step" % (cfg.M * (8 * cfg.L + 128) / 1e6)}
@@ -150,11 +156,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--threads", type=int, default=0, help="KS_OPT_BLOCK_THREADS (0 = automatic)")
     ap.add_argument("--atomic-mode", type=int, default=0)
+    ap.add_argument("--rng", default="literal", choices=["literal", "packed4"],
+                    help="draw contract: literal = BASELINE.json (one Philox block per agent); packed4 = the "
+                         "separately named PACKED4 contract (DESIGN.md A22), reported beside it, never instead of it")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-microbench", action="store_true")
     ap.add_argument("--all-configs", action="store_true", help="also time C1..C5 (extra keys)")
     args = ap.parse_args()
     cfg = CONFIGS[args.config]
+    if args.rng == "packed4":
+        cfg = dataclasses.replace(cfg, params=packed4(cfg.params))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -271,7 +282,7 @@ def main():
         return
 
     # ---- roofline of the dominant kernel (ks_persistent_kernel): ALU / issue bound
-    model = "zi" if cfg.params["model"] == KS_MODEL_ZI else "mix3"
+    model = ("zi" if (cfg.params["model"] & 1) == KS_MODEL_ZI else "mix3") + ("_packed4" if cfg.params["model"] >= 2 else "")
     avg_kern_s = float(np.mean(kern_ms)) * 1e-3
     peaks = {}
     try:
@@ -286,7 +297,7 @@ def main():
     executed = EXEC_MULTS_PER_EVENT[model] * events_per_step / avg_kern_s / 1e12
     roofline = {"bound": "alu", "kernel": "ks_persistent_kernel", "achieved": achieved, "peak": peak,
                 "unit": "T 32x32->64-bit integer multiplies/s", "frac": achieved / peak,
-                "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name),
+                "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name if args.rng == "literal" else cfg.name + "_packed4"),
                 "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "avg_launch_ms": avg_kern_s * 1e3,
                 "executed_mults_per_event": EXEC_MULTS_PER_EVENT[model], "fmaheavy_pipe_frac_from_executed": executed / peak,
                 "peak_source": "derived (DESIGN.md 7.2): %d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
@@ -325,7 +336,7 @@ def main():
         wide, _ = ks.ks_bench_int_pipe(0)
         lop, _ = ks.ks_bench_int_pipe(1)
         mix, _ = ks.ks_bench_int_pipe(2)
-        atomics_per_event = 1.0 if model == "zi" else 4.0 / 3.0
+        atomics_per_event = 1.0 if model.startswith("zi") else 4.0 / 3.0
         kev = events_per_step / avg_kern_s
         line["microbench"] = {
             "smem_atomic_peak_lane_ops_per_s": peak_ops, "smem_atomic_pattern_lane_ops_per_s": pat_ops,

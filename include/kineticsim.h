@@ -56,7 +56,15 @@ typedef enum {
 
 typedef enum {
   KS_MODEL_ZI = 0,  /* every agent is a zero-intelligence noise trader (BASELINE.json configs[0..3]) */
-  KS_MODEL_MIX3 = 1 /* agent a: a%3 = 0 noise, 1 market maker, 2 momentum (BASELINE.json configs[4]) */
+  KS_MODEL_MIX3 = 1, /* agent a: a%3 = 0 noise, 1 market maker, 2 momentum (BASELINE.json configs[4]) */
+  /* The same rules under the PACKED4 draw contract (reading A22) -- a
+   * separately named contract with its own orders, NOT the BASELINE.json one: one Philox block
+   * serves four consecutive agents, w = Philox(ctr = (a >> 2, step, market, 0), key)[a & 3], and
+   * every draw comes out of that word by successive multiply-extract: o = mulhi(w, n),
+   * x1 = lo32(w*n); q = 1 + mulhi(x1, qmax), x2 = lo32(x1*qmax); coin = x2 >> 31 (maker:
+   * s = 1 + mulhi(w, spread_max)).  Plain atomics only (KS_OPT_ATOMIC_MODE 0). */
+  KS_MODEL_ZI_PACKED4 = 2,
+  KS_MODEL_MIX3_PACKED4 = 3
 } ks_model;
 
 /*

@@ -89,11 +89,11 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   if (M < 1 || A < 0 || !is_pow2(L) || L < 32) { set_err("ks_create: need M >= 1, A >= 0, L a power of two >= 32"); return KS_ERR_INVALID_ARG; }
   if (L > kMaxL) { set_err("ks_create: L > 32768 is not supported (p* must fit 16 bits of the trajectory hash)"); return KS_ERR_UNSUPPORTED; }
   if ((reinterpret_cast<uintptr_t>(d_state) & 15) != 0) { set_err("ks_create: d_state must be 16-byte aligned"); return KS_ERR_INVALID_ARG; }
-  if (p->model != KS_MODEL_ZI && p->model != KS_MODEL_MIX3) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
+  if (p->model < KS_MODEL_ZI || p->model > KS_MODEL_MIX3_PACKED4) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
   if (p->noise_delta < 0 || p->noise_delta >= L || p->noise_qmax < 1 || p->noise_qmax > kMaxQty || p->init_price >= L) {
     set_err("ks_create: bad noise parameters or init_price"); return KS_ERR_INVALID_ARG;
   }
-  if (p->model == KS_MODEL_MIX3 &&
+  if ((p->model & 1) == KS_MODEL_MIX3 &&
       (p->maker_spread_max < 1 || p->maker_spread_max > L || p->maker_qty < 1 || p->maker_qty > kMaxQty ||
        p->mom_delta < 0 || p->mom_delta >= L || p->mom_qmax < 1 || p->mom_qmax > kMaxQty)) {
     set_err("ks_create: bad maker/momentum parameters"); return KS_ERR_INVALID_ARG;
@@ -116,7 +116,7 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0;
   s->dev_smem_optin = optin; s->num_sms = sms;
   s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
-  if (p->model == KS_MODEL_ZI) {
+  if ((p->model & 1) == KS_MODEL_ZI) {
     s->n_noise = A; s->n_maker = 0; s->n_mom = 0;
     s->inflow_per_step = (int64_t)A * p->noise_qmax;
   } else {
@@ -169,6 +169,7 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_ATOMIC_MODE:
       if (value != 0 && value != 1) break;
       if (value == 1 && (s->opt_cluster > 1 || s->L > kMaxLPerCta)) break;   // the cluster kernel has plain atomics only
+      if (value == 1 && s->p.model >= KS_MODEL_ZI_PACKED4) break;            // so has the PACKED4 path
       s->opt_atomic = value; return KS_OK;
     case KS_OPT_CLEAR_PATH:
       if (value != 0 && value != 1) break;
@@ -218,9 +219,9 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   return pl;
 }
 
-template <int MODEL, int ATOM>
+template <int MODEL, int ATOM, bool PACKED>
 static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_persistent_kernel<MODEL, ATOM>;
+  auto kern = ks::ks_persistent_kernel<MODEL, ATOM, PACKED>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -231,9 +232,9 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
 
 // Cluster launch: grid = M*C CTAs in clusters of C (cluster <-> market), 8*L/C bytes of shared
 // memory per CTA.
-template <int MODEL>
+template <int MODEL, bool PACKED>
 static cudaError_t launch_cluster(const ks::KernelParams& P, int C, int T, cudaStream_t st) {
-  auto kern = ks::ks_cluster_kernel<MODEL>;
+  auto kern = ks::ks_cluster_kernel<MODEL, PACKED>;
   const size_t smem = (size_t)8 * (size_t)(P.L / C);
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
@@ -281,7 +282,7 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   P.maker_spread_max = s->p.maker_spread_max; P.maker_qty = s->p.maker_qty;
   P.mom_n = s->p.mom_delta + 1; P.mom_qmax = s->p.mom_qmax;
   P.dmax = s->p.noise_delta;
-  if (s->p.model == KS_MODEL_MIX3) {
+  if ((s->p.model & 1) == KS_MODEL_MIX3) {
     if (s->p.maker_spread_max > P.dmax) P.dmax = s->p.maker_spread_max;
     if (s->p.mom_delta > P.dmax) P.dmax = s->p.mom_delta;
   }
@@ -292,6 +293,7 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
 
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
+  const bool mix = (s->p.model & 1) == KS_MODEL_MIX3, packed = s->p.model >= KS_MODEL_ZI_PACKED4;
   int C = s->opt_cluster;
   if (C == 0) C = s->L > kMaxLPerCta ? s->L / kMaxLPerCta : 1;
   if (C > 1) {
@@ -302,13 +304,16 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
     while ((1 << log2C) < C) ++log2C;
     P.log2C = log2C;
     if ((long long)s->M * C > 0x7fffffffLL) { set_err("%s: M * cluster size exceeds the grid limit", who); return KS_ERR_UNSUPPORTED; }
-    e = s->p.model == KS_MODEL_ZI ? launch_cluster<0>(P, C, T, st) : launch_cluster<1>(P, C, T, st);
+    if (!packed) e = mix ? launch_cluster<1, false>(P, C, T, st) : launch_cluster<0, false>(P, C, T, st);
+    else         e = mix ? launch_cluster<1, true>(P, C, T, st) : launch_cluster<0, true>(P, C, T, st);
   } else {
     const LaunchPlan pl = plan_launch(s);
-    if (s->p.model == KS_MODEL_ZI)
-      e = s->opt_atomic ? launch_persistent<0, 1>(P, pl.T, pl.smem, st) : launch_persistent<0, 0>(P, pl.T, pl.smem, st);
+    if (packed)
+      e = mix ? launch_persistent<1, 0, true>(P, pl.T, pl.smem, st) : launch_persistent<0, 0, true>(P, pl.T, pl.smem, st);
+    else if (!mix)
+      e = s->opt_atomic ? launch_persistent<0, 1, false>(P, pl.T, pl.smem, st) : launch_persistent<0, 0, false>(P, pl.T, pl.smem, st);
     else
-      e = s->opt_atomic ? launch_persistent<1, 1>(P, pl.T, pl.smem, st) : launch_persistent<1, 0>(P, pl.T, pl.smem, st);
+      e = s->opt_atomic ? launch_persistent<1, 1, false>(P, pl.T, pl.smem, st) : launch_persistent<1, 0, false>(P, pl.T, pl.smem, st);
   }
   if (e != cudaSuccess) { set_err("%s: launch failed: %s", who, cudaGetErrorString(e)); return KS_ERR_CUDA; }
   g_launches++;

@@ -56,7 +56,7 @@ struct ClusterBook {
 
 // grid = M*C CTAs in clusters of C = 1 << P.log2C (cluster <-> market), block = T threads,
 // dynamic shared memory = 8*Lc bytes.  MODEL: 0 = ZI, 1 = MIX3.
-template <int MODEL>
+template <int MODEL, bool PACKED>
 __global__ void ks_cluster_kernel(const __grid_constant__ KernelParams P) {
   extern __shared__ __align__(16) int32_t book[];     // [2][Lc]: this CTA's ticks, bid then ask
   __shared__ long long s_rec[16];
@@ -77,7 +77,7 @@ __global__ void ks_cluster_kernel(const __grid_constant__ KernelParams P) {
   int32_t* gbook = P.books + (size_t)cluster_id * 2 * (size_t)L;
   long long* grec = P.recs + (size_t)cluster_id * 16;
   const MarketUniform mu = market_uniform(P, market);
-  const GenPlan<MODEL> gplan = gen_plan<MODEL>(P, (int)rank * T + tid, C * T);
+  const GenPlan<MODEL> gplan = gen_plan<MODEL>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, (int)rank * T + tid, C * T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
   bref.log2L = log2L; bref.log2Lc = log2Lc;
   const ClusterBook io{bref.saddr, log2Lc};
@@ -142,7 +142,7 @@ __global__ void ks_cluster_kernel(const __grid_constant__ KernelParams P) {
     last = s_ctl[0];
     RuleCtx rc;
     rc.last = last; rc.dp = last - prev; rc.L = L; rc.noclamp = false; rc.bid_lo = 0; rc.ask_lo = 0;
-    generate_step<MODEL, 3>(P, bref, mu, u, rc, gplan, sink);
+    generate_step<MODEL, 3, PACKED>(P, bref, mu, u, rc, gplan, rank == 0 && tid == 0, sink);
     cluster_sync();                                    // B1: the combined book is complete in every CTA
 
     if (rank == 0 && warp == 0) {

@@ -103,10 +103,9 @@ __device__ __forceinline__ StepUniform step_uniform(const KernelParams& P, const
 // Philox4x32-10 of agent a from p0 = M0*a (round 0's product).  Outputs w0, w1, w2 (w3 is
 // reserved and never computed).  NEED02 = false skips the last round's M0 product and w0 (the
 // maker rule reads w1 only).
-template <bool NEED02>
-__device__ __forceinline__ void philox_from_p0(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
-                                               uint64_t p0, uint32_t& w0, uint32_t& w1, uint32_t& w2) {
-  uint32_t c0, c1, c2, c3;
+// rounds 0..8 from p0 = M0*c0_in: the state (c0, c1, c2, c3) that enters the last round
+__device__ __forceinline__ void philox_rounds_0_8(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
+                                                  uint64_t p0, uint32_t& c0, uint32_t& c1, uint32_t& c2, uint32_t& c3) {
   {                                       // rounds 0-1
     const uint32_t n2 = hi32(p0) ^ P.k1[0];
     const uint64_t p1 = (uint64_t)kPhiloxM1 * n2;
@@ -132,6 +131,13 @@ __device__ __forceinline__ void philox_from_p0(const KernelParams& P, const Mark
     c0 = t0;
     c2 = t2;
   }
+}
+
+template <bool NEED02>
+__device__ __forceinline__ void philox_from_p0(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
+                                               uint64_t p0, uint32_t& w0, uint32_t& w1, uint32_t& w2) {
+  uint32_t c0, c1, c2, c3;
+  philox_rounds_0_8(P, mu, u, p0, c0, c1, c2, c3);
   uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
   w1 = lo32(a1);
   if (NEED02) {
@@ -140,6 +146,19 @@ __device__ __forceinline__ void philox_from_p0(const KernelParams& P, const Mark
   } else {
     w0 = 0; w2 = 0;
   }
+}
+
+// PACKED4 contract (A22): all four words of the block of agents 4b..4b+3, p0 = M0*b.
+__device__ __forceinline__ void philox_block_from_p0(const KernelParams& P, const MarketUniform& mu,
+                                                     const StepUniform& u, uint64_t p0, uint32_t (&w)[4]) {
+  uint32_t c0, c1, c2, c3;
+  philox_rounds_0_8(P, mu, u, p0, c0, c1, c2, c3);
+  const uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
+  const uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
+  w[0] = hi32(a1) ^ c1 ^ P.k0[9];
+  w[1] = lo32(a1);
+  w[2] = hi32(a0) ^ c3 ^ P.k1[9];
+  w[3] = lo32(a0);
 }
 
 // a2: add one order to the shared-memory book at byte offset `off` from the start of the [2][L]
@@ -243,6 +262,52 @@ __device__ __forceinline__ void momentum_order(const KernelParams& P, const Book
   book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
 }
 
+// ---- PACKED4 rules (A22): every draw of an agent out of ONE word by successive
+// multiply-extract: o = hi(w*n), x1 = lo(w*n); q-1 = hi(x1*qmax), x2 = lo(x1*qmax); coin = x2>>31.
+// Two IMAD.WIDE per agent (the +1 of q rides in the second one's 64-bit addend).
+// No-clamp noise path: m = coin mask (all-ones for a buy); sell tick = (last-delta) + o, buy tick
+// = (last-delta) + (n-1-o) = (last-delta+n) + ~o, so addr = base(m) + 4*(o ^ m) with
+// base = &ask[last-delta] or &bid[last-delta+n]: SHF + 2 LOP3 + LEA on the alu pipe.
+template <int ATOM, bool CLAMP>
+__device__ __forceinline__ void noise_order_packed(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                                   uint32_t w, int& sink) {
+  const uint64_t p1 = (uint64_t)w * (uint32_t)P.noise_n;
+  const uint64_t p2 = (uint64_t)lo32(p1) * (uint32_t)P.noise_qmax + P.q_addend;
+  const int q = (int)hi32(p2);
+  const uint32_t o = hi32(p1);
+  if (!CLAMP) {
+    const uint32_t m = (uint32_t)((int32_t)lo32(p2) >> 31);
+    const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
+    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top));
+    book_add_at<ATOM>(book, base + ((o ^ m) << 2), q, sink);
+  } else {
+    const bool buy = (int32_t)lo32(p2) < 0;
+    const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - (int)o : (rc.last - P.noise_delta) + (int)o, rc.L);
+    book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
+  }
+}
+
+template <int ATOM>
+__device__ __forceinline__ void momentum_order_packed(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                                      uint32_t w, int& sink) {
+  const uint64_t p1 = (uint64_t)w * (uint32_t)P.mom_n;
+  const uint64_t p2 = (uint64_t)lo32(p1) * (uint32_t)P.mom_qmax + P.q_addend;
+  const int q = (int)hi32(p2);
+  const int o = (int)hi32(p1);
+  const bool buy = rc.dp > 0 ? true : (rc.dp < 0 ? false : ((int32_t)lo32(p2) < 0));
+  const int tick = clamp_tick(buy ? rc.last + o : rc.last - o, rc.L);
+  book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
+}
+
+// One agent of type KIND under PACKED4 from its word.
+template <int ATOM, int KIND, bool CLAMP>
+__device__ __forceinline__ void packed_agent(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                             uint32_t w, int& sink) {
+  if (KIND == 0)      noise_order_packed<ATOM, CLAMP>(P, book, rc, w, sink);
+  else if (KIND == 1) maker_order<ATOM>(P, book, rc, w, sink);
+  else                momentum_order_packed<ATOM>(P, book, rc, w, sink);
+}
+
 // The agents of one class that a thread visits: first, first + a_step, ... < a_end.  p0 = M0*first;
 // n_uniform trips are made by every thread of the CTA (a uniform loop, no per-agent bound
 // check), `extra` marks the threads that own one agent more (ragged tail).
@@ -290,6 +355,44 @@ __device__ __forceinline__ void generate_class(const KernelParams& P, const Book
   if (pl.extra) one(p0);
 }
 
+// PACKED4: one class of BLOCKS of four agents.  MIX = false: all noise.  MIX = true: the blocks of
+// class CLS are b = 3i + CLS, so agent 4b + j has type (4b + j) mod 3 = (CLS + j) mod 3 -- uniform
+// over the warp for every j.
+template <int ATOM, bool MIX, int CLS, bool CLAMP>
+__device__ __forceinline__ void generate_class_packed(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                                      const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
+                                                      uint64_t p0_inc, int& sink) {
+  auto one = [&](uint64_t p0) {
+    uint32_t w[4];
+    philox_block_from_p0(P, mu, u, p0, w);
+    packed_agent<ATOM, MIX ? (CLS + 0) % 3 : 0, CLAMP>(P, book, rc, w[0], sink);
+    packed_agent<ATOM, MIX ? (CLS + 1) % 3 : 0, CLAMP>(P, book, rc, w[1], sink);
+    packed_agent<ATOM, MIX ? (CLS + 2) % 3 : 0, CLAMP>(P, book, rc, w[2], sink);
+    packed_agent<ATOM, MIX ? (CLS + 3) % 3 : 0, CLAMP>(P, book, rc, w[3], sink);
+  };
+  uint64_t p0 = pl.p0;
+#pragma unroll kGenUnroll
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
+  if (pl.extra) one(p0);
+}
+
+// PACKED4: the ragged last block (A mod 4 != 0), agents 4b .. A-1, by one thread; types at run time.
+template <int ATOM, bool MIX>
+__device__ __noinline__ void generate_partial_block_packed(const KernelParams& P, const BookRef& book,
+                                                           const MarketUniform& mu, const StepUniform& u,
+                                                           const RuleCtx& rc, int& sink) {
+  const uint32_t b = (uint32_t)P.A >> 2, rem = (uint32_t)P.A & 3u;
+  uint32_t w[4];
+  philox_block_from_p0(P, mu, u, (uint64_t)kPhiloxM0 * b, w);
+  for (uint32_t j = 0; j < rem; ++j) {
+    const uint32_t kind = MIX ? (4u * b + j) % 3u : 0u;
+    const uint32_t wj = j == 0 ? w[0] : (j == 1 ? w[1] : w[2]);
+    if (kind == 0)      packed_agent<ATOM, 0, true>(P, book, rc, wj, sink);
+    else if (kind == 1) packed_agent<ATOM, 1, true>(P, book, rc, wj, sink);
+    else                packed_agent<ATOM, 2, true>(P, book, rc, wj, sink);
+  }
+}
+
 // The per-thread plans of a launch: MODEL 0 one class (a = tid + k*T), MODEL 1 three classes
 // (agent a = 3j + c has type c, j = tid + k*T; each class runs in its own warp-uniform loop --
 // integer atomics commute, so the agent -> thread mapping cannot change a byte of the result).
@@ -299,19 +402,20 @@ struct GenPlan {
   uint64_t p0_inc;       // M0 * a_step
 };
 
+// `count` = number of items the classes enumerate: agents (literal contract) or full blocks of four
+// agents (PACKED4).
 template <int MODEL>
-__device__ __forceinline__ GenPlan<MODEL> gen_plan(const KernelParams& P, int tid, int T) {
+__device__ __forceinline__ GenPlan<MODEL> gen_plan(uint32_t count, int tid, int T) {
   GenPlan<MODEL> g;
-  const uint32_t A = (uint32_t)P.A;
   if (MODEL == 0) {
     g.p0_inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
-    g.cls[0] = class_plan((uint32_t)tid, (uint32_t)(T - 1), A, (uint32_t)T);
+    g.cls[0] = class_plan((uint32_t)tid, (uint32_t)(T - 1), count, (uint32_t)T);
   } else {
     const uint32_t st = 3u * (uint32_t)T;
     g.p0_inc = (uint64_t)kPhiloxM0 * st;
 #pragma unroll
     for (int c = 0; c < (MODEL == 0 ? 1 : 3); ++c)
-      g.cls[c] = class_plan(3u * (uint32_t)tid + (uint32_t)c, 3u * (uint32_t)(T - 1) + (uint32_t)c, A, st);
+      g.cls[c] = class_plan(3u * (uint32_t)tid + (uint32_t)c, 3u * (uint32_t)(T - 1) + (uint32_t)c, count, st);
   }
   // hide that p0_inc is a product: otherwise p0 += p0_inc is turned back into IMAD.WIDE(M0, a_step, p0)
   asm volatile("" : "+l"(g.p0_inc));
@@ -319,15 +423,35 @@ __device__ __forceinline__ GenPlan<MODEL> gen_plan(const KernelParams& P, int ti
 }
 
 // a1 + a2 for one market-step: every thread of the CTA generates the orders of its agents.
-template <int MODEL, int ATOM>
+// `first_thread`: this is thread 0 of the market's thread set (owns PACKED4's ragged last block).
+template <int MODEL, int ATOM, bool PACKED>
 __device__ __forceinline__ void generate_step(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                               const StepUniform& u, const RuleCtx& rc, const GenPlan<MODEL>& g,
-                                              int& sink) {
-  if (ATOM != 3 && rc.noclamp) generate_class<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
-  else            generate_class<ATOM, 0, true >(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
-  if (MODEL == 1) {
-    generate_class<ATOM, 1, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 1], g.p0_inc, sink);
-    generate_class<ATOM, 2, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 2], g.p0_inc, sink);
+                                              bool first_thread, int& sink) {
+  const bool fast = ATOM != 3 && rc.noclamp;
+  if (!PACKED) {
+    if (fast) generate_class<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+    else      generate_class<ATOM, 0, true >(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+    if (MODEL == 1) {
+      generate_class<ATOM, 1, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 1], g.p0_inc, sink);
+      generate_class<ATOM, 2, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 2], g.p0_inc, sink);
+    }
+  } else {
+    if (MODEL == 0) {
+      if (fast) generate_class_packed<ATOM, false, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+      else      generate_class_packed<ATOM, false, 0, true >(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+    } else {
+      if (fast) {
+        generate_class_packed<ATOM, true, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+        generate_class_packed<ATOM, true, 1, false>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 1], g.p0_inc, sink);
+        generate_class_packed<ATOM, true, 2, false>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 2], g.p0_inc, sink);
+      } else {
+        generate_class_packed<ATOM, true, 0, true>(P, book, mu, u, rc, g.cls[0], g.p0_inc, sink);
+        generate_class_packed<ATOM, true, 1, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 1], g.p0_inc, sink);
+        generate_class_packed<ATOM, true, 2, true>(P, book, mu, u, rc, g.cls[MODEL == 0 ? 0 : 2], g.p0_inc, sink);
+      }
+    }
+    if ((P.A & 3) != 0 && first_thread) generate_partial_block_packed<ATOM, MODEL == 1>(P, book, mu, u, rc, sink);
   }
 }
 

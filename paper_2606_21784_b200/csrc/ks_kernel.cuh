@@ -61,8 +61,9 @@ __device__ __forceinline__ void update_record(long long* rec, int last, int vmax
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
 // dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
+// PACKED: the PACKED4 draw contract (one Philox block per four agents, A22).
 // ---------------------------------------------------------------------------------------------
-template <int MODEL, int ATOM>
+template <int MODEL, int ATOM, bool PACKED>
 __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
   __shared__ long long s_rec[16];
@@ -77,7 +78,7 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   long long* grec = P.recs + (size_t)blockIdx.x * 16;
   const MarketUniform mu = market_uniform(P, market);
 
-  const GenPlan<MODEL> gplan = gen_plan<MODEL>(P, tid, T);
+  const GenPlan<MODEL> gplan = gen_plan<MODEL>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, tid, T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
 
   // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
@@ -130,7 +131,7 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
     rc.last = last; rc.dp = last - prev; rc.L = L;
     rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
     // a1 + a2: order generation and aggregation
-    generate_step<MODEL, ATOM>(P, bref, mu, u, rc, gplan, sink);
+    generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
     __syncthreads();                                   // B1: the combined book is complete
 
     // a3-a6: clearing by warp 0 on the active window

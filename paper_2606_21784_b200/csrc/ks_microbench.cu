@@ -43,19 +43,19 @@ __global__ void smem_atomic_kernel(int L, int delta, int iters, int* out) {
 }
 
 // ---- (2) generation only ---------------------------------------------------------------------
-template <int MODEL>
+template <int MODEL, bool PACKED>
 __global__ void generate_only_kernel(const __grid_constant__ ks::KernelParams P, int* out) {
   const int tid = threadIdx.x, T = blockDim.x;
   const uint32_t market = P.market_base + blockIdx.x;
   const ks::MarketUniform mu = ks::market_uniform(P, market);
-  const ks::GenPlan<MODEL> gplan = ks::gen_plan<MODEL>(P, tid, T);
+  const ks::GenPlan<MODEL> gplan = ks::gen_plan<MODEL>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, tid, T);
   ks::BookRef bref; bref.ptr = nullptr; bref.saddr = 0;
   int sink = 0;
   int last = P.L / 2, prev = P.L / 2;
   for (long long s = 0; s < P.S; ++s) {
     const ks::StepUniform u = ks::step_uniform(P, mu, (uint32_t)s);
     const ks::RuleCtx rc = ks::rule_ctx(P, bref, last, prev);
-    ks::generate_step<MODEL, 2>(P, bref, mu, u, rc, gplan, sink);
+    ks::generate_step<MODEL, 2, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
   }
   if (sink == 0x12345678) out[0] = sink;
 }
@@ -172,10 +172,15 @@ ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L,
   cudaStream_t st = (cudaStream_t)stream;
   int* d_out = nullptr;
   if (cudaMalloc(&d_out, 64) != cudaSuccess) return KS_ERR_CUDA;
-  const int model = p->model;
+  const int model = p->model & 1, packed = p->model >> 1;
   auto launch = [&]() {
-    if (model == KS_MODEL_ZI) generate_only_kernel<0><<<M, threads, smem, st>>>(P, d_out);
-    else                      generate_only_kernel<1><<<M, threads, smem, st>>>(P, d_out);
+    if (model == 0) {
+      if (packed) generate_only_kernel<0, true><<<M, threads, smem, st>>>(P, d_out);
+      else        generate_only_kernel<0, false><<<M, threads, smem, st>>>(P, d_out);
+    } else {
+      if (packed) generate_only_kernel<1, true><<<M, threads, smem, st>>>(P, d_out);
+      else        generate_only_kernel<1, false><<<M, threads, smem, st>>>(P, d_out);
+    }
   };
   ks_status rc = time_best(launch, warmup, reps, st, seconds);
   cudaFree(d_out);

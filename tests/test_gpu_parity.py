@@ -5,7 +5,8 @@ import numpy as np
 import pytest
 
 from ks_testlib import assert_rows_equal, ints, oracle_rows, read_golden
-from paper_2606_21784_b200.workloads import (CONFIGS, mix3_params, random_books, sampled_markets, zi_params)
+from paper_2606_21784_b200.workloads import (CONFIGS, mix3_params, packed4, random_books, sampled_markets,
+                                             zi_params)
 
 pytestmark = pytest.mark.gpu
 
@@ -172,6 +173,51 @@ def test_book_larger_than_one_sm(ks, oracle):
     with pytest.raises(ks.KsError):
         sim.ks_run(9)                                  # KS_ERR_OVERFLOW, nothing enqueued
     sim.ks_destroy()
+
+
+# ------------------------------------------------------------------ PACKED4 draw contract
+@pytest.mark.parametrize("model", ["zi", "mix3"])
+def test_packed4_contract_matches_the_oracle(ks, oracle, model):
+    """SURVEY.md S8(f)-1 / DESIGN.md A22: one Philox block per four agents, draws by successive
+    multiply-extract.  Ragged agent counts (A mod 4 = 0..3, A < 4), every block size, both
+    clearing paths, split and launch-per-step runs, the cluster path, prices pinned to the grid
+    edges (clamp path) -- all bit-exact against the oracle's PACKED4 mode."""
+    if model == "zi":
+        M, L, S, seed, p = 23, 256, 70, 9, packed4(zi_params(16, 100))
+    else:
+        M, L, S, seed, p = 13, 1024, 50, 4, packed4(mix3_params())
+    ids = np.arange(M)
+    for A in (1000, 1001, 1002, 1003, 3, 0):
+        eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+        for T in ((0, 32, 96, 1024) if A == 1001 else (0,)):
+            b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T)])
+            assert_rows_equal(b, r, ids, eb, er, "packed4 A=%d T=%d" % (A, T))
+    A = 1001
+    eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+    for kw in (dict(split=[1, 9, S - 10]), dict(stepwise=True), dict(opts=[(ks.KS_OPT_CLEAR_PATH, 1)]),
+               dict(opts=[(ks.KS_OPT_CLUSTER_SIZE, 2)]), dict(opts=[(ks.KS_OPT_CLUSTER_SIZE, 8), (ks.KS_OPT_BLOCK_THREADS, 64)])):
+        b, r = _gpu(ks, M, L, A, p, seed, S, **kw)
+        assert_rows_equal(b, r, ids, eb, er, "packed4 %r" % (kw,))
+    for init in (0, L - 1, 5):
+        q = dict(p, init_price=init)
+        eb, er = oracle_rows(oracle, q, L, 333, seed, ids, 40)
+        b, r = _gpu(ks, M, L, 333, q, seed, 40)
+        assert_rows_equal(b, r, ids, eb, er, "packed4 init_price=%d" % init)
+    sim = ks.KsSim(2, L, 100, p, 0)
+    with pytest.raises(ks.KsError):
+        sim.ks_set_option(ks.KS_OPT_ATOMIC_MODE, 1)    # PACKED4 has plain atomics only
+    sim.ks_destroy()
+
+
+def test_packed4_full_size_c4_sampled_markets(ks, oracle):
+    """C4 under PACKED4 at full size in the launch configuration bench.py --rng packed4 times;
+    the oracle runs the 64 seeded sampled markets."""
+    c = CONFIGS["C4"]
+    p = packed4(c.params)
+    b, r = _gpu(ks, c.M, c.L, c.A, p, c.seed, c.S)
+    ids = sampled_markets(c.M, c.seed)
+    eb, er = oracle_rows(oracle, p, c.L, c.A, c.seed, ids, c.S)
+    assert_rows_equal(b, r, ids, eb, er, "C4 packed4")
 
 
 # ------------------------------------------------------------------ book injection / edge cases
