@@ -55,6 +55,14 @@ struct KernelParams {
   long long orders_per_step;                      // A + number of makers
 };
 
+// u32 x u32 -> u64 as ONE mul.wide.u32 (IMAD.WIDE.U32).  Written as PTX because the compiler,
+// given (uint64_t)a * b with a loop-invariant b, hoists the zero-extension of b and then emits a
+// 64 x 64 multiply whose (zero) cross term costs an extra add per product.
+__device__ __forceinline__ uint64_t mul_wide_u32(uint32_t a, uint32_t b) {
+  uint64_t r;
+  asm("mul.wide.u32 %0, %1, %2;" : "=l"(r) : "r"(a), "r"(b));
+  return r;
+}
 __device__ __forceinline__ uint32_t hi32(uint64_t x) { return (uint32_t)(x >> 32); }
 __device__ __forceinline__ uint32_t lo32(uint64_t x) { return (uint32_t)x; }
 
@@ -264,25 +272,33 @@ __device__ __forceinline__ void momentum_order(const KernelParams& P, const Book
 
 // ---- PACKED4 rules (A22): every draw of an agent out of ONE word by successive
 // multiply-extract: o = hi(w*n), x1 = lo(w*n); q-1 = hi(x1*qmax), x2 = lo(x1*qmax); coin = x2>>31.
-// Two IMAD.WIDE per agent (the +1 of q rides in the second one's 64-bit addend).
-// No-clamp noise path: m = coin mask (all-ones for a buy); sell tick = (last-delta) + o, buy tick
-// = (last-delta) + (n-1-o) = (last-delta+n) + ~o, so addr = base(m) + 4*(o ^ m) with
-// base = &ask[last-delta] or &bid[last-delta+n]: SHF + 2 LOP3 + LEA on the alu pipe.
+// Two IMAD.WIDE per agent.
+// No-clamp noise path: the first multiply is by 4n, so that its high word is the byte offset:
+// w*4n = (4o + r)*2^32 + (x1 << 2 mod 2^32), r = top two bits of x1; x1 itself is the funnel shift
+// (hi:lo) >> 2 (one SHF).  m = coin mask (all-ones for a buy); sell tick = (last-delta) + o, buy
+// tick = (last-delta) + (n-1-o) = (last-delta+n) + ~o, and (4o + r) ^ m = 4*(~o) + (3-r) for a
+// buy, so off = ((4o + r) ^ m) & ~3 (one LOP3) and addr = &ask[last-delta] + (m & (&bid[last-
+// delta+n] - &ask[last-delta])) + off: a three-operand IADD3.  Everything but the two multiplies
+// runs on the alu pipe.
 template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order_packed(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                                    uint32_t w, int& sink) {
-  const uint64_t p1 = (uint64_t)w * (uint32_t)P.noise_n;
-  const uint64_t p2 = (uint64_t)lo32(p1) * (uint32_t)P.noise_qmax + P.q_addend;
-  const int q = (int)hi32(p2);
-  const uint32_t o = hi32(p1);
   if (!CLAMP) {
+    const uint64_t p1 = mul_wide_u32(w, (uint32_t)P.noise_n4);
+    const uint32_t x1 = __funnelshift_r(lo32(p1), hi32(p1), 2);
+    const uint64_t p2 = mul_wide_u32(x1, (uint32_t)P.noise_qmax);
+    const int q = (int)hi32(p2) + 1;
     const uint32_t m = (uint32_t)((int32_t)lo32(p2) >> 31);
-    const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
-    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top));
-    book_add_at<ATOM>(book, base + ((o ^ m) << 2), q, sink);
+    const uint32_t off = (hi32(p1) ^ m) & ~3u;
+    const uint32_t side_off = m & (rc.bid_lo + (uint32_t)P.noise_n4 - rc.ask_lo);
+    book_add_at<ATOM>(book, rc.ask_lo + side_off + off, q, sink);
   } else {
+    const uint64_t p1 = mul_wide_u32(w, (uint32_t)P.noise_n);
+    const uint64_t p2 = mul_wide_u32(lo32(p1), (uint32_t)P.noise_qmax);
+    const int q = (int)hi32(p2) + 1;
+    const int o = (int)hi32(p1);
     const bool buy = (int32_t)lo32(p2) < 0;
-    const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - (int)o : (rc.last - P.noise_delta) + (int)o, rc.L);
+    const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - o : (rc.last - P.noise_delta) + o, rc.L);
     book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
   }
 }
@@ -290,9 +306,9 @@ __device__ __forceinline__ void noise_order_packed(const KernelParams& P, const 
 template <int ATOM>
 __device__ __forceinline__ void momentum_order_packed(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                                       uint32_t w, int& sink) {
-  const uint64_t p1 = (uint64_t)w * (uint32_t)P.mom_n;
-  const uint64_t p2 = (uint64_t)lo32(p1) * (uint32_t)P.mom_qmax + P.q_addend;
-  const int q = (int)hi32(p2);
+  const uint64_t p1 = mul_wide_u32(w, (uint32_t)P.mom_n);
+  const uint64_t p2 = mul_wide_u32(lo32(p1), (uint32_t)P.mom_qmax);
+  const int q = (int)hi32(p2) + 1;
   const int o = (int)hi32(p1);
   const bool buy = rc.dp > 0 ? true : (rc.dp < 0 ? false : ((int32_t)lo32(p2) < 0));
   const int tick = clamp_tick(buy ? rc.last + o : rc.last - o, rc.L);
