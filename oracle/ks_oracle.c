@@ -26,6 +26,9 @@
  *                      DESIGN.md (combined = resting + incoming).
  *   ko_derived         fp64 statistics derived from the integer sums (PAPER.md:302,
  *                      PAPER.md:442-456).
+ *   ko_run_markets_traced, ko_trace_stats   per-step (price, volume) trace and the return
+ *                      statistics of SIV-J (Fig.7): volatility, excess
+ *                      kurtosis, volume per step, ACF of r and |r| (reading A23).
  *
  * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors,
  * the paper's worked example Eq.11-18, brute-force Eq.1-2 on tiny books, greedy
@@ -39,6 +42,7 @@
 #include <stddef.h>
 #include <string.h>
 #include <stdlib.h>
+#include <math.h>
 
 #define KO_API __attribute__((visibility("default")))
 
@@ -255,8 +259,9 @@ KO_API void ko_init_record(int64_t rec[16], int32_t L, int32_t init_price) {
  *   -1 negative depth, -2 executed buy volume != executed sell volume != Vmax,
  *   -3 a per-side sum reached 2^31 (the library's int32 contract would overflow).
  * ---------------------------------------------------------------------------------------- */
-KO_API int32_t ko_run_market(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
-                             uint32_t m, int64_t S, int64_t* bid, int64_t* ask, int64_t rec[16]) {
+static int32_t ko_run_market_impl(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
+                                  uint32_t m, int64_t S, int64_t* bid, int64_t* ask, int64_t rec[16],
+                                  int32_t* trace) {
   for (int64_t s = 0; s < S; ++s) {
     int32_t last = (int32_t)rec[F_LAST], prev = (int32_t)rec[F_PREV];
     uint32_t t = (uint32_t)rec[F_STEPS];
@@ -305,26 +310,94 @@ KO_API int32_t ko_run_market(const ko_params* P, int32_t L, int32_t A, uint64_t 
     h = (h ^ x) * 0x100000001b3ull;
     rec[F_HASH] = (int64_t)h;
     rec[F_STEPS] += 1;
+    /* per-step trace: the price after the step and the executed volume */
+    if (trace) { trace[2 * s] = (int32_t)rec[F_LAST]; trace[2 * s + 1] = (int32_t)vmax; }
   }
   return 0;
 }
 
+KO_API int32_t ko_run_market(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
+                             uint32_t m, int64_t S, int64_t* bid, int64_t* ask, int64_t rec[16]) {
+  return ko_run_market_impl(P, L, A, seed, m, S, bid, ask, rec, NULL);
+}
+
 /* Run S steps of n markets (global ids in ids[]) from the int32 state (books[n][2][L], side 0
  * = bid, 1 = ask; recs[n][16]) and write the state back.  Single-threaded loop. */
-KO_API int32_t ko_run_markets(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
-                              const uint32_t* ids, int32_t n, int64_t S,
-                              int32_t* books, int64_t* recs) {
+static int32_t ko_run_markets_impl(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
+                                   const uint32_t* ids, int32_t n, int64_t S,
+                                   int32_t* books, int64_t* recs, int32_t* trace) {
   int64_t* bid = (int64_t*)malloc(sizeof(int64_t) * (size_t)L);
   int64_t* ask = (int64_t*)malloc(sizeof(int64_t) * (size_t)L);
   int32_t rc = 0;
   for (int32_t i = 0; i < n && rc == 0; ++i) {
     int32_t* b = books + (size_t)i * 2 * (size_t)L;
     for (int32_t p = 0; p < L; ++p) { bid[p] = b[p]; ask[p] = b[L + p]; }
-    rc = ko_run_market(P, L, A, seed, ids[i], S, bid, ask, recs + (size_t)i * 16);
+    rc = ko_run_market_impl(P, L, A, seed, ids[i], S, bid, ask, recs + (size_t)i * 16,
+                            trace ? trace + (size_t)i * 2 * (size_t)S : NULL);
     for (int32_t p = 0; p < L; ++p) { b[p] = (int32_t)bid[p]; b[L + p] = (int32_t)ask[p]; }
   }
   free(bid); free(ask);
   return rc;
+}
+
+KO_API int32_t ko_run_markets(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
+                              const uint32_t* ids, int32_t n, int64_t S,
+                              int32_t* books, int64_t* recs) {
+  return ko_run_markets_impl(P, L, A, seed, ids, n, S, books, recs, NULL);
+}
+
+/* The same, also recording trace[n][S][2] = (price after the step, executed volume Vmax) for the
+ * S steps of this call (the paper "records the price returns"). */
+KO_API int32_t ko_run_markets_traced(const ko_params* P, int32_t L, int32_t A, uint64_t seed,
+                                     const uint32_t* ids, int32_t n, int64_t S,
+                                     int32_t* books, int64_t* recs, int32_t* trace) {
+  return ko_run_markets_impl(P, L, A, seed, ids, n, S, books, recs, trace);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Return statistics of ONE market's trace[S][2] (SIV-J, Fig.7; DESIGN.md
+ * reading A23), plain two-pass definitions in fp64.  Returns r_t = p_t - p_{t-1} between
+ * consecutive traced steps, t = 1..S-1 (n = S-1 of them); x-bar = mean.
+ *   out[0] volatility   = sqrt(m2), m2 = sum (r - rbar)^2 / n            ("std dev", Fig.7)
+ *   out[1] excess kurt. = m4 / m2^2 - 3, m4 = sum (r - rbar)^4 / n       (NaN if m2 = 0)
+ *   out[2] volume/step  = sum_t Vmax_t / S                               (all S steps)
+ *   out[3] mean return  = rbar
+ *   out[4 + k-1]     ACF_r(k)   = sum_{t=k+1..n} (r_t - rbar)(r_{t-k} - rbar) / sum_t (r_t - rbar)^2
+ *   out[4 + K + k-1] ACF_|r|(k) = the same for x_t = |r_t|               k = 1..K (NaN if 0/0)
+ * n < 1 -> everything but out[2] is NaN.
+ * ---------------------------------------------------------------------------------------- */
+KO_API void ko_trace_stats(const int32_t* trace, int64_t S, int32_t K, double* out) {
+  double nan = 0.0; nan = nan / nan;
+  const int64_t n = S - 1;
+  double vsum = 0.0;
+  for (int64_t t = 0; t < S; ++t) vsum += (double)trace[2 * t + 1];
+  for (int32_t i = 0; i < 4 + 2 * K; ++i) out[i] = nan;
+  out[2] = S > 0 ? vsum / (double)S : nan;
+  if (n < 1) return;
+  double* r = (double*)malloc(sizeof(double) * (size_t)n);
+  double* a = (double*)malloc(sizeof(double) * (size_t)n);
+  double rbar = 0.0, abar = 0.0;
+  for (int64_t t = 0; t < n; ++t) {
+    r[t] = (double)((int64_t)trace[2 * (t + 1)] - (int64_t)trace[2 * t]);
+    a[t] = r[t] < 0 ? -r[t] : r[t];
+    rbar += r[t]; abar += a[t];
+  }
+  rbar /= (double)n; abar /= (double)n;
+  double m2 = 0.0, m4 = 0.0, a2 = 0.0;
+  for (int64_t t = 0; t < n; ++t) {
+    double d = r[t] - rbar, e = a[t] - abar;
+    m2 += d * d; m4 += d * d * d * d; a2 += e * e;
+  }
+  out[0] = sqrt(m2 / (double)n);
+  out[1] = m2 > 0 ? (m4 / (double)n) / ((m2 / (double)n) * (m2 / (double)n)) - 3.0 : nan;
+  out[3] = rbar;
+  for (int32_t k = 1; k <= K; ++k) {
+    double cr = 0.0, ca = 0.0;
+    for (int64_t t = k; t < n; ++t) { cr += (r[t] - rbar) * (r[t - k] - rbar); ca += (a[t] - abar) * (a[t - k] - abar); }
+    out[4 + k - 1] = m2 > 0 ? cr / m2 : nan;
+    out[4 + K + k - 1] = a2 > 0 ? ca / a2 : nan;
+  }
+  free(r); free(a);
 }
 
 /* fp64 statistics derived on the host from the integer record:

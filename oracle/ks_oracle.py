@@ -40,7 +40,7 @@ def build(force: bool = False) -> str:
         if force or stale:
             tmp = _LIB + ".tmp.%d" % os.getpid()
             subprocess.check_call(["gcc", "-O2", "-std=c99", "-Wall", "-Wextra", "-shared", "-fPIC",
-                                   "-fvisibility=hidden", "-o", tmp, _SRC])
+                                   "-fvisibility=hidden", "-o", tmp, _SRC, "-lm"])
             os.replace(tmp, _LIB)
     return _LIB
 
@@ -62,6 +62,11 @@ def lib():
         L.ko_run_markets.argtypes = [C.POINTER(KoParams), C.c_int32, C.c_int32, C.c_uint64, u32p,
                                      C.c_int32, C.c_int64, i32p, i64p]
         L.ko_run_markets.restype = C.c_int32
+        L.ko_run_markets_traced.argtypes = [C.POINTER(KoParams), C.c_int32, C.c_int32, C.c_uint64, u32p,
+                                            C.c_int32, C.c_int64, i32p, i64p, i32p]
+        L.ko_run_markets_traced.restype = C.c_int32
+        L.ko_trace_stats.argtypes = [i32p, C.c_int64, C.c_int32, C.POINTER(C.c_double)]
+        L.ko_trace_stats.restype = None
         L.ko_derived.argtypes = [i64p, C.POINTER(C.c_double)]
         L.ko_derived.restype = None
         _lib = L
@@ -135,6 +140,32 @@ def run_markets(params: dict, L: int, A: int, seed: int, ids, S: int, books=None
     if rc != 0:
         raise RuntimeError("oracle consistency assertion failed, code %d" % rc)
     return books, recs
+
+
+def run_markets_traced(params: dict, L: int, A: int, seed: int, ids, S: int, books=None, recs=None):
+    """run_markets that also returns trace int32 [n][S][2] = (price after the step, Vmax)."""
+    ids = np.ascontiguousarray(np.asarray(ids, dtype=np.uint32))
+    n = ids.shape[0]
+    if books is None:
+        books, recs = init_state(n, L, int(params["init_price"]))
+    else:
+        books = np.ascontiguousarray(books, dtype=np.int32).copy()
+        recs = np.ascontiguousarray(recs, dtype=np.int64).copy()
+    trace = np.zeros((n, S, 2), dtype=np.int32)
+    P = _params(params)
+    rc = lib().ko_run_markets_traced(C.byref(P), L, A, seed, _ptr(ids, C.c_uint32), n, S,
+                                     _ptr(books, C.c_int32), _ptr(recs, C.c_int64), _ptr(trace, C.c_int32))
+    if rc != 0:
+        raise RuntimeError("oracle consistency assertion failed, code %d" % rc)
+    return books, recs, trace
+
+
+def trace_stats(trace, K: int):
+    """trace int32 [S][2] of one market -> float64 [4 + 2K] (see ko_trace_stats)."""
+    t = np.ascontiguousarray(trace, dtype=np.int32)
+    out = np.zeros(4 + 2 * K, dtype=np.float64)
+    lib().ko_trace_stats(_ptr(t, C.c_int32), t.shape[0], K, _ptr(out, C.c_double))
+    return out
 
 
 def derived(rec):
