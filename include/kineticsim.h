@@ -144,6 +144,33 @@ KS_API ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, con
  */
 KS_API ks_status ks_run(ks_sim* s, int64_t S, void* stream);
 
+/*
+ * ks_run that also records the per-step trace of this call (the paper "records
+ * the price returns" of every market for its SIV-J sweep).
+ *   d_trace  DEVICE, caller-owned, 8-byte aligned: int32 [M][S][2]; entry [m][i] = (price after
+ *            step i of this call -- p* if the step traded, else the unchanged last price --,
+ *            executed volume Vmax, 0 if none).  Written in 256-byte coalesced chunks, 8*M*S bytes
+ *            in all; nothing else about the run changes (same bytes in d_state as ks_run).
+ * Errors as ks_run, plus KS_ERR_INVALID_ARG for a NULL or misaligned d_trace.
+ */
+KS_API ks_status ks_run_traced(ks_sim* s, int64_t S, int32_t* d_trace, void* stream);
+
+/*
+ * Return statistics of a trace (SIV-J, Fig.7; reading A23), one kernel,
+ * one warp per market.  d_trace: DEVICE int32 [M][S][2] as written by ks_run_traced.  d_out: DEVICE
+ * double [M][4 + 2K].  With r_t = p_t - p_{t-1} between consecutive traced steps (n = S-1 returns):
+ *   [0] volatility = population std of r       [1] excess kurtosis = m4/m2^2 - 3 (central moments)
+ *   [2] volume per step = sum Vmax / S         [3] mean return
+ *   [4 .. 4+K)    ACF_r(k),   k = 1..K:  sum_{t>k} (r_t - rbar)(r_{t-k} - rbar) / sum_t (r_t - rbar)^2
+ *   [4+K .. 4+2K) ACF_|r|(k), k = 1..K
+ * A quantity with a zero denominator is NaN.  Sums are exact integers (128-bit where needed); only
+ * the final quotients are rounded.  Range: every |r_t| <= 46340 (L <= 32768 guarantees it) and
+ * S^4 * max|r|^4 < 2^126.
+ * KS_ERR_INVALID_ARG for NULL pointers, M < 1, S < 1, K < 0 or K > 256.
+ */
+KS_API ks_status ks_trace_stats(const int32_t* d_trace, int32_t M, int64_t S, int32_t K, double* d_out,
+                                void* stream);
+
 /* Copy the books / the records out of d_state.  dst: HOST or DEVICE pointer (cudaMemcpyDefault),
  * int32 [M][2][L] resp. ks_market_stats [M]; a host destination must stay valid until the stream
  * work is done (pinned memory makes the copy asynchronous).  Alg.1 "Ensure". */

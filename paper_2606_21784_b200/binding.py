@@ -25,7 +25,7 @@ DERIVED_FIELDS = ("mean_px", "vwap", "vol_per_step", "ret_mean", "ret_var", "exc
 
 # every symbol the two headers declare (tests check the library exports exactly these)
 EXPORTS = ("ks_state_bytes", "ks_create", "ks_create_ex", "ks_run", "ks_read_books", "ks_read_stats",
-           "ks_write_books", "ks_set_option", "ks_derive_stats", "ks_destroy", "ks_last_error",
+           "ks_write_books", "ks_run_traced", "ks_trace_stats", "ks_set_option", "ks_derive_stats", "ks_destroy", "ks_last_error",
            "ks_launch_count", "ks_run_stepwise", "ks_bench_smem_atomic", "ks_bench_generate_only",
            "ks_bench_int_pipe")
 
@@ -59,6 +59,8 @@ def load():
     L.ks_create_ex.argtypes = [C.POINTER(vp), i32, i32, i32, pp, u64, u32, vp, vp]; L.ks_create_ex.restype = i32
     L.ks_run.argtypes = [vp, i64, vp]; L.ks_run.restype = i32
     L.ks_run_stepwise.argtypes = [vp, i64, vp]; L.ks_run_stepwise.restype = i32
+    L.ks_run_traced.argtypes = [vp, i64, vp, vp]; L.ks_run_traced.restype = i32
+    L.ks_trace_stats.argtypes = [vp, i32, i64, i32, vp, vp]; L.ks_trace_stats.restype = i32
     L.ks_read_books.argtypes = [vp, vp, vp]; L.ks_read_books.restype = i32
     L.ks_read_stats.argtypes = [vp, vp, vp]; L.ks_read_stats.restype = i32
     L.ks_write_books.argtypes = [vp, vp, vp]; L.ks_write_books.restype = i32
@@ -153,6 +155,11 @@ class KsSim:
     def ks_run_stepwise(self, S: int, stream=None):
         _check(load().ks_run_stepwise(self._h, S, _stream_ptr(stream)))
 
+    def ks_run_traced(self, S: int, d_trace, stream=None):
+        """d_trace: CUDA int32 tensor [M][S][2] (price after the step, Vmax)."""
+        assert d_trace.is_cuda and d_trace.numel() >= self.M * S * 2
+        _check(load().ks_run_traced(self._h, S, d_trace.data_ptr(), _stream_ptr(stream)))
+
     def ks_read_books(self, dst, stream=None):
         _check(load().ks_read_books(self._h, _ptr_of(dst), _stream_ptr(stream)))
 
@@ -190,6 +197,16 @@ class KsSim:
             self.ks_destroy()
         except Exception:
             pass
+
+
+def ks_trace_stats(d_trace, M: int, S: int, K: int, d_out=None, stream=None):
+    """d_trace: CUDA int32 [M][S][2]; returns (or fills) a CUDA float64 tensor [M][4 + 2K]."""
+    import torch
+    if d_out is None:
+        d_out = torch.empty((M, 4 + 2 * K), dtype=torch.float64, device=d_trace.device)
+    assert d_trace.is_cuda and d_out.is_cuda and d_out.numel() >= M * (4 + 2 * K)
+    _check(load().ks_trace_stats(d_trace.data_ptr(), M, S, K, d_out.data_ptr(), _stream_ptr(stream)))
+    return d_out
 
 
 def ks_bench_smem_atomic(mode, delta, L, threads=256, ctas_per_sm=8, iters=2000, warmup=2, reps=5, stream=None):

@@ -2,6 +2,7 @@
 #include "../../include/kineticsim.h"
 #include "../../include/kineticsim_bench.h"
 #include "ks_cluster.cuh"
+#include "ks_trace.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -251,7 +252,7 @@ static cudaError_t launch_cluster(const ks::KernelParams& P, int C, int T, cudaS
   return cudaLaunchKernelEx(&cfg, kern, P);
 }
 
-static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
+static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, int32_t* d_trace = nullptr) {
   if (!s) { set_err("%s: NULL handle", who); return KS_ERR_INVALID_ARG; }
   if (S < 0) { set_err("%s: S < 0", who); return KS_ERR_INVALID_ARG; }
   if (S == 0) return KS_OK;
@@ -288,6 +289,7 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
   }
   P.fresh = s->fresh;
   P.force_generic = s->opt_clear;
+  P.trace = reinterpret_cast<int2*>(d_trace);
   P.S = S;
   P.orders_per_step = (long long)s->A + s->n_maker;
 
@@ -325,6 +327,22 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who) {
 extern "C" {
 
 ks_status ks_run(ks_sim* s, int64_t S, void* stream) { return run_impl(s, S, stream, "ks_run"); }
+
+ks_status ks_run_traced(ks_sim* s, int64_t S, int32_t* d_trace, void* stream) {
+  if (!d_trace) { set_err("ks_run_traced: NULL trace buffer"); return KS_ERR_INVALID_ARG; }
+  if ((reinterpret_cast<uintptr_t>(d_trace) & 7) != 0) { set_err("ks_run_traced: d_trace must be 8-byte aligned"); return KS_ERR_INVALID_ARG; }
+  return run_impl(s, S, stream, "ks_run_traced", d_trace);
+}
+
+ks_status ks_trace_stats(const int32_t* d_trace, int32_t M, int64_t S, int32_t K, double* d_out, void* stream) {
+  if (!d_trace || !d_out || M < 1 || S < 1 || K < 0 || K > 256) { set_err("ks_trace_stats: bad argument"); return KS_ERR_INVALID_ARG; }
+  const int warps = 4;
+  ks::ks_trace_stats_kernel<<<(M + warps - 1) / warps, warps * 32, 0, (cudaStream_t)stream>>>(
+      reinterpret_cast<const int2*>(d_trace), M, (long long)S, K, d_out);
+  KS_CUDA(cudaGetLastError());
+  g_launches++;
+  return KS_OK;
+}
 
 // a8 ablation: the same kernel, one launch per step, book through HBM between launches.
 ks_status ks_run_stepwise(ks_sim* s, int64_t S, void* stream) {

@@ -57,11 +57,12 @@ struct ClusterBook {
 // grid = M*C CTAs in clusters of C = 1 << P.log2C (cluster <-> market), block = T threads,
 // dynamic shared memory = 8*Lc bytes.  MODEL: 0 = ZI, 1 = MIX3.
 template <int MODEL, bool PACKED>
-__global__ void ks_cluster_kernel(const __grid_constant__ KernelParams P) {
+__global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_constant__ KernelParams P) {
   extern __shared__ __align__(16) int32_t book[];     // [2][Lc]: this CTA's ticks, bid then ask
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
   __shared__ int s_red32[64];
+  __shared__ int2 s_trace[32];                        // staged trace entries (rank 0, only when P.trace)
   __shared__ int s_ctl[4];                            // [0] = price at the start of the step (written by rank 0)
   __shared__ long long s_ctot[8][2];                  // rank 0 only: per-rank (sum_bid, sum_ask)
   __shared__ int s_cext[8][2];                        // rank 0 only: per-rank (bmax, amin), global ticks
@@ -159,6 +160,8 @@ __global__ void ks_cluster_kernel(const __grid_constant__ KernelParams P) {
         update_record(s_rec, last, vmax, pstar, new_last);
         for (int r = 0; r < C; ++r) st_cluster_s32(mapa_shared(ctl_saddr, (uint32_t)r), new_last);
       }
+      if (P.trace) trace_step(s_trace, P.trace + (size_t)cluster_id * (size_t)P.S, s, P.S, lane,
+                              vmax > 0 ? pstar : last, vmax);
     }
     cluster_sync();                                    // B2: residual book and new price visible
     prev = last;

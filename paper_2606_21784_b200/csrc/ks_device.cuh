@@ -51,6 +51,7 @@ struct KernelParams {
   int32_t fresh;                                  // books are known to be all zero: skip the load
   int32_t force_generic;                          // ablation/test: always use the chunked scan
   int32_t log2C;                                  // cluster kernel only: CTAs per market = 1 << log2C
+  int2* trace;                                    // DEVICE [M][S] (price after the step, Vmax), or NULL
   long long S;                                    // steps to run
   long long orders_per_step;                      // A + number of makers
 };
@@ -167,6 +168,20 @@ __device__ __forceinline__ void philox_block_from_p0(const KernelParams& P, cons
   w[1] = lo32(a1);
   w[2] = hi32(a0) ^ c3 ^ P.k1[9];
   w[3] = lo32(a0);
+}
+
+// Per-step trace: lane 0 of the clearing warp stages (price, Vmax) of step s in
+// shared memory; every 32 steps (and after the last one) the warp flushes the staged entries with
+// one coalesced 256-byte store.  gtrace points at this market's S entries.
+__device__ __forceinline__ void trace_step(int2* s_trace, int2* gtrace, long long s, long long S, int lane,
+                                           int price, int vmax) {
+  const int slot = (int)(s & 31);
+  if (lane == 0) s_trace[slot] = make_int2(price, vmax);
+  __syncwarp();
+  if (slot == 31 || s == S - 1) {
+    if (lane <= slot) gtrace[s - slot + lane] = s_trace[lane];
+    __syncwarp();
+  }
 }
 
 // a2: add one order to the shared-memory book at byte offset `off` from the start of the [2][L]

@@ -64,11 +64,12 @@ __device__ __forceinline__ void update_record(long long* rec, int last, int vmax
 // PACKED: the PACKED4 draw contract (one Philox block per four agents, A22).
 // ---------------------------------------------------------------------------------------------
 template <int MODEL, int ATOM, bool PACKED>
-__global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
+__global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
   __shared__ int s_red32[64];
+  __shared__ int2 s_trace[32];                        // staged trace entries (only when P.trace)
   __shared__ __align__(16) int s_ctl[4];              // per-step broadcast: last, &bid[last-delta], &ask[last-delta], noclamp
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
@@ -150,6 +151,8 @@ __global__ void ks_persistent_kernel(const __grid_constant__ KernelParams P) {
         update_record(s_rec, last, vmax, pstar, new_last);
         publish(new_last);
       }
+      if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)P.S, s, P.S, lane,
+                              vmax > 0 ? pstar : last, vmax);
     }
     __syncthreads();                                   // B2: residual book and new price visible
     prev = last;

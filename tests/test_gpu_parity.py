@@ -220,6 +220,83 @@ def test_packed4_full_size_c4_sampled_markets(ks, oracle):
     assert_rows_equal(b, r, ids, eb, er, "C4 packed4")
 
 
+# ------------------------------------------------------------------ per-step trace + SIV-J statistics
+def _gpu_traced(ks, M, L, A, params, seed, runs, K, opts=()):
+    import torch
+    sim = ks.KsSim(M, L, A, params, seed)
+    for o, v in opts:
+        sim.ks_set_option(o, v)
+    traces = []
+    for S in runs:
+        tr = torch.full((M, S, 2), -7, dtype=torch.int32, device="cuda")
+        sim.ks_run_traced(S, tr)
+        traces.append(tr)
+    full = torch.cat(traces, dim=1).contiguous()
+    st = ks.ks_trace_stats(full, M, full.shape[1], K)
+    torch.cuda.synchronize()
+    b, r = sim.books_to_host(), sim.stats_to_host()
+    sim.ks_destroy()
+    return b, r, full.cpu().numpy(), st.cpu().numpy()
+
+
+def _assert_stats_close(got, exp, what):
+    """The GPU forms every statistic as the quotient of two exact integers; the oracle evaluates
+    the plain two-pass fp64 definitions.  1e-12 relative (north_star); for the autocorrelations,
+    which are normalised to [-1, 1] and may be arbitrarily close to 0, 1e-12 absolute."""
+    assert np.array_equal(np.isnan(got), np.isnan(exp)), what
+    m = ~np.isnan(exp)
+    tol = 1e-12 * np.maximum(np.abs(exp[m]), 1.0)
+    assert np.all(np.abs(got[m] - exp[m]) <= tol), "%s: max err %g" % (what, np.max(np.abs(got[m] - exp[m])))
+
+
+@pytest.mark.parametrize("case", ["zi", "mix3", "packed4", "cluster"])
+def test_trace_and_return_statistics(ks, oracle, case):
+    """the (price, Vmax) trace is bit-exact against the oracle's, tracing
+    leaves the state bytes unchanged, traces of split runs concatenate, ragged step counts (not a
+    multiple of the 32-entry staging buffer) flush completely, and the SIV-J statistics agree."""
+    K = 20
+    opts = ()
+    if case == "zi":
+        M, L, A, seed, p, runs = 37, 256, 700, 9, zi_params(16, 100), [45, 1, 32, 83]
+    elif case == "mix3":
+        M, L, A, seed, p, runs = 21, 1024, 900, 4, mix3_params(), [150]
+    elif case == "packed4":
+        M, L, A, seed, p, runs = 19, 512, 1001, 6, packed4(mix3_params()), [64, 37]
+    else:
+        M, L, A, seed, p, runs = 9, 512, 600, 8, zi_params(32, 50), [70]
+        opts = [(ks.KS_OPT_CLUSTER_SIZE, 4)]
+    S = sum(runs)
+    ids = np.arange(M)
+    eb, er, et = oracle.run_markets_traced(p, L, A, seed, ids, S)
+    b, r, tr, st = _gpu_traced(ks, M, L, A, p, seed, runs, K, opts)
+    assert_rows_equal(b, r, ids, eb, er, "traced " + case)
+    assert np.array_equal(tr, et), "trace differs from the oracle"
+    exp = np.stack([oracle.trace_stats(et[i], K) for i in range(M)])
+    _assert_stats_close(st, exp, "trace stats " + case)
+
+
+def test_trace_stats_degenerate_series(ks, oracle):
+    """Hand-made traces through ks_trace_stats alone: constant price (zero variance -> NaN),
+    alternating +-1 returns (ACF (-1)^k (n-k)/n), one traced step (no returns), large moves near
+    the int64 guard."""
+    import torch
+    K, S = 6, 101
+    p = np.zeros((5, S, 2), dtype=np.int32)
+    p[0, :, 0] = 77; p[0, :, 1] = 3
+    p[1, :, 0] = 100 + (np.arange(S) % 2)
+    p[2, :, 0] = np.arange(S) * 5
+    p[3, :, 0] = np.where(np.arange(S) % 7 < 3, 32767, 0); p[3, :, 1] = 2 ** 31 - 1
+    rng = np.random.default_rng(3)
+    p[4, :, 0] = 500 + np.cumsum(rng.integers(-20, 21, size=S)); p[4, :, 1] = rng.integers(0, 1000, size=S)
+    d = torch.from_numpy(p).cuda()
+    got = ks.ks_trace_stats(d, 5, S, K).cpu().numpy()
+    exp = np.stack([oracle.trace_stats(p[i], K) for i in range(5)])
+    _assert_stats_close(got, exp, "degenerate")
+    assert got[1, 0] == 1.0 and got[1, 1] == -2.0 and got[1, 4] == -(100 - 1) / 100
+    one = ks.ks_trace_stats(d[:, :1, :].contiguous(), 5, 1, K).cpu().numpy()
+    assert np.array_equal(one[:, 2], p[:, 0, 1].astype(np.float64)) and np.isnan(np.delete(one, 2, axis=1)).all()
+
+
 # ------------------------------------------------------------------ book injection / edge cases
 def test_paper_worked_example_through_the_library(ks):
     """PAPER.md:315-354 (Eq.11-18) embedded at ticks 10..14 of an L=32 grid, A = 0: zero padding
