@@ -59,6 +59,10 @@ typedef struct {
   int32_t mom_delta;        /* momentum offset uniform in [0, delta]                         */
   int32_t mom_qmax;         /* momentum quantity uniform in 1..qmax                          */
   int32_t init_price;       /* < 0 -> L/2                                                    */
+  /* model 4 only (the paper's own agent model, ko_gen_orders_paper) */
+  int32_t paper_n_mom;      /* number of momentum agents                                     */
+  int32_t paper_n_maker;    /* number of market makers                                       */
+  int32_t paper_pmkt_q16;   /* P_mkt = paper_pmkt_q16 / 65536                                */
 } ko_params;
 
 /* record field indices (SURVEY.md Appendix A "Stats record") */
@@ -165,6 +169,65 @@ static int32_t ko_gen_orders_packed4(const ko_params* P, int32_t L, int32_t last
   return 1;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Model 4: the paper's own agent model (SIII-C; DESIGN.md
+ * reading A24), in doubled-integer arithmetic so that no half-tick is ever rounded in floating
+ * point.  State retrieval (Eq.3): bb = highest tick with resting bid depth, ba =
+ * lowest tick with resting ask depth, at the start of the step;
+ *     mid2 = 2*mid = bb + ba if both sides rest, else 2*last.
+ * round(x) is round-half-up: round(m2/2) = floor((m2 + 1) / 2).  Classes by contiguous index
+ * ranges (the paper gives class FRACTIONS): agents [0, A - n_mom - n_maker) noise,
+ * then n_mom momentum, then n_maker makers.  Words of Philox(ctr = (a, t, m, 0)):
+ *   w0>>31 coin; w1 -> eta; w2 -> quantity; w3>>16 < pmkt_q16 -> marketable.
+ *   noise    buy = coin; eta = mulhi(w1, 2D+1) - D; p = round(mid + eta); q = 1 + mulhi(w2, qmax);
+ *            marketable: p = L-1 for a buy, 0 for a sell
+ *   momentum ret = sgn(mid2 - mid2_prev) (mid2_prev = doubled mid at the start of the previous
+ *            step; 2*init before the first); buy = ret>0 ? 1 : ret<0 ? 0 : coin;
+ *            p = round(mid + 1) for a buy, round(mid - 1) for a sell; q = 1 + mulhi(w2, mom_qmax);
+ *            marketable like noise
+ *   maker    buys if (a + t) mod 2 == 0 else sells; p = round(mid - h) for a bid, round(mid + h)
+ *            for an ask, h = maker_spread_max ticks; q = 1 + mulhi(w2, maker_qty); never
+ *            marketable
+ * p is clamped to the grid (A15).  One order per agent.
+ * ---------------------------------------------------------------------------------------- */
+static int32_t ko_round_half_up(int64_t m2) {            /* floor((m2 + 1) / 2) for any sign */
+  int64_t x = m2 + 1;
+  return (int32_t)(x >= 0 ? x / 2 : -((-x + 1) / 2));
+}
+
+KO_API int32_t ko_gen_orders_paper(const ko_params* P, int32_t L, int32_t mid2, int32_t mid2_prev,
+                                   uint64_t seed, uint32_t m, uint32_t t, uint32_t a, int32_t A,
+                                   int32_t* side, int32_t* tick, int32_t* qty) {
+  uint32_t ctr[4] = { a, t, m, 0u };
+  uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+  uint32_t w[4];
+  ko_philox4x32_10(ctr, key, w);
+  const int32_t n_noise = A - P->paper_n_mom - P->paper_n_maker;
+  const int coin = (int)(w[0] >> 31);
+  const int mkt = (int32_t)(w[3] >> 16) < P->paper_pmkt_q16;
+  int buy; int64_t p2; int32_t q; int can_mkt = 1;
+  if ((int32_t)a < n_noise) {
+    int64_t eta = (int64_t)ko_mulhi(w[1], (uint32_t)(2 * P->noise_delta + 1)) - (int64_t)P->noise_delta;
+    buy = coin;
+    p2 = (int64_t)mid2 + 2 * eta;
+    q = 1 + (int32_t)ko_mulhi(w[2], (uint32_t)P->noise_qmax);
+  } else if ((int32_t)a < n_noise + P->paper_n_mom) {
+    int64_t d = (int64_t)mid2 - (int64_t)mid2_prev;
+    buy = d > 0 ? 1 : (d < 0 ? 0 : coin);
+    p2 = (int64_t)mid2 + (buy ? 2 : -2);
+    q = 1 + (int32_t)ko_mulhi(w[2], (uint32_t)P->mom_qmax);
+  } else {
+    buy = ((a + t) & 1u) == 0u;
+    p2 = (int64_t)mid2 + (buy ? -2 : 2) * (int64_t)P->maker_spread_max;
+    q = 1 + (int32_t)ko_mulhi(w[2], (uint32_t)P->maker_qty);
+    can_mkt = 0;
+  }
+  int32_t p = ko_clamp((int64_t)ko_round_half_up(p2), L);
+  if (can_mkt && mkt) p = buy ? L - 1 : 0;
+  *side = buy ? 0 : 1; *tick = p; *qty = q;
+  return 1;
+}
+
 KO_API int32_t ko_gen_orders(const ko_params* P, int32_t L, int32_t last, int32_t prev,
                              uint64_t seed, uint32_t m, uint32_t t, uint32_t a,
                              int32_t side[2], int32_t tick[2], int32_t qty[2]) {
@@ -251,6 +314,12 @@ KO_API void ko_init_record(int64_t rec[16], int32_t L, int32_t init_price) {
   rec[F_HASH] = (int64_t)0xcbf29ce484222325ull;
 }
 
+/* model 4: f[13] starts as the doubled opening price (the "previous mid") */
+KO_API void ko_init_record_paper(int64_t rec[16], int32_t L, int32_t init_price) {
+  ko_init_record(rec, L, init_price);
+  rec[F_PREV] = 2 * rec[F_LAST];
+}
+
 /* ------------------------------------------------------------------------------------------
  * Run S steps of ONE market with global id m, continuing from (bid, ask, rec).
  * bid/ask are int64[L] (the oracle's book is 64-bit; ko_run_markets narrows it and checks).
@@ -265,10 +334,21 @@ static int32_t ko_run_market_impl(const ko_params* P, int32_t L, int32_t A, uint
   for (int64_t s = 0; s < S; ++s) {
     int32_t last = (int32_t)rec[F_LAST], prev = (int32_t)rec[F_PREV];
     uint32_t t = (uint32_t)rec[F_STEPS];
+    /* model 4: state retrieval (Eq.3) on the resting book; rec[F_PREV] holds the
+     * doubled mid of the previous step instead of the previous price */
+    int32_t mid2 = 2 * last;
+    if (P->model == 4) {
+      int32_t bb = -1, ba = L;
+      for (int32_t p = 0; p < L; ++p) { if (bid[p] > 0) bb = p; }
+      for (int32_t p = L - 1; p >= 0; --p) { if (ask[p] > 0) ba = p; }
+      if (bb >= 0 && ba < L) mid2 = bb + ba;
+    }
     /* 1. orders: every agent sees (last, prev) as they were at the start of the step */
     for (int32_t a = 0; a < A; ++a) {
       int32_t side[2], tick[2], qty[2];
-      int32_t n = ko_gen_orders(P, L, last, prev, seed, m, t, (uint32_t)a, side, tick, qty);
+      int32_t n = P->model == 4
+                      ? ko_gen_orders_paper(P, L, mid2, prev, seed, m, t, (uint32_t)a, A, side, tick, qty)
+                      : ko_gen_orders(P, L, last, prev, seed, m, t, (uint32_t)a, side, tick, qty);
       for (int32_t i = 0; i < n; ++i) {
         if (side[i] == 0) { bid[tick[i]] += qty[i]; rec[F_SUBBUY] += qty[i]; }
         else              { ask[tick[i]] += qty[i]; rec[F_SUBSELL] += qty[i]; }
@@ -288,7 +368,7 @@ static int32_t ko_run_market_impl(const ko_params* P, int32_t L, int32_t A, uint
     if (before_b - after_b != vmax || before_a - after_a != vmax) return -2;
     /* 5. state and statistics */
     int64_t before = rec[F_LAST];
-    rec[F_PREV] = rec[F_LAST];
+    rec[F_PREV] = P->model == 4 ? (int64_t)mid2 : rec[F_LAST];
     uint64_t x;
     if (vmax > 0) {
       rec[F_LAST] = pstar;

@@ -20,7 +20,7 @@ _lock = threading.Lock()
 _lib = None
 
 PARAM_FIELDS = ("model", "noise_delta", "noise_qmax", "maker_spread_max", "maker_qty",
-                "mom_delta", "mom_qmax", "init_price")
+                "mom_delta", "mom_qmax", "init_price", "paper_n_mom", "paper_n_maker", "paper_pmkt_q16")
 
 # record field names, in order
 REC_FIELDS = ("steps", "n_trades", "sum_vol", "sum_px", "sum_px2", "sum_pxvol", "sum_ret",
@@ -59,6 +59,11 @@ def lib():
         L.ko_clear_step.restype = None
         L.ko_init_record.argtypes = [i64p, C.c_int32, C.c_int32]
         L.ko_init_record.restype = None
+        L.ko_init_record_paper.argtypes = [i64p, C.c_int32, C.c_int32]
+        L.ko_init_record_paper.restype = None
+        L.ko_gen_orders_paper.argtypes = [C.POINTER(KoParams), C.c_int32, C.c_int32, C.c_int32, C.c_uint64,
+                                          C.c_uint32, C.c_uint32, C.c_uint32, C.c_int32, i32p, i32p, i32p]
+        L.ko_gen_orders_paper.restype = C.c_int32
         L.ko_run_markets.argtypes = [C.POINTER(KoParams), C.c_int32, C.c_int32, C.c_uint64, u32p,
                                      C.c_int32, C.c_int64, i32p, i64p]
         L.ko_run_markets.restype = C.c_int32
@@ -74,7 +79,7 @@ def lib():
 
 
 def _params(p: dict) -> KoParams:
-    return KoParams(*[int(p[n]) for n in PARAM_FIELDS])
+    return KoParams(*[int(p.get(n, 0)) for n in PARAM_FIELDS])
 
 
 def _ptr(a, ct):
@@ -111,13 +116,23 @@ def clear_step(bid, ask):
     return dict(D=D, S=S, V=V, pstar=int(ps.value), vmax=int(vm.value), new_bid=b, new_ask=a)
 
 
-def init_state(n: int, L: int, init_price: int = -1):
-    """Fresh state for n markets: (books int32 [n][2][L] = 0, recs int64 [n][16])."""
+def init_state(n: int, L: int, init_price: int = -1, model: int = 0):
+    """Fresh state for n markets: (books int32 [n][2][L] = 0, recs int64 [n][16]).  Model 4 keeps
+    the doubled previous mid in f[13]."""
     books = np.zeros((n, 2, L), dtype=np.int32)
     recs = np.zeros((n, 16), dtype=np.int64)
     for i in range(n):
-        lib().ko_init_record(_ptr(recs[i], C.c_int64), L, init_price)
+        (lib().ko_init_record_paper if model == 4 else lib().ko_init_record)(_ptr(recs[i], C.c_int64), L, init_price)
     return books, recs
+
+
+def gen_orders_paper(params: dict, L: int, mid2: int, mid2_prev: int, seed: int, m: int, t: int, a: int, A: int):
+    """Model 4 -> (side, tick, qty)."""
+    side = C.c_int32(0); tick = C.c_int32(0); qty = C.c_int32(0)
+    P = _params(params)
+    lib().ko_gen_orders_paper(C.byref(P), L, mid2, mid2_prev, seed, m, t, a, A,
+                              C.byref(side), C.byref(tick), C.byref(qty))
+    return int(side.value), int(tick.value), int(qty.value)
 
 
 def run_markets(params: dict, L: int, A: int, seed: int, ids, S: int, books=None, recs=None):
@@ -129,7 +144,7 @@ def run_markets(params: dict, L: int, A: int, seed: int, ids, S: int, books=None
     ids = np.ascontiguousarray(np.asarray(ids, dtype=np.uint32))
     n = ids.shape[0]
     if books is None:
-        books, recs = init_state(n, L, int(params["init_price"]))
+        books, recs = init_state(n, L, int(params["init_price"]), int(params["model"]))
     else:
         books = np.ascontiguousarray(books, dtype=np.int32).copy()
         recs = np.ascontiguousarray(recs, dtype=np.int64).copy()
@@ -147,7 +162,7 @@ def run_markets_traced(params: dict, L: int, A: int, seed: int, ids, S: int, boo
     ids = np.ascontiguousarray(np.asarray(ids, dtype=np.uint32))
     n = ids.shape[0]
     if books is None:
-        books, recs = init_state(n, L, int(params["init_price"]))
+        books, recs = init_state(n, L, int(params["init_price"]), int(params["model"]))
     else:
         books = np.ascontiguousarray(books, dtype=np.int32).copy()
         recs = np.ascontiguousarray(recs, dtype=np.int64).copy()

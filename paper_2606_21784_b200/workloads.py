@@ -26,6 +26,22 @@ def packed4(params: dict) -> dict:
     return q
 
 
+KS_MODEL_PAPER = 4           # the paper's own agent model (A24)
+
+
+def paper_params(A: int, alpha_mom: float, alpha_maker: float = 0.15, delta: int = 8, qmax: int = 10,
+                 half_spread: int = 2, p_mkt: float = 0.05, init_price: int = -1) -> dict:
+    """The paper's agent mix: class FRACTIONS turned into contiguous index
+    ranges -- noise first, then round(alpha_mom*A) momentum agents, then round(alpha_maker*A)
+    makers; mid-price reference, marketable orders with probability p_mkt.  The numeric values of
+    delta / qmax / half_spread / p_mkt are not given in the paper: these defaults are ours."""
+    n_mom, n_maker = int(round(alpha_mom * A)), int(round(alpha_maker * A))
+    assert n_mom + n_maker <= A
+    return dict(model=KS_MODEL_PAPER, noise_delta=delta, noise_qmax=qmax, maker_spread_max=half_spread,
+                maker_qty=qmax, mom_delta=0, mom_qmax=qmax, init_price=init_price,
+                paper_n_mom=n_mom, paper_n_maker=n_maker, paper_pmkt_q16=int(round(p_mkt * 65536)))
+
+
 def zi_params(delta: int, qmax: int, init_price: int = -1) -> dict:
     """Zero-intelligence configs (BASELINE.json configs[0..3])."""
     return dict(model=KS_MODEL_ZI, noise_delta=delta, noise_qmax=qmax, maker_spread_max=1,
