@@ -64,7 +64,24 @@ typedef enum {
    * x1 = lo32(w*n); q = 1 + mulhi(x1, qmax), x2 = lo32(x1*qmax); coin = x2 >> 31 (maker:
    * s = 1 + mulhi(w, spread_max)).  Plain atomics only (KS_OPT_ATOMIC_MODE 0). */
   KS_MODEL_ZI_PACKED4 = 2,
-  KS_MODEL_MIX3_PACKED4 = 3
+  KS_MODEL_MIX3_PACKED4 = 3,
+  /* The paper's own agent model (SIII-C; reading A24),
+   * a separately named model beside the BASELINE.json ones.  Reference price: the mid of the RESTING
+   * book at the start of the step in doubled-integer form, mid2 = bb + ba (highest bid tick + lowest
+   * ask tick), or 2*last when a side is empty (Eq.3); round(m2/2) = floor((m2+1)/2).
+   * Classes are contiguous index ranges: agents [0, A - paper_n_mom - paper_n_maker) noise, then
+   * paper_n_mom momentum, then paper_n_maker makers.  Words of Philox(ctr = (a, step, market, 0)):
+   *   noise     buy = w0>>31; eta = mulhi(w1, 2*noise_delta+1) - noise_delta; p = round(mid + eta);
+   *             q = 1 + mulhi(w2, noise_qmax)
+   *   momentum  buy = sgn(mid2 - previous mid2) > 0, < 0 -> sell, = 0 -> w0>>31; p = round(mid +/- 1);
+   *             q = 1 + mulhi(w2, mom_qmax)
+   *   maker     buys iff (a + step) is even; p = round(mid - h) for a bid, round(mid + h) for an ask,
+   *             h = maker_spread_max; q = 1 + mulhi(w2, maker_qty); never marketable
+   *   noise and momentum orders are marketable iff (w3 >> 16) < paper_pmkt_q16: p = L-1 for a buy,
+   *   0 for a sell.  p is clamped to the grid.  Record field f[13] holds mid2 of the last executed
+   *   step (2*init before the first) instead of the previous price.
+   * L <= 16384 (no cluster path), plain atomics only. */
+  KS_MODEL_PAPER = 4
 } ks_model;
 
 /*
@@ -89,6 +106,10 @@ typedef struct {
   int32_t mom_delta;        /* momentum offset uniform in [0, mom_delta]            */
   int32_t mom_qmax;         /* momentum quantity uniform in 1..mom_qmax             */
   int32_t init_price;       /* opening last = prev; < 0 means L/2                   */
+  /* KS_MODEL_PAPER only (ignored otherwise; set to 0) */
+  int32_t paper_n_mom;      /* number of momentum agents                            */
+  int32_t paper_n_maker;    /* number of market makers                              */
+  int32_t paper_pmkt_q16;   /* P_mkt = paper_pmkt_q16 / 65536, 0..65536             */
 } ks_agent_params;
 
 /*

@@ -18,7 +18,7 @@ KS_OK, KS_ERR_INVALID_ARG, KS_ERR_UNSUPPORTED, KS_ERR_OVERFLOW, KS_ERR_CUDA, KS_
 KS_OPT_BLOCK_THREADS, KS_OPT_ATOMIC_MODE, KS_OPT_CLEAR_PATH, KS_OPT_CLUSTER_SIZE = 0, 1, 2, 3
 
 PARAM_FIELDS = ("model", "noise_delta", "noise_qmax", "maker_spread_max", "maker_qty", "mom_delta",
-                "mom_qmax", "init_price")
+                "mom_qmax", "init_price", "paper_n_mom", "paper_n_maker", "paper_pmkt_q16")
 REC_FIELDS = ("steps", "n_trades", "sum_vol", "sum_px", "sum_px2", "sum_pxvol", "sum_ret", "sum_ret2",
               "sum_ret3", "sum_ret4", "sub_buy", "sub_sell", "last", "prev", "traj_hash", "n_orders")
 DERIVED_FIELDS = ("mean_px", "vwap", "vol_per_step", "ret_mean", "ret_var", "excess_kurtosis")
@@ -86,7 +86,7 @@ def _check(status: int):
 
 
 def _params(p: dict) -> KsAgentParams:
-    return KsAgentParams(*[int(p[n]) for n in PARAM_FIELDS])
+    return KsAgentParams(*[int(p.get(n, 0)) for n in PARAM_FIELDS])
 
 
 def _stream_ptr(stream) -> int:

@@ -90,11 +90,18 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   if (M < 1 || A < 0 || !is_pow2(L) || L < 32) { set_err("ks_create: need M >= 1, A >= 0, L a power of two >= 32"); return KS_ERR_INVALID_ARG; }
   if (L > kMaxL) { set_err("ks_create: L > 32768 is not supported (p* must fit 16 bits of the trajectory hash)"); return KS_ERR_UNSUPPORTED; }
   if ((reinterpret_cast<uintptr_t>(d_state) & 15) != 0) { set_err("ks_create: d_state must be 16-byte aligned"); return KS_ERR_INVALID_ARG; }
-  if (p->model < KS_MODEL_ZI || p->model > KS_MODEL_MIX3_PACKED4) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
+  if (p->model < KS_MODEL_ZI || p->model > KS_MODEL_PAPER) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
   if (p->noise_delta < 0 || p->noise_delta >= L || p->noise_qmax < 1 || p->noise_qmax > kMaxQty || p->init_price >= L) {
     set_err("ks_create: bad noise parameters or init_price"); return KS_ERR_INVALID_ARG;
   }
-  if ((p->model & 1) == KS_MODEL_MIX3 &&
+  if (p->model == KS_MODEL_PAPER) {
+    if (p->maker_spread_max < 0 || p->maker_spread_max >= L || p->maker_qty < 1 || p->maker_qty > kMaxQty ||
+        p->mom_qmax < 1 || p->mom_qmax > kMaxQty || p->paper_n_mom < 0 || p->paper_n_maker < 0 ||
+        (int64_t)p->paper_n_mom + p->paper_n_maker > A || p->paper_pmkt_q16 < 0 || p->paper_pmkt_q16 > 65536) {
+      set_err("ks_create: bad parameters of the paper agent model"); return KS_ERR_INVALID_ARG;
+    }
+    if (L > kMaxLPerCta) { set_err("ks_create: the paper agent model has no cluster path (L <= 16384)"); return KS_ERR_UNSUPPORTED; }
+  } else if ((p->model & 1) == KS_MODEL_MIX3 &&
       (p->maker_spread_max < 1 || p->maker_spread_max > L || p->maker_qty < 1 || p->maker_qty > kMaxQty ||
        p->mom_delta < 0 || p->mom_delta >= L || p->mom_qmax < 1 || p->mom_qmax > kMaxQty)) {
     set_err("ks_create: bad maker/momentum parameters"); return KS_ERR_INVALID_ARG;
@@ -117,7 +124,11 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0;
   s->dev_smem_optin = optin; s->num_sms = sms;
   s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
-  if ((p->model & 1) == KS_MODEL_ZI) {
+  if (p->model == KS_MODEL_PAPER) {
+    s->n_mom = p->paper_n_mom; s->n_maker = 0; s->n_noise = A - p->paper_n_mom - p->paper_n_maker;
+    s->inflow_per_step = (int64_t)s->n_noise * p->noise_qmax + (int64_t)p->paper_n_mom * p->mom_qmax +
+                         (int64_t)p->paper_n_maker * p->maker_qty;
+  } else if ((p->model & 1) == KS_MODEL_ZI) {
     s->n_noise = A; s->n_maker = 0; s->n_mom = 0;
     s->inflow_per_step = (int64_t)A * p->noise_qmax;
   } else {
@@ -142,7 +153,8 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   if (blocks > sms * 16) blocks = sms * 16;
   if (blocks < 1) blocks = 1;
   ks::ks_init_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<int4*>(books_ptr(s)), nvec, recs_ptr(s), M,
-                                                              s->p.init_price);
+                                                              s->p.init_price,
+                                                              p->model == KS_MODEL_PAPER ? 2 * s->p.init_price : s->p.init_price);
   e = cudaGetLastError();
   if (e != cudaSuccess) {
     set_err("ks_create: init launch failed: %s", cudaGetErrorString(e));
@@ -170,14 +182,14 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_ATOMIC_MODE:
       if (value != 0 && value != 1) break;
       if (value == 1 && (s->opt_cluster > 1 || s->L > kMaxLPerCta)) break;   // the cluster kernel has plain atomics only
-      if (value == 1 && s->p.model >= KS_MODEL_ZI_PACKED4) break;            // so has the PACKED4 path
+      if (value == 1 && s->p.model >= KS_MODEL_ZI_PACKED4) break;            // so have PACKED4 and the paper model
       s->opt_atomic = value; return KS_OK;
     case KS_OPT_CLEAR_PATH:
       if (value != 0 && value != 1) break;
       s->opt_clear = value; return KS_OK;
     case KS_OPT_CLUSTER_SIZE:
       if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break;
-      if (value > 1 && (s->L / value < 32 || s->opt_atomic)) break;
+      if (value > 1 && (s->L / value < 32 || s->opt_atomic || s->p.model == KS_MODEL_PAPER)) break;
       if (value == 1 && s->L > kMaxLPerCta) break;
       s->opt_cluster = value; return KS_OK;
     default: break;
@@ -283,7 +295,12 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
   P.maker_spread_max = s->p.maker_spread_max; P.maker_qty = s->p.maker_qty;
   P.mom_n = s->p.mom_delta + 1; P.mom_qmax = s->p.mom_qmax;
   P.dmax = s->p.noise_delta;
-  if ((s->p.model & 1) == KS_MODEL_MIX3) {
+  if (s->p.model == KS_MODEL_PAPER) {
+    if (s->p.maker_spread_max > P.dmax) P.dmax = s->p.maker_spread_max;
+    if (P.dmax < 1) P.dmax = 1;
+    P.dmax += 1;                                       // round-half-up can add one tick
+    P.paper_n_noise = s->n_noise; P.paper_n_mom = s->p.paper_n_mom; P.paper_pmkt_q16 = s->p.paper_pmkt_q16;
+  } else if ((s->p.model & 1) == KS_MODEL_MIX3) {
     if (s->p.maker_spread_max > P.dmax) P.dmax = s->p.maker_spread_max;
     if (s->p.mom_delta > P.dmax) P.dmax = s->p.mom_delta;
   }
@@ -295,9 +312,12 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
 
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
-  const bool mix = (s->p.model & 1) == KS_MODEL_MIX3, packed = s->p.model >= KS_MODEL_ZI_PACKED4;
+  const bool paper = s->p.model == KS_MODEL_PAPER;
+  const bool mix = !paper && (s->p.model & 1) == KS_MODEL_MIX3;
+  const bool packed = !paper && s->p.model >= KS_MODEL_ZI_PACKED4;
   int C = s->opt_cluster;
   if (C == 0) C = s->L > kMaxLPerCta ? s->L / kMaxLPerCta : 1;
+  if (C > 1 && paper) { set_err("%s: the paper agent model has no cluster path", who); return KS_ERR_UNSUPPORTED; }
   if (C > 1) {
     // cluster path: the C*T threads of a cluster share the agents
     int T = s->opt_threads ? s->opt_threads : 256;
@@ -310,7 +330,9 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     else         e = mix ? launch_cluster<1, true>(P, C, T, st) : launch_cluster<0, true>(P, C, T, st);
   } else {
     const LaunchPlan pl = plan_launch(s);
-    if (packed)
+    if (paper)
+      e = launch_persistent<2, 0, false>(P, pl.T, pl.smem, st);
+    else if (packed)
       e = mix ? launch_persistent<1, 0, true>(P, pl.T, pl.smem, st) : launch_persistent<0, 0, true>(P, pl.T, pl.smem, st);
     else if (!mix)
       e = s->opt_atomic ? launch_persistent<0, 1, false>(P, pl.T, pl.smem, st) : launch_persistent<0, 0, false>(P, pl.T, pl.smem, st);

@@ -52,6 +52,9 @@ struct KernelParams {
   int32_t force_generic;                          // ablation/test: always use the chunked scan
   int32_t log2C;                                  // cluster kernel only: CTAs per market = 1 << log2C
   int2* trace;                                    // DEVICE [M][S] (price after the step, Vmax), or NULL
+  // model 4 (the paper's agent model, A24): class sizes and the marketable threshold;
+  // the half spread is maker_spread_max and the makers' qmax is maker_qty
+  int32_t paper_n_noise, paper_n_mom, paper_pmkt_q16;
   long long S;                                    // steps to run
   long long orders_per_step;                      // A + number of makers
 };
@@ -233,6 +236,8 @@ struct RuleCtx {
   bool noclamp;          // last - noise_delta >= 0 and last + noise_delta <= L-1: the noise clamp is the identity
   uint32_t bid_lo;       // shared address of bid[last - noise_delta]
   uint32_t ask_lo;       // shared address of ask[last - noise_delta]
+  int mid2;              // model 4: doubled mid price of the resting book (Eq.3); dp = sgn(mid2 - previous mid2)
+  int* mkt_flags;        // model 4: shared int[2], set when a marketable buy [0] / sell [1] was generated
 };
 
 // a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; sell tick = (last - delta) + o, buy tick =
@@ -337,6 +342,36 @@ __device__ __forceinline__ void packed_agent(const KernelParams& P, const BookRe
   if (KIND == 0)      noise_order_packed<ATOM, CLAMP>(P, book, rc, w, sink);
   else if (KIND == 1) maker_order<ATOM>(P, book, rc, w, sink);
   else                momentum_order_packed<ATOM>(P, book, rc, w, sink);
+}
+
+// ---- model 4, the paper's agent model (SIII-C; A24), doubled-integer
+// prices: round(m2 / 2) half up = (m2 + 1) >> 1 (arithmetic shift = floor).  KIND 0 noise,
+// 1 momentum, 2 maker.  `parity` = (a + t) & 1 of this thread's agents (T is even, so it is the
+// same for all of them).  Marketable orders go to the grid boundary and raise a flag so that the
+// clearing warp widens its window to that boundary.
+template <int ATOM, int KIND>
+__device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
+                                            const uint32_t (&w)[4], uint32_t parity, int& sink) {
+  bool buy; int p2, q;
+  if (KIND == 0) {
+    buy = (int32_t)w[0] < 0;
+    p2 = rc.mid2 + 2 * ((int)__umulhi(w[1], (uint32_t)P.noise_n) - P.noise_delta);
+    q = 1 + (int)__umulhi(w[2], (uint32_t)P.noise_qmax);
+  } else if (KIND == 1) {
+    buy = rc.dp > 0 ? true : (rc.dp < 0 ? false : ((int32_t)w[0] < 0));
+    p2 = rc.mid2 + (buy ? 2 : -2);
+    q = 1 + (int)__umulhi(w[2], (uint32_t)P.mom_qmax);
+  } else {
+    buy = parity == 0u;
+    p2 = rc.mid2 + (buy ? -2 : 2) * P.maker_spread_max;
+    q = 1 + (int)__umulhi(w[2], (uint32_t)P.maker_qty);
+  }
+  int tick = clamp_tick((p2 + 1) >> 1, rc.L);
+  if (KIND != 2 && (int)(w[3] >> 16) < P.paper_pmkt_q16) {
+    tick = buy ? rc.L - 1 : 0;
+    rc.mkt_flags[buy ? 0 : 1] = 1;
+  }
+  book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
 }
 
 // The agents of one class that a thread visits: first, first + a_step, ... < a_end.  p0 = M0*first;
@@ -451,6 +486,80 @@ __device__ __forceinline__ GenPlan<MODEL> gen_plan(uint32_t count, int tid, int 
   // hide that p0_inc is a product: otherwise p0 += p0_inc is turned back into IMAD.WIDE(M0, a_step, p0)
   asm volatile("" : "+l"(g.p0_inc));
   return g;
+}
+
+template <int ATOM, int KIND>
+__device__ __forceinline__ void generate_class_paper(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                                     const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
+                                                     uint64_t p0_inc, uint32_t parity, int& sink) {
+  auto one = [&](uint64_t p0) {
+    uint32_t w[4];
+    philox_block_from_p0(P, mu, u, p0, w);
+    paper_order<ATOM, KIND>(P, book, rc, w, parity, sink);
+  };
+  uint64_t p0 = pl.p0;
+#pragma unroll kGenUnroll
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
+  if (pl.extra) one(p0);
+}
+
+// model 4: three classes on contiguous agent ranges [0, n_noise), [n_noise, n_noise + n_mom), [.., A)
+__device__ __forceinline__ GenPlan<2> gen_plan_paper(const KernelParams& P, int tid, int T) {
+  GenPlan<2> g;
+  const uint32_t e0 = (uint32_t)P.paper_n_noise, e1 = e0 + (uint32_t)P.paper_n_mom, e2 = (uint32_t)P.A;
+  g.p0_inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
+  g.cls[0] = class_plan((uint32_t)tid, (uint32_t)(T - 1), e0, (uint32_t)T);
+  g.cls[1] = class_plan(e0 + (uint32_t)tid, e0 + (uint32_t)(T - 1), e1, (uint32_t)T);
+  g.cls[2] = class_plan(e1 + (uint32_t)tid, e1 + (uint32_t)(T - 1), e2, (uint32_t)T);
+  asm volatile("" : "+l"(g.p0_inc));
+  return g;
+}
+
+template <int ATOM>
+__device__ __forceinline__ void generate_step_paper(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                                    const StepUniform& u, const RuleCtx& rc, const GenPlan<2>& g,
+                                                    int tid, uint32_t t, int& sink) {
+  const uint32_t maker_first = (uint32_t)P.paper_n_noise + (uint32_t)P.paper_n_mom + (uint32_t)tid;
+  generate_class_paper<ATOM, 0>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, sink);
+  generate_class_paper<ATOM, 1>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, sink);
+  generate_class_paper<ATOM, 2>(P, book, mu, u, rc, g.cls[2], g.p0_inc, (maker_first + t) & 1u, sink);
+}
+
+// The highest tick < `from` with bid depth (-1 if none) / the lowest tick >= `from` with ask depth
+// (L if none): chunked warp scans, used by model 4 when the cleared window holds no depth on a
+// side and the exact best quote (Eq.3) lies outside it.
+template <class IO>
+static __device__ __noinline__ int best_bid_below(const IO& io, int L, int from, int lane) {
+  for (int c = (from - 1) & ~127; from > 0 && c >= 0; c -= 128) {
+    const int t = c + 4 * lane;
+    int best = -1;
+    if (t < L) {
+      const int4 v = io.ld4(0, t);
+      const int vals[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) if (vals[j] > 0 && t + j < from) best = t + j;
+    }
+    best = __reduce_max_sync(0xffffffffu, best);
+    if (best >= 0) return best;
+  }
+  return -1;
+}
+
+template <class IO>
+static __device__ __noinline__ int best_ask_from(const IO& io, int L, int from, int lane) {
+  for (int c = max(from, 0) & ~127; c < L; c += 128) {
+    const int t = c + 4 * lane;
+    int best = 0x7fffffff;
+    if (t < L) {
+      const int4 v = io.ld4(1, t);
+      const int vals[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int j = 3; j >= 0; --j) if (vals[j] > 0 && t + j >= from) best = t + j;
+    }
+    best = __reduce_min_sync(0xffffffffu, best);
+    if (best != 0x7fffffff) return best;
+  }
+  return L;
 }
 
 // a1 + a2 for one market-step: every thread of the CTA generates the orders of its agents.

@@ -58,9 +58,22 @@ __device__ __forceinline__ void update_record(long long* rec, int last, int vmax
   rec[F_LAST] = new_last;
 }
 
+// The per-thread generation plan of a launch (MODEL 2 = the paper's agent model has its own).
+template <int MODEL>
+__device__ __forceinline__ GenPlan<MODEL> make_gen_plan(const KernelParams& P, bool packed, int tid, int T) {
+  return gen_plan<MODEL>(packed ? (uint32_t)P.A >> 2 : (uint32_t)P.A, tid, T);
+}
+template <>
+__device__ __forceinline__ GenPlan<2> make_gen_plan<2>(const KernelParams& P, bool, int tid, int T) {
+  return gen_plan_paper(P, tid, T);
+}
+
+__device__ __forceinline__ int sign_of(int x) { return (x > 0) - (x < 0); }
+
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
-// dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3.  ATOM: see book_add.
+// dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3, 2 = the paper's agent
+// model (mid-price reference, A24).  ATOM: see book_add.
 // PACKED: the PACKED4 draw contract (one Philox block per four agents, A22).
 // ---------------------------------------------------------------------------------------------
 template <int MODEL, int ATOM, bool PACKED>
@@ -71,6 +84,8 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   __shared__ int s_red32[64];
   __shared__ int2 s_trace[32];                        // staged trace entries (only when P.trace)
   __shared__ __align__(16) int s_ctl[4];              // per-step broadcast: last, &bid[last-delta], &ask[last-delta], noclamp
+                                                      // (MODEL 2: last, mid2, sgn(mid2 - previous mid2), 0)
+  __shared__ int s_mkt[2];                            // MODEL 2: a marketable buy / sell was generated this step
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
   const int L = P.L;
@@ -79,7 +94,7 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   long long* grec = P.recs + (size_t)blockIdx.x * 16;
   const MarketUniform mu = market_uniform(P, market);
 
-  const GenPlan<MODEL> gplan = gen_plan<MODEL>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, tid, T);
+  const GenPlan<MODEL> gplan = make_gen_plan<MODEL>(P, PACKED, tid, T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
 
   // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
@@ -120,7 +135,16 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
     RuleCtx rc = rule_ctx(P, bref, new_last, new_last);
     *reinterpret_cast<int4*>(s_ctl) = make_int4(new_last, (int)rc.bid_lo, (int)rc.ask_lo, rc.noclamp ? 1 : 0);
   };
-  if (tid == 0) publish(last);
+  // MODEL 2: Eq.3 on the exact best quotes of the resting book; f[13] holds the
+  // doubled mid of the previous step
+  auto publish_paper = [&](int new_last, int bb, int ba, int mid2_before) {
+    const int mid2 = (bb >= 0 && ba < L) ? bb + ba : 2 * new_last;
+    *reinterpret_cast<int4*>(s_ctl) = make_int4(new_last, mid2, sign_of(mid2 - mid2_before), 0);
+  };
+  if (tid == 0) {
+    if (MODEL == 2) { publish_paper(last, bmax, amin, prev); s_mkt[0] = 0; s_mkt[1] = 0; }
+    else publish(last);
+  }
   __syncthreads();
   // ---- S steps, all on-chip
   for (long long s = 0; s < P.S; ++s) {
@@ -129,27 +153,54 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
     const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
     last = ctl.x;
     RuleCtx rc;
-    rc.last = last; rc.dp = last - prev; rc.L = L;
-    rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
-    // a1 + a2: order generation and aggregation
-    generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+    rc.last = last; rc.L = L;
+    if constexpr (MODEL == 2) {
+      rc.mid2 = ctl.y; rc.dp = ctl.z; rc.noclamp = false; rc.bid_lo = 0; rc.ask_lo = 0; rc.mkt_flags = s_mkt;
+      generate_step_paper<ATOM>(P, bref, mu, u, rc, gplan, tid, t, sink);
+    } else {
+      rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
+      rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
+      // a1 + a2: order generation and aggregation
+      generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+    }
     __syncthreads();                                   // B1: the combined book is complete
 
     // a3-a6: clearing by warp 0 on the active window
     if (warp == 0) {
-      int lo = max(0, min(amin, last - P.dmax));
-      int hi = min(L - 1, max(bmax, last + P.dmax));
-      int vmax, pstar, nb, na;
+      int lo, hi;
+      if (MODEL == 2) {
+        lo = max(0, min(amin, (rc.mid2 >> 1) - P.dmax));
+        hi = min(L - 1, max(bmax, ((rc.mid2 + 1) >> 1) + P.dmax));
+        if (s_mkt[0]) hi = L - 1;                      // marketable buys sit at tick L-1,
+        if (s_mkt[1]) lo = 0;                          // marketable sells at tick 0
+        __syncwarp();
+      } else {
+        lo = max(0, min(amin, last - P.dmax));
+        hi = min(L - 1, max(bmax, last + P.dmax));
+      }
+      int vmax, pstar, nb, na, base, wend;
       int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
       const LocalBook io{book, L};
-      if (P.force_generic || width8 > 256) clear_generic(io, L, lo & ~3, hi, lane, vmax, pstar, nb, na);
-      else if (width4 <= 128)              clear_window<4>(io, L, lo & ~3, lane, vmax, pstar, nb, na);
-      else                                 clear_window<8>(io, L, lo & ~7, lane, vmax, pstar, nb, na);
+      if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, nb, na); }
+      else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, nb, na); }
+      else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, nb, na); }
+      if (MODEL == 2) {
+        // the mid price needs the EXACT best quotes: a side with no depth inside the window is
+        // searched outside it (rare: the window was emptied on that side)
+        if (nb < base) nb = best_bid_below(io, L, base, lane);
+        if (na >= wend) na = best_ask_from(io, L, wend, lane);
+      }
       bmax = nb; amin = na;
       if (lane == 0) {
         int new_last;
         update_record(s_rec, last, vmax, pstar, new_last);
-        publish(new_last);
+        if (MODEL == 2) {
+          s_rec[F_PREV] = rc.mid2;
+          publish_paper(new_last, nb, na, rc.mid2);
+          s_mkt[0] = 0; s_mkt[1] = 0;
+        } else {
+          publish(new_last);
+        }
       }
       if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)P.S, s, P.S, lane,
                               vmax > 0 ? pstar : last, vmax);
@@ -185,14 +236,15 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
 }
 
 // ks_create: empty books, opening price, zero accumulators (Alg.1 l.2-3).
-__global__ void ks_init_kernel(int4* books4, size_t nvec, long long* recs, int M, int init_price) {
+__global__ void ks_init_kernel(int4* books4, size_t nvec, long long* recs, int M, int init_price, int init_prev) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t v = i; v < nvec; v += stride) books4[v] = make_int4(0, 0, 0, 0);
   for (size_t r = i; r < (size_t)M * 16; r += stride) {
     int f = (int)(r & 15);
     long long val = 0;
-    if (f == F_LAST || f == F_PREV) val = init_price;
+    if (f == F_LAST) val = init_price;
+    if (f == F_PREV) val = init_prev;                  // model 4: the doubled opening price (previous mid)
     if (f == F_HASH) val = (long long)kHashBasis;
     recs[r] = val;
   }

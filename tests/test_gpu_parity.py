@@ -5,8 +5,8 @@ import numpy as np
 import pytest
 
 from ks_testlib import assert_rows_equal, ints, oracle_rows, read_golden
-from paper_2606_21784_b200.workloads import (CONFIGS, mix3_params, packed4, random_books, sampled_markets,
-                                             zi_params)
+from paper_2606_21784_b200.workloads import (CONFIGS, mix3_params, packed4, paper_params, random_books,
+                                             sampled_markets, zi_params)
 
 pytestmark = pytest.mark.gpu
 
@@ -295,6 +295,46 @@ def test_trace_stats_degenerate_series(ks, oracle):
     assert got[1, 0] == 1.0 and got[1, 1] == -2.0 and got[1, 4] == -(100 - 1) / 100
     one = ks.ks_trace_stats(d[:, :1, :].contiguous(), 5, 1, K).cpu().numpy()
     assert np.array_equal(one[:, 2], p[:, 0, 1].astype(np.float64)) and np.isnan(np.delete(one, 2, axis=1)).all()
+
+
+# ------------------------------------------------------------------ the paper's own agent model
+@pytest.mark.parametrize("alpha_mom", [0.0, 0.15, 0.7])
+def test_paper_agent_model_matches_the_oracle(ks, oracle, alpha_mom):
+    """SURVEY.md S8(f)-2 / DESIGN.md A24: mid-price reference (Eq.3) from the exact best quotes of
+    the resting book, marketable orders at the grid boundary, parity makers, momentum on mid
+    changes, classes by index ranges.  Several grid sizes (full-grid windows through
+    clear_window<4>/<8> and the chunked scan), block sizes, split / launch-per-step runs, injected
+    books whose best quotes lie far outside the active window, the trace."""
+    import torch
+    for (M, L, A, S, T, pm) in [(17, 128, 200, 120, 0, 0.05), (9, 256, 333, 60, 96, 0.2), (7, 2048, 500, 50, 0, 0.02),
+                                (5, 64, 90, 80, 1024, 0.0), (6, 512, 64, 60, 32, 1.0)]:
+        p = paper_params(A, alpha_mom, 0.15, delta=min(8, L // 8), p_mkt=pm)
+        ids = np.arange(M)
+        eb, er = oracle_rows(oracle, p, L, A, 5, ids, S)
+        for kw in (dict(), dict(split=[1, S // 2, S - 1 - S // 2]), dict(stepwise=True), dict(opts=[(ks.KS_OPT_CLEAR_PATH, 1)])):
+            opts = list(kw.pop("opts", [])) + [(ks.KS_OPT_BLOCK_THREADS, T)]
+            b, r = _gpu(ks, M, L, A, p, 5, S, opts=opts, **kw)
+            assert_rows_equal(b, r, ids, eb, er, "paper model L=%d alpha=%.2f %r" % (L, alpha_mom, kw))
+    # injected books: crossed / one-sided / sparse far-away quotes
+    M, L, A = 8, 1024, 150
+    p = paper_params(A, alpha_mom, 0.15, delta=6, p_mkt=0.0)
+    books = random_books(M, L, seed=3, max_qty=30, fill=0.01)
+    books[0] = 0
+    books[1, 1] = 0
+    books[2] = 0; books[2, 0, 3] = 5; books[2, 1, 1000] = 5           # quotes far from the price
+    books[3] = random_books(1, L, seed=9, fill=0.002, crossed=False)[0]
+    eb0, er0 = oracle.init_state(M, L, -1, model=4)
+    eb, er, et = oracle.run_markets_traced(p, L, A, 7, np.arange(M), 40, books, er0)
+    sim = ks.KsSim(M, L, A, p, 7)
+    sim.ks_write_books(torch.from_numpy(books).cuda())
+    tr = torch.empty((M, 40, 2), dtype=torch.int32, device="cuda")
+    sim.ks_run_traced(40, tr)
+    b, r = sim.books_to_host(), sim.stats_to_host()
+    assert_rows_equal(b, r, np.arange(M), eb, er, "paper model injected")
+    assert np.array_equal(tr.cpu().numpy(), et)
+    with pytest.raises(ks.KsError):
+        sim.ks_set_option(ks.KS_OPT_CLUSTER_SIZE, 2)
+    sim.ks_destroy()
 
 
 # ------------------------------------------------------------------ book injection / edge cases
