@@ -27,7 +27,7 @@ if ROOT not in sys.path:
 
 import dataclasses  # noqa: E402
 
-from paper_2606_21784_b200.workloads import CONFIGS, KS_MODEL_ZI, packed4, sampled_markets  # noqa: E402
+from paper_2606_21784_b200.workloads import CONFIGS, KS_MODEL_ZI, packed4, paper_params, sampled_markets  # noqa: E402
 
 # Roofline of ks_persistent_kernel: the fmaheavy pipe that executes the 32x32->64
 # multiplies.  Algorithmic multiplies per agent event: 20 of Philox4x32-10 + the
@@ -377,6 +377,39 @@ def main():
             "slowdown_vs_persistent": ms / extra["C2"]["ms_median_of_3"],
             "algorithmic_hbm_bytes": hbm_bytes, "hbm_GBps": hbm_bytes / (ms * 1e-3) / 1e9,
             "persistent_hbm_bytes": float(c.M) * (8 * c.L + 128)}
+
+    if args.all_configs and world == 1:
+        # SIV-J sweep shape: alpha_mom = 0 .. 0.70 in steps of 0.05, alpha_maker
+        # = 0.15, M = 64 markets x S = 1000 steps each, the paper's own agent model (model 4), traced,
+        # statistics on the device.  A = 200 (12.8e6 events / 64 / 1000: PAPER.md:458); L, Delta,
+        # q_max, P_mkt are not given -- workloads.paper_params defaults.  Context, not a parity case.
+        Ms, Ls, As, Ss, K = 64, 128, 200, 1000, 20
+        st = torch.empty(ks.ks_state_bytes(Ms, Ls), dtype=torch.uint8, device=dev)
+        tr = torch.empty((Ms, Ss, 2), dtype=torch.int32, device=dev)
+        out = torch.empty((Ms, 4 + 2 * K), dtype=torch.float64, device=dev)
+        alphas = [round(0.05 * i, 2) for i in range(15)]
+        rows = []
+
+        def sweep(record):
+            for al in alphas:
+                sim = ks.KsSim(Ms, Ls, As, paper_params(As, al), 5, state=st)
+                sim.ks_run_traced(Ss, tr)
+                ks.ks_trace_stats(tr, Ms, Ss, K, out)
+                if record:
+                    o = out.cpu().numpy()
+                    rows.append({"alpha_mom": al, "volatility": float(np.nanmean(o[:, 0])), "excess_kurtosis": float(np.nanmean(o[:, 1])),
+                                 "volume_per_step": float(np.nanmean(o[:, 2])), "acf_r_lag1": float(np.nanmean(o[:, 4])),
+                                 "acf_abs_r_lag1": float(np.nanmean(o[:, 4 + K]))})
+                sim.ks_destroy()
+
+        sweep(False)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); sweep(False); b.record(); torch.cuda.synchronize()
+        sweep(True)
+        line["sivj_sweep"] = {"configs": len(alphas), "M": Ms, "L": Ls, "A": As, "S": Ss, "agent_events": len(alphas) * Ms * As * Ss,
+                              "ms_total_device": a.elapsed_time(b), "paper": "< 250 ms for 12.8e6 events (RTX 5090, PAPER.md:458)",
+                              "mean_over_markets": rows}
 
     if not args.no_cpu_baseline and world == 1:
         n_mk = min(cfg.M, 64)
