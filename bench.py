@@ -379,6 +379,25 @@ def main():
             "persistent_hbm_bytes": float(c.M) * (8 * c.L + 128)}
 
     if args.all_configs and world == 1:
+        # context runs in the paper's own shapes: Table IV's fixed workload M=8192,
+        # A=256, L=128, S=500 and the latency configuration M=4096, A=256 with
+        # zero-intelligence agents Delta=8, q<=10, seed 5 -- NOT the paper's agent model or GPU
+        from paper_2606_21784_b200.workloads import zi_params
+        ctx = {}
+        for name, Mp in (("table4_M8192_A256_L128_S500", 8192), ("latency_M4096_A256_L128_S500", 4096)):
+            st = torch.empty(ks.ks_state_bytes(Mp, 128), dtype=torch.uint8, device=dev)
+            ts = []
+            for i in range(6):
+                sim = ks.KsSim(Mp, 128, 256, zi_params(8, 10), 5, state=st)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); sim.ks_run(500); b.record(); torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b)); sim.ks_destroy()
+            ms = float(np.median(ts[1:]))
+            ctx[name] = {"ms_median_of_5": ms, "events_per_s": Mp * 256 * 500 / (ms * 1e-3), "us_per_step": ms * 1e3 / 500}
+        ctx["paper"] = "KineticSim on RTX 5090: 20.2 ms, 5.2e10 events/s (Table IV); 22.1 us median per step at M=4096 (PAPER.md:438)"
+        line["paper_shape_context"] = ctx
+
+    if args.all_configs and world == 1:
         # SIV-J sweep shape: alpha_mom = 0 .. 0.70 in steps of 0.05, alpha_maker
         # = 0.15, M = 64 markets x S = 1000 steps each, the paper's own agent model (model 4), traced,
         # statistics on the device.  A = 200 (12.8e6 events / 64 / 1000: PAPER.md:458); L, Delta,

@@ -52,6 +52,12 @@ struct ClusterBook {
     asm volatile("st.shared::cluster.v4.s32 [%0], {%1, %2, %3, %4};"
                  ::"r"(addr(side, tick)), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
   }
+  __device__ __forceinline__ int ld1(int side, int tick) const {
+    int v;
+    asm volatile("ld.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(addr(side, tick)) : "memory");
+    return v;
+  }
+  __device__ __forceinline__ void st1(int side, int tick, int v) const { st_cluster_s32(addr(side, tick), v); }
 };
 
 // grid = M*C CTAs in clusters of C = 1 << P.log2C (cluster <-> market), block = T threads,
@@ -152,6 +158,7 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
       int vmax, pstar, nb, na;
       int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
       if (P.force_generic || width8 > 256) clear_generic(io, L, lo & ~3, hi, lane, vmax, pstar, nb, na);
+      else if (hi - lo < 32)               clear_window1(io, L, lo, lane, vmax, pstar, nb, na);
       else if (width4 <= 128)              clear_window<4>(io, L, lo & ~3, lane, vmax, pstar, nb, na);
       else                                 clear_window<8>(io, L, lo & ~7, lane, vmax, pstar, nb, na);
       bmax = nb; amin = na;

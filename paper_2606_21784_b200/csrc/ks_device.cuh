@@ -617,6 +617,8 @@ struct LocalBook {
   __device__ __forceinline__ void st4(int side, int tick, int4 v) const {
     *reinterpret_cast<int4*>((side ? book + L : book) + tick) = v;
   }
+  __device__ __forceinline__ int ld1(int side, int tick) const { return (side ? book + L : book)[tick]; }
+  __device__ __forceinline__ void st1(int side, int tick, int v) const { (side ? book + L : book)[tick] = v; }
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -701,6 +703,39 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
   amin_new = __reduce_min_sync(FULL, la);
   if (bmax_new < 0) bmax_new = base - 1;
   if (amin_new == 0x7fffffff) amin_new = min(L, base + 32 * K);
+}
+
+// a3-a5 for a window of at most 32 ticks starting at `base` (any alignment): one tick per lane, no
+// inner loops -- the short path for small offset ranges (C1, C3: delta = 8), where the clearing
+// chain is what bounds the step.  Same definitions as clear_window.
+template <class IO>
+__device__ __forceinline__ void clear_window1(const IO& io, int L, int base, int lane,
+                                              int& vmax, int& pstar, int& bmax_new, int& amin_new) {
+  const unsigned FULL = 0xffffffffu;
+  const int tick = base + lane;
+  const bool in = tick < L;
+  int b = in ? io.ld1(0, tick) : 0, a = in ? io.ld1(1, tick) : 0;
+  int D = b, S = a;                     // inclusive suffix of bids / prefix of asks over lanes
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    int vb = __shfl_down_sync(FULL, D, d);
+    int va = __shfl_up_sync(FULL, S, d);
+    if (lane + d < 32) D += vb;
+    if (lane >= d) S += va;
+  }
+  const int V = min(D, S);
+  vmax = __reduce_max_sync(FULL, V);
+  pstar = __reduce_min_sync(FULL, (V == vmax && vmax > 0) ? tick : 0x7fffffff);
+  if (vmax > 0) {
+    const int nbid = min(b, max(0, D - vmax)), nask = min(a, max(0, S - vmax));
+    if (in && nbid != b) io.st1(0, tick, nbid);
+    if (in && nask != a) io.st1(1, tick, nask);
+    b = nbid; a = nask;
+  }
+  bmax_new = __reduce_max_sync(FULL, b > 0 ? tick : -1);
+  amin_new = __reduce_min_sync(FULL, a > 0 ? tick : 0x7fffffff);
+  if (bmax_new < 0) bmax_new = base - 1;
+  if (amin_new == 0x7fffffff) amin_new = min(L, base + 32);
 }
 
 // General window of any width: chunks of 128 ticks, three passes (total bid depth; profiles and

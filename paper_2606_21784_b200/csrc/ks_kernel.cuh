@@ -182,6 +182,7 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
       int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
       const LocalBook io{book, L};
       if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, nb, na); }
+      else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, nb, na); }
       else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, nb, na); }
       else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, nb, na); }
       if (MODEL == 2) {
