@@ -443,7 +443,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 25957888 + 239323648,            # profiles/r1c_persistent_full.md
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 28012544 + 239491840,            # profiles/r1e_persistent_full.md
                                   "C4_packed4": 20602880 + 231495936}    # profiles/r1d_packed_persistent_full.md
 
 if __name__ == "__main__":
