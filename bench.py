@@ -336,6 +336,9 @@ def main():
         wide, _ = ks.ks_bench_int_pipe(0)
         lop, _ = ks.ks_bench_int_pipe(1)
         mix, _ = ks.ks_bench_int_pipe(2)
+        mix2, _ = ks.ks_bench_int_pipe(3)
+        mix3, _ = ks.ks_bench_int_pipe(4)
+        cyc = lambda ops_s, per: sms * 4 * sm_max_mhz * 1e6 * 32 * per / ops_s      # SMSP cycles per IMAD.WIDE
         atomics_per_event = 1.0 if model.startswith("zi") else 4.0 / 3.0
         kev = events_per_step / avg_kern_s
         line["microbench"] = {
@@ -343,6 +346,8 @@ def main():
             "smem_atomic_pattern_warp_aggregated_lane_ops_per_s": agg_ops, "smem_atomic_same_address_lane_ops_per_s": one_ops,
             "generate_only_events_per_s": gen_ev, "imad_wide_thread_ops_per_s": wide, "lop3_thread_ops_per_s": lop,
             "imad_wide_lop3_mix_thread_ops_per_s": mix,
+            "smsp_cycles_per_imad_wide": {"alone": cyc(wide, 1), "with_1_lop3": cyc(mix, 2), "with_2_lop3": cyc(mix2, 3),
+                                          "with_3_lop3": cyc(mix3, 4)},
             "frac_of_smem_atomic_peak": kev * atomics_per_event / peak_ops,
             "frac_of_smem_atomic_pattern": kev * atomics_per_event / pat_ops,
             "frac_of_generate_only": kev / gen_ev,

@@ -42,8 +42,9 @@ KS_API ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int
                                         void* stream, double* events_per_s, double* seconds);
 
 /* Raw issue rates of the two instructions Philox is made of.  kind 0: IMAD.WIDE.U32 (u32 x u32 ->
- * u64), kind 1: LOP3 (three-input xor), kind 2: one of each, interleaved.  Each thread runs 8
- * independent dependency chains.  *thread_ops_per_s receives thread-level operations per second
+ * u64), kind 1: LOP3 (three-input xor), kind 2: one of each, interleaved (the Philox round
+ * pattern), kind 3 / 4: one IMAD.WIDE with two / three LOP3 (what every further alu-pipe instruction
+ * costs the multiply stream).  Each thread runs 8 independent dependency chains.  *thread_ops_per_s receives thread-level operations per second
  * over the whole GPU (divide by 32 x SMs x 4 x clock for warp instructions per cycle per
  * scheduler). */
 KS_API ks_status ks_bench_int_pipe(int32_t kind, int32_t threads, int32_t ctas_per_sm, int32_t iters,

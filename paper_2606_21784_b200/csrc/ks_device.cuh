@@ -21,6 +21,13 @@
 #define KS_GEN_UNROLL 2      // independent Philox chains per thread in the generation loop
 #endif
 
+#ifndef KS_VECTOR_KEYS
+#define KS_VECTOR_KEYS 0     // Philox round keys in per-thread registers (1) or uniform registers (0)
+#endif
+#ifndef KS_P0_WIDE
+#define KS_P0_WIDE 0         // round-0 product advanced by one IMAD.WIDE accumulate (1) or by a 64-bit add (0)
+#endif
+
 namespace ks {
 
 constexpr int kGenUnroll = KS_GEN_UNROLL;
@@ -84,9 +91,31 @@ __device__ __forceinline__ uint32_t lo32(uint64_t x) { return (uint32_t)x; }
 // (IMAD.WIDE/IMAD.HI hold an SMSP's fmaheavy pipe for 4 cycles per warp), so per
 // event the path issues 16 IMAD.WIDE + 1 IMAD.HI for rounds 1..9 and 2 IMAD.HI for the agent rule.
 // ---------------------------------------------------------------------------------------------
-struct MarketUniform {   // depends on the market only
+// The round keys as the hot loop reads them.  The kernel is bound by the DISPATCH of 16-lane math
+// instructions (every IMAD.* / LOP3 / IADD3 holds the shared alu+fma dispatch port for 2 cycles;
+// DESIGN.md 7.2), and a LOP3 with a uniform-register operand measures ~0.2 cycles slower than
+// one with three vector operands, so the keys are copied once into per-thread registers through
+// an opaque move (the compiler would otherwise keep them uniform).
+struct Keys { uint32_t k0[10], k1[10]; };
+
+__device__ __forceinline__ Keys load_keys(const KernelParams& P) {
+  Keys K;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+#if KS_VECTOR_KEYS
+    asm volatile("mov.u32 %0, %1;" : "=r"(K.k0[r]) : "r"(P.k0[r]));
+    asm volatile("mov.u32 %0, %1;" : "=r"(K.k1[r]) : "r"(P.k1[r]));
+#else
+    K.k0[r] = P.k0[r]; K.k1[r] = P.k1[r];
+#endif
+  }
+  return K;
+}
+
+struct MarketUniform {   // depends on the market only (plus the launch's keys, carried along)
   uint32_t hm;     // hi(M1*m)
   uint32_t n1k;    // lo(M1*m) ^ k0[1]
+  Keys K;          // round keys for the per-event rounds
 };
 struct StepUniform {     // depends on (market, step)
   uint32_t d2x;    // hi(M0*n0) ^ k1[1]
@@ -99,6 +128,7 @@ __device__ __forceinline__ MarketUniform market_uniform(const KernelParams& P, u
   MarketUniform mu;
   mu.hm = hi32(pm);
   mu.n1k = lo32(pm) ^ P.k0[1];
+  mu.K = load_keys(P);
   return mu;
 }
 
@@ -119,7 +149,7 @@ __device__ __forceinline__ StepUniform step_uniform(const KernelParams& P, const
 __device__ __forceinline__ void philox_rounds_0_8(const KernelParams& P, const MarketUniform& mu, const StepUniform& u,
                                                   uint64_t p0, uint32_t& c0, uint32_t& c1, uint32_t& c2, uint32_t& c3) {
   {                                       // rounds 0-1
-    const uint32_t n2 = hi32(p0) ^ P.k1[0];
+    const uint32_t n2 = hi32(p0) ^ mu.K.k1[0];
     const uint64_t p1 = (uint64_t)kPhiloxM1 * n2;
     c0 = hi32(p1) ^ mu.n1k;
     c1 = lo32(p1);
@@ -128,7 +158,7 @@ __device__ __forceinline__ void philox_rounds_0_8(const KernelParams& P, const M
   {                                       // round 2: c3 = d3 is uniform, d3 ^ k1[2] was pre-xored
     uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
     uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
-    uint32_t t0 = hi32(a1) ^ c1 ^ P.k0[2];
+    uint32_t t0 = hi32(a1) ^ c1 ^ mu.K.k0[2];
     uint32_t t2 = hi32(a0) ^ u.d3k;
     c1 = lo32(a1); c3 = lo32(a0); c0 = t0; c2 = t2;
   }
@@ -136,8 +166,8 @@ __device__ __forceinline__ void philox_rounds_0_8(const KernelParams& P, const M
   for (int r = 3; r < 9; ++r) {
     uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
     uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
-    uint32_t t0 = hi32(a1) ^ c1 ^ P.k0[r];
-    uint32_t t2 = hi32(a0) ^ c3 ^ P.k1[r];
+    uint32_t t0 = hi32(a1) ^ c1 ^ mu.K.k0[r];
+    uint32_t t2 = hi32(a0) ^ c3 ^ mu.K.k1[r];
     c1 = lo32(a1);
     c3 = lo32(a0);
     c0 = t0;
@@ -153,8 +183,8 @@ __device__ __forceinline__ void philox_from_p0(const KernelParams& P, const Mark
   uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
   w1 = lo32(a1);
   if (NEED02) {
-    w0 = hi32(a1) ^ c1 ^ P.k0[9];
-    w2 = __umulhi(kPhiloxM0, c0) ^ c3 ^ P.k1[9];
+    w0 = hi32(a1) ^ c1 ^ mu.K.k0[9];
+    w2 = __umulhi(kPhiloxM0, c0) ^ c3 ^ mu.K.k1[9];
   } else {
     w0 = 0; w2 = 0;
   }
@@ -167,9 +197,9 @@ __device__ __forceinline__ void philox_block_from_p0(const KernelParams& P, cons
   philox_rounds_0_8(P, mu, u, p0, c0, c1, c2, c3);
   const uint64_t a0 = (uint64_t)kPhiloxM0 * c0;
   const uint64_t a1 = (uint64_t)kPhiloxM1 * c2;
-  w[0] = hi32(a1) ^ c1 ^ P.k0[9];
+  w[0] = hi32(a1) ^ c1 ^ mu.K.k0[9];
   w[1] = lo32(a1);
-  w[2] = hi32(a0) ^ c3 ^ P.k1[9];
+  w[2] = hi32(a0) ^ c3 ^ mu.K.k1[9];
   w[3] = lo32(a0);
 }
 
@@ -395,6 +425,13 @@ __device__ __forceinline__ ClassPlan class_plan(uint32_t first, uint32_t first_o
 
 // p + inc as an explicit carry chain, so that it stays one IADD3 + one IADD3.X on the alu pipe and
 // is neither turned back into a multiply nor duplicated per unrolled copy.
+struct P0Step { uint64_t inc; uint32_t a_step; };   // inc = M0 * a_step
+
+// Advance the round-0 product p0 = M0*a by a_step agents.  KS_P0_WIDE: one IMAD.WIDE with p0 as its
+// 64-bit addend -- ONE dispatch slot; the alternative (IADD3 + carry add) spares the fma pipe but
+// costs two slots, and dispatch is what binds.
+__device__ __forceinline__ uint64_t advance_p0(uint64_t p, uint64_t inc, uint32_t a_step);
+
 __device__ __forceinline__ uint64_t add64_alu(uint64_t p, uint64_t inc) {
   uint32_t lo, hi;
   asm volatile("add.cc.u32 %0, %2, %4;\n\taddc.u32 %1, %3, %5;"
@@ -403,11 +440,21 @@ __device__ __forceinline__ uint64_t add64_alu(uint64_t p, uint64_t inc) {
   return ((uint64_t)hi << 32) | lo;
 }
 
+__device__ __forceinline__ uint64_t advance_p0(uint64_t p, uint64_t inc, uint32_t a_step) {
+#if KS_P0_WIDE
+  uint64_t r;
+  asm volatile("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(a_step), "r"(kPhiloxM0), "l"(p));
+  return r;
+#else
+  return add64_alu(p, inc);
+#endif
+}
+
 // One agent class of one market-step, rule KIND (0 noise, 1 maker, 2 momentum).
 template <int ATOM, int KIND, bool CLAMP>
 __device__ __forceinline__ void generate_class(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                                const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
-                                               uint64_t p0_inc, int& sink) {
+                                               const P0Step& p0_inc, int& sink) {
   auto one = [&](uint64_t p0) {
     uint32_t w0, w1, w2;
     philox_from_p0<KIND != 1>(P, mu, u, p0, w0, w1, w2);
@@ -417,7 +464,7 @@ __device__ __forceinline__ void generate_class(const KernelParams& P, const Book
   };
   uint64_t p0 = pl.p0;
 #pragma unroll kGenUnroll
-  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, p0_inc.inc, p0_inc.a_step); }
   if (pl.extra) one(p0);
 }
 
@@ -427,7 +474,7 @@ __device__ __forceinline__ void generate_class(const KernelParams& P, const Book
 template <int ATOM, bool MIX, int CLS, bool CLAMP>
 __device__ __forceinline__ void generate_class_packed(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                                       const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
-                                                      uint64_t p0_inc, int& sink) {
+                                                      const P0Step& p0_inc, int& sink) {
   auto one = [&](uint64_t p0) {
     uint32_t w[4];
     philox_block_from_p0(P, mu, u, p0, w);
@@ -438,7 +485,7 @@ __device__ __forceinline__ void generate_class_packed(const KernelParams& P, con
   };
   uint64_t p0 = pl.p0;
 #pragma unroll kGenUnroll
-  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, p0_inc.inc, p0_inc.a_step); }
   if (pl.extra) one(p0);
 }
 
@@ -465,7 +512,7 @@ __device__ __noinline__ void generate_partial_block_packed(const KernelParams& P
 template <int MODEL>
 struct GenPlan {
   ClassPlan cls[MODEL == 0 ? 1 : 3];
-  uint64_t p0_inc;       // M0 * a_step
+  P0Step p0_inc;         // a_step and M0 * a_step
 };
 
 // `count` = number of items the classes enumerate: agents (literal contract) or full blocks of four
@@ -474,24 +521,26 @@ template <int MODEL>
 __device__ __forceinline__ GenPlan<MODEL> gen_plan(uint32_t count, int tid, int T) {
   GenPlan<MODEL> g;
   if (MODEL == 0) {
-    g.p0_inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
+    g.p0_inc.a_step = (uint32_t)T;
+    g.p0_inc.inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
     g.cls[0] = class_plan((uint32_t)tid, (uint32_t)(T - 1), count, (uint32_t)T);
   } else {
     const uint32_t st = 3u * (uint32_t)T;
-    g.p0_inc = (uint64_t)kPhiloxM0 * st;
+    g.p0_inc.a_step = st;
+    g.p0_inc.inc = (uint64_t)kPhiloxM0 * st;
 #pragma unroll
     for (int c = 0; c < (MODEL == 0 ? 1 : 3); ++c)
       g.cls[c] = class_plan(3u * (uint32_t)tid + (uint32_t)c, 3u * (uint32_t)(T - 1) + (uint32_t)c, count, st);
   }
   // hide that p0_inc is a product: otherwise p0 += p0_inc is turned back into IMAD.WIDE(M0, a_step, p0)
-  asm volatile("" : "+l"(g.p0_inc));
+  asm volatile("" : "+l"(g.p0_inc.inc));
   return g;
 }
 
 template <int ATOM, int KIND>
 __device__ __forceinline__ void generate_class_paper(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                                      const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
-                                                     uint64_t p0_inc, uint32_t parity, int& sink) {
+                                                     const P0Step& p0_inc, uint32_t parity, int& sink) {
   auto one = [&](uint64_t p0) {
     uint32_t w[4];
     philox_block_from_p0(P, mu, u, p0, w);
@@ -499,7 +548,7 @@ __device__ __forceinline__ void generate_class_paper(const KernelParams& P, cons
   };
   uint64_t p0 = pl.p0;
 #pragma unroll kGenUnroll
-  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = add64_alu(p0, p0_inc); }
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, p0_inc.inc, p0_inc.a_step); }
   if (pl.extra) one(p0);
 }
 
@@ -507,11 +556,12 @@ __device__ __forceinline__ void generate_class_paper(const KernelParams& P, cons
 __device__ __forceinline__ GenPlan<2> gen_plan_paper(const KernelParams& P, int tid, int T) {
   GenPlan<2> g;
   const uint32_t e0 = (uint32_t)P.paper_n_noise, e1 = e0 + (uint32_t)P.paper_n_mom, e2 = (uint32_t)P.A;
-  g.p0_inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
+  g.p0_inc.a_step = (uint32_t)T;
+  g.p0_inc.inc = (uint64_t)kPhiloxM0 * (uint32_t)T;
   g.cls[0] = class_plan((uint32_t)tid, (uint32_t)(T - 1), e0, (uint32_t)T);
   g.cls[1] = class_plan(e0 + (uint32_t)tid, e0 + (uint32_t)(T - 1), e1, (uint32_t)T);
   g.cls[2] = class_plan(e1 + (uint32_t)tid, e1 + (uint32_t)(T - 1), e2, (uint32_t)T);
-  asm volatile("" : "+l"(g.p0_inc));
+  asm volatile("" : "+l"(g.p0_inc.inc));
   return g;
 }
 

@@ -61,11 +61,14 @@ __global__ void generate_only_kernel(const __grid_constant__ ks::KernelParams P,
 }
 
 // ---- (3) raw pipes ---------------------------------------------------------------------------
+// KIND 0: IMAD.WIDE (with accumulate); 1: LOP3; 2: one IMAD.WIDE + one dependent LOP3 (the Philox
+// round pattern); 3, 4: one IMAD.WIDE + two / three LOP3 -- how much every further alu-pipe
+// instruction costs the multiply stream.
 template <int KIND>
 __global__ void int_pipe_kernel(int iters, uint32_t seed, uint32_t* out) {
-  uint32_t c[8], d[8];
+  uint32_t c[8], d[8], e[8];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) { c[j] = seed + threadIdx.x * 8u + j; d[j] = c[j] ^ 0x9E3779B9u; }
+  for (int j = 0; j < 8; ++j) { c[j] = seed + threadIdx.x * 8u + j; d[j] = c[j] ^ 0x9E3779B9u; e[j] = d[j] * 3u; }
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -79,12 +82,19 @@ __global__ void int_pipe_kernel(int iters, uint32_t seed, uint32_t* out) {
           c[j] = c[j] ^ d[j] ^ seed;                                                       // LOP3
           if (KIND == 1) d[j] = d[j] ^ c[j] ^ 0x85EBCA6Bu;
         }
+        if (KIND >= 3) {
+          const uint64_t p = (uint64_t)ks::kPhiloxM0 * c[j];
+          const uint32_t hi = (uint32_t)(p >> 32), lo = (uint32_t)p;
+          c[j] = hi ^ d[j] ^ seed; d[j] = lo;                                              // LOP3 #1
+          e[j] = e[j] ^ lo ^ seed;                                                         // LOP3 #2
+          if (KIND == 4) e[j] = (e[j] & hi) ^ seed;                                        // LOP3 #3
+        }
       }
     }
   }
   uint32_t acc = 0;
 #pragma unroll
-  for (int j = 0; j < 8; ++j) acc ^= c[j] ^ d[j];
+  for (int j = 0; j < 8; ++j) acc ^= c[j] ^ d[j] ^ e[j];
   if (acc == 0x12345678u) out[0] = acc;
 }
 
@@ -191,7 +201,7 @@ ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L,
 
 ks_status ks_bench_int_pipe(int32_t kind, int32_t threads, int32_t ctas_per_sm, int32_t iters, int32_t warmup,
                             int32_t reps, void* stream, double* thread_ops_per_s, double* seconds) {
-  if (!thread_ops_per_s || !seconds || kind < 0 || kind > 2 || threads < 32 || threads > 1024 || threads % 32 ||
+  if (!thread_ops_per_s || !seconds || kind < 0 || kind > 4 || threads < 32 || threads > 1024 || threads % 32 ||
       ctas_per_sm < 1 || iters < 1 || reps < 1)
     return KS_ERR_INVALID_ARG;
   const int sms = num_sms();
@@ -203,12 +213,14 @@ ks_status ks_bench_int_pipe(int32_t kind, int32_t threads, int32_t ctas_per_sm, 
   auto launch = [&]() {
     if (kind == 0)      int_pipe_kernel<0><<<grid, threads, 0, st>>>(iters, 7u, d_out);
     else if (kind == 1) int_pipe_kernel<1><<<grid, threads, 0, st>>>(iters, 7u, d_out);
-    else                int_pipe_kernel<2><<<grid, threads, 0, st>>>(iters, 7u, d_out);
+    else if (kind == 2) int_pipe_kernel<2><<<grid, threads, 0, st>>>(iters, 7u, d_out);
+    else if (kind == 3) int_pipe_kernel<3><<<grid, threads, 0, st>>>(iters, 7u, d_out);
+    else                int_pipe_kernel<4><<<grid, threads, 0, st>>>(iters, 7u, d_out);
   };
   ks_status rc = time_best(launch, warmup, reps, st, seconds);
   cudaFree(d_out);
   if (rc != KS_OK) return rc;
-  const double per_iter = (kind == 2 ? 2.0 : (kind == 1 ? 2.0 : 1.0)) * 32.0;   // ops per thread per iteration
+  const double per_iter = (kind == 0 ? 1.0 : (kind <= 2 ? 2.0 : (kind == 3 ? 3.0 : 4.0))) * 32.0;   // ops per thread per iteration
   *thread_ops_per_s = (double)grid * threads * (double)iters * per_iter / *seconds;
   return KS_OK;
 }
