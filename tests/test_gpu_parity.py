@@ -337,6 +337,23 @@ def test_paper_agent_model_matches_the_oracle(ks, oracle, alpha_mom):
     sim.ks_destroy()
 
 
+def test_paper_agent_model_full_size_sampled_markets(ks, oracle):
+    """Model 4 in the C4 shape (M = 65536 markets, L = 512, A = 4096; S = 200 so that the oracle,
+    which scans the whole book for Eq.3 every step, stays in seconds) in the automatic launch plan:
+    64 seeded sampled markets against the oracle, conservation on every market."""
+    c = CONFIGS["C4"]
+    S = 200
+    p = paper_params(c.A, 0.15, 0.15, delta=32, qmax=100, half_spread=3, p_mkt=0.02)
+    b, r = _gpu(ks, c.M, c.L, c.A, p, c.seed, S)
+    ids = sampled_markets(c.M, c.seed, 64)
+    eb, er = oracle_rows(oracle, p, c.L, c.A, c.seed, ids, S)
+    assert_rows_equal(b, r, ids, eb, er, "model 4, C4 shape")
+    r64 = r.astype(np.int64)
+    tot = b.astype(np.int64).sum(axis=2)
+    assert (b >= 0).all() and (r64[:, 0] == S).all()
+    assert (r64[:, 10] == r64[:, 2] + tot[:, 0]).all() and (r64[:, 11] == r64[:, 2] + tot[:, 1]).all()
+
+
 # ------------------------------------------------------------------ book injection / edge cases
 def test_paper_worked_example_through_the_library(ks):
     """PAPER.md:315-354 (Eq.11-18) embedded at ticks 10..14 of an L=32 grid, A = 0: zero padding
