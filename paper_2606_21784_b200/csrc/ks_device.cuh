@@ -271,26 +271,23 @@ struct RuleCtx {
 };
 
 // a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; sell tick = (last - delta) + o, buy tick =
-// last - (o - delta) = (last - delta) + (n-1-o).  q = 1 + mulhi(w2, qmax) is the high word of
-// w2*qmax + 2^32: one IMAD.HI with the +1 folded into its 64-bit addend.
-// No-clamp path: the whole address comes out of ONE IMAD.HI, because the fma pipe that executes
-// the multiplies is the bound and every IMAD.IADD the compiler would emit for an address add
-// costs it two more cycles:
-//   sell:  hi(w1*4n + {hi: &ask[last-delta], lo: 0})       = &ask[last-delta] + 4o + r,  r in 0..3
-//   buy:   hi(~w1*4n + {hi: &bid[last-delta], lo: 4n-1})   = &bid[last-delta] + 4(n-1-o) + (3-r)
-// (floor(4y) = 4 floor(y) + r; and with w*4n = H*2^32 + Lo, (2^32-1-w)*4n + 4n-1 =
-// (4n-1-H)*2^32 + (2^32-1-Lo), so the high word is exactly 4n-1-H), then & ~3 drops r.
-// m = w0 >> 31 (arithmetic) is all-ones for a buy: x = w1 ^ m, addend = {ask_lo ^ (m & (ask_lo ^
-// bid_lo)), m & (4n-1)} -- alu-pipe instructions only.
+// last - (o - delta) = (last - delta) + (n-1-o) = (last - delta + n) + ~o.  q = 1 + mulhi(w2, qmax)
+// is the high word of w2*qmax + 2^32: one IMAD.HI with the +1 folded into its 64-bit addend.
+// No-clamp path: m = w0 >> 31 (arithmetic) is all-ones for a buy, and
+//   addr = base(m) + 4*(o ^ m),  base = &ask[last-delta] or &bid[last-delta+n]
+// -- SHF + 2 LOP3 + one shift-add beside the two multiplies.  The kernel is bound by the number of
+// math instructions it dispatches (~1 % of run time per instruction per event), so
+// the rule is written for the fewest instructions, whichever pipe runs them.
 template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                             uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
   const int q = (int)hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend);
   if (!CLAMP) {
     const uint32_t m = (uint32_t)((int32_t)w0 >> 31);
-    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ rc.bid_lo));
-    const uint64_t addend = ((uint64_t)base << 32) | (m & (uint32_t)(P.noise_n4 - 1));
-    const uint32_t addr = hi32((uint64_t)(w1 ^ m) * (uint32_t)P.noise_n4 + addend) & ~3u;
+    const uint32_t o = __umulhi(w1, (uint32_t)P.noise_n);
+    const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
+    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top));
+    const uint32_t addr = base + ((o ^ m) << 2);
     book_add_at<ATOM>(book, addr, q, sink);
   } else {
     const bool buy = (int32_t)w0 < 0;
@@ -322,33 +319,28 @@ __device__ __forceinline__ void momentum_order(const KernelParams& P, const Book
 
 // ---- PACKED4 rules (A22): every draw of an agent out of ONE word by successive
 // multiply-extract: o = hi(w*n), x1 = lo(w*n); q-1 = hi(x1*qmax), x2 = lo(x1*qmax); coin = x2>>31.
-// Two IMAD.WIDE per agent.
-// No-clamp noise path: the first multiply is by 4n, so that its high word is the byte offset:
-// w*4n = (4o + r)*2^32 + (x1 << 2 mod 2^32), r = top two bits of x1; x1 itself is the funnel shift
-// (hi:lo) >> 2 (one SHF).  m = coin mask (all-ones for a buy); sell tick = (last-delta) + o, buy
-// tick = (last-delta) + (n-1-o) = (last-delta+n) + ~o, and (4o + r) ^ m = 4*(~o) + (3-r) for a
-// buy, so off = ((4o + r) ^ m) & ~3 (one LOP3) and addr = &ask[last-delta] + (m & (&bid[last-
-// delta+n] - &ask[last-delta])) + off: a three-operand IADD3.  Everything but the two multiplies
-// runs on the alu pipe.
+// Two IMAD.WIDE per agent.  (ptxas splits a mad.wide.u32 with a 64-bit addend into multiply + two
+// adds when the multiplier is a uniform register, so the +1 of q is a plain add.)
+// No-clamp noise path: m = coin mask (all-ones for a buy); sell tick = (last-delta) + o, buy tick
+// = (last-delta) + (n-1-o) = (last-delta+n) + ~o, so addr = base(m) + 4*(o ^ m) with base =
+// &ask[last-delta] or &bid[last-delta+n]: SHF + 2 LOP3 + one shift-add -- four instructions
+// beside the two multiplies; what bounds the kernel is the number of math instructions dispatched
+// (DESIGN.md 7.2), so the count is what matters, not which pipe runs them.
 template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order_packed(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                                    uint32_t w, int& sink) {
+  const uint64_t p1 = mul_wide_u32(w, (uint32_t)P.noise_n);
+  const uint64_t p2 = mul_wide_u32(lo32(p1), (uint32_t)P.noise_qmax);
+  const int q = (int)hi32(p2) + 1;
+  const uint32_t o = hi32(p1);
   if (!CLAMP) {
-    const uint64_t p1 = mul_wide_u32(w, (uint32_t)P.noise_n4);
-    const uint32_t x1 = __funnelshift_r(lo32(p1), hi32(p1), 2);
-    const uint64_t p2 = mul_wide_u32(x1, (uint32_t)P.noise_qmax);
-    const int q = (int)hi32(p2) + 1;
     const uint32_t m = (uint32_t)((int32_t)lo32(p2) >> 31);
-    const uint32_t off = (hi32(p1) ^ m) & ~3u;
-    const uint32_t side_off = m & (rc.bid_lo + (uint32_t)P.noise_n4 - rc.ask_lo);
-    book_add_at<ATOM>(book, rc.ask_lo + side_off + off, q, sink);
+    const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
+    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top));
+    book_add_at<ATOM>(book, base + ((o ^ m) << 2), q, sink);
   } else {
-    const uint64_t p1 = mul_wide_u32(w, (uint32_t)P.noise_n);
-    const uint64_t p2 = mul_wide_u32(lo32(p1), (uint32_t)P.noise_qmax);
-    const int q = (int)hi32(p2) + 1;
-    const int o = (int)hi32(p1);
     const bool buy = (int32_t)lo32(p2) < 0;
-    const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - o : (rc.last - P.noise_delta) + o, rc.L);
+    const int tick = clamp_tick(buy ? (rc.last + P.noise_delta) - (int)o : (rc.last - P.noise_delta) + (int)o, rc.L);
     book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
   }
 }
