@@ -160,6 +160,7 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
     } else {
       rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
       rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
+      rc.bid_last = rc.bid_lo + 4u * (uint32_t)P.noise_delta; rc.ask_last = rc.ask_lo + 4u * (uint32_t)P.noise_delta;
       // a1 + a2: order generation and aggregation
       generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
     }
