@@ -209,6 +209,9 @@ typedef enum {
   KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 64..1024, multiple of 32          */
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
   KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
+  KS_OPT_PIPELINE = 4,      /* software pipeline for few markets (the next step's draws overlap the clearing):
+                               0 = automatic, 1 = never, 2 = whenever legal (zero-intelligence model, plain
+                               atomics, >= 64 threads, at most 4 agents per generating thread)               */
   KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
                                i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
                                book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and

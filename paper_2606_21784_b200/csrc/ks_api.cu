@@ -46,7 +46,7 @@ struct ks_sim {
   int64_t steps_done;
   int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster;
+  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
   // ks_write_books depth check
@@ -121,7 +121,7 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   if (!s) { set_err("ks_create: out of host memory"); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
   s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0;
   s->dev_smem_optin = optin; s->num_sms = sms;
   s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_PAPER) {
@@ -187,6 +187,9 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_CLEAR_PATH:
       if (value != 0 && value != 1) break;
       s->opt_clear = value; return KS_OK;
+    case KS_OPT_PIPELINE:
+      if (value != 0 && value != 1 && value != 2) break;
+      s->opt_pipe = value; return KS_OK;
     case KS_OPT_CLUSTER_SIZE:
       if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break;
       if (value > 1 && (s->L / value < 32 || s->opt_atomic || s->p.model == KS_MODEL_PAPER)) break;
@@ -235,9 +238,9 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   return pl;
 }
 
-template <int MODEL, int ATOM, bool PACKED>
+template <int MODEL, int ATOM, bool PACKED, bool PIPE = false>
 static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_persistent_kernel<MODEL, ATOM, PACKED>;
+  auto kern = ks::ks_persistent_kernel<MODEL, ATOM, PACKED, PIPE>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -332,8 +335,24 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     if (!packed) e = mix ? launch_cluster<1, false>(P, C, T, st) : launch_cluster<0, false>(P, C, T, st);
     else         e = mix ? launch_cluster<1, true>(P, C, T, st) : launch_cluster<0, true>(P, C, T, st);
   } else {
-    const LaunchPlan pl = plan_launch(s);
-    if (paper)
+    // software pipeline (kernel template PIPE): legal for the literal zero-intelligence contract
+    // with plain atomics when every generating thread (warps >= 1) holds at most kPipeEvents events;
+    // automatic when the grid leaves the GPU underfilled, i.e. the step latency is what counts (C3).
+    // Block size for it: the smallest power of two whose generating threads hold <= 3 events each
+    // (measured on C3: T = 256 -> 7.4 ms, T = 512 -> 8.0 ms, unpipelined 8.9 ms).
+    LaunchPlan pl = plan_launch(s);
+    const bool pipe_model = !paper && !mix && !packed && !s->opt_atomic;
+    const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
+    if (pipe_model && !s->opt_threads && s->opt_pipe != 1 && (s->opt_pipe == 2 || underfilled)) {
+      int Tp = 64;
+      while (Tp < 1024 && (long long)(Tp - 32) * 3 < s->A) Tp *= 2;
+      if ((long long)(Tp - 32) * ks::kPipeEvents >= s->A) pl.T = Tp;
+    }
+    const bool pipe_legal = pipe_model && pl.T >= 64 && (long long)(pl.T - 32) * ks::kPipeEvents >= s->A;
+    const bool pipe = pipe_legal && s->opt_pipe != 1 && (s->opt_pipe == 2 || underfilled);
+    if (pipe)
+      e = launch_persistent<0, 0, false, true>(P, pl.T, pl.smem, st);
+    else if (paper)
       e = launch_persistent<2, 0, false>(P, pl.T, pl.smem, st);
     else if (packed)
       e = mix ? launch_persistent<1, 0, true>(P, pl.T, pl.smem, st) : launch_persistent<0, 0, true>(P, pl.T, pl.smem, st);

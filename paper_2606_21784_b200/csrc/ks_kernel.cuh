@@ -68,6 +68,8 @@ __device__ __forceinline__ GenPlan<2> make_gen_plan<2>(const KernelParams& P, bo
   return gen_plan_paper(P, tid, T);
 }
 
+constexpr int kPipeEvents = 4;     // PIPE kernels: events per generating thread held in registers
+
 __device__ __forceinline__ int sign_of(int x) { return (x > 0) - (x < 0); }
 
 // ---------------------------------------------------------------------------------------------
@@ -75,8 +77,13 @@ __device__ __forceinline__ int sign_of(int x) { return (x > 0) - (x < 0); }
 // dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3, 2 = the paper's agent
 // model (mid-price reference, A24).  ATOM: see book_add.
 // PACKED: the PACKED4 draw contract (one Philox block per four agents, A22).
+// PIPE (MODEL 0, ATOM 0, literal contract, few markets): software pipeline for the latency-bound
+// regime (C3).  The Philox words of a step do not depend on the price, only the address does: warp 0
+// holds no agents and only clears; while it clears step s, the other warps draw (offset, side,
+// quantity) of step s+1 into registers (at most 4 events per thread), and after the barrier they
+// only compute addresses and issue the atomics.  Same orders, same bytes.
 // ---------------------------------------------------------------------------------------------
-template <int MODEL, int ATOM, bool PACKED>
+template <int MODEL, int ATOM, bool PACKED, bool PIPE = false>
 __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
   __shared__ long long s_rec[16];
@@ -94,7 +101,8 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   long long* grec = P.recs + (size_t)blockIdx.x * 16;
   const MarketUniform mu = market_uniform(P, market);
 
-  const GenPlan<MODEL> gplan = make_gen_plan<MODEL>(P, PACKED, tid, T);
+  const GenPlan<MODEL> gplan = PIPE ? gen_plan<MODEL>(warp > 0 ? (uint32_t)P.A : 0u, tid >= 32 ? tid - 32 : 0, T - 32)
+                                    : make_gen_plan<MODEL>(P, PACKED, tid, T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
 
   // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
@@ -146,69 +154,122 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
     else publish(last);
   }
   __syncthreads();
-  // ---- S steps, all on-chip
-  for (long long s = 0; s < P.S; ++s) {
-    const uint32_t t = t0 + (uint32_t)s;
-    const StepUniform u = step_uniform(P, mu, t);
-    const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
-    last = ctl.x;
-    RuleCtx rc;
-    rc.last = last; rc.L = L;
-    if constexpr (MODEL == 2) {
-      rc.mid2 = ctl.y; rc.dp = ctl.z; rc.noclamp = false; rc.bid_lo = 0; rc.ask_lo = 0; rc.mkt_flags = s_mkt;
-      generate_step_paper<ATOM>(P, bref, mu, u, rc, gplan, tid, t, sink);
+  // a3-a6: clearing by warp 0 on the active window (called by warp 0 only)
+  auto clear_step = [&](long long s, const RuleCtx& rc) {
+    int lo, hi;
+    if (MODEL == 2) {
+      lo = max(0, min(amin, (rc.mid2 >> 1) - P.dmax));
+      hi = min(L - 1, max(bmax, ((rc.mid2 + 1) >> 1) + P.dmax));
+      if (s_mkt[0]) hi = L - 1;                      // marketable buys sit at tick L-1,
+      if (s_mkt[1]) lo = 0;                          // marketable sells at tick 0
+      __syncwarp();
     } else {
-      rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
-      rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
-      rc.bid_last = rc.bid_lo + 4u * (uint32_t)P.noise_delta; rc.ask_last = rc.ask_lo + 4u * (uint32_t)P.noise_delta;
-      // a1 + a2: order generation and aggregation
-      generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+      lo = max(0, min(amin, last - P.dmax));
+      hi = min(L - 1, max(bmax, last + P.dmax));
     }
-    __syncthreads();                                   // B1: the combined book is complete
-
-    // a3-a6: clearing by warp 0 on the active window
-    if (warp == 0) {
-      int lo, hi;
+    int vmax, pstar, nb, na, base, wend;
+    int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
+    const LocalBook io{book, L};
+    if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, nb, na); }
+    else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, nb, na); }
+    else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, nb, na); }
+    else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, nb, na); }
+    if (MODEL == 2) {
+      // the mid price needs the EXACT best quotes: a side with no depth inside the window is
+      // searched outside it (rare: the window was emptied on that side)
+      if (nb < base) nb = best_bid_below(io, L, base, lane);
+      if (na >= wend) na = best_ask_from(io, L, wend, lane);
+    }
+    bmax = nb; amin = na;
+    if (lane == 0) {
+      int new_last;
+      update_record(s_rec, last, vmax, pstar, new_last);
       if (MODEL == 2) {
-        lo = max(0, min(amin, (rc.mid2 >> 1) - P.dmax));
-        hi = min(L - 1, max(bmax, ((rc.mid2 + 1) >> 1) + P.dmax));
-        if (s_mkt[0]) hi = L - 1;                      // marketable buys sit at tick L-1,
-        if (s_mkt[1]) lo = 0;                          // marketable sells at tick 0
-        __syncwarp();
+        s_rec[F_PREV] = rc.mid2;
+        publish_paper(new_last, nb, na, rc.mid2);
+        s_mkt[0] = 0; s_mkt[1] = 0;
       } else {
-        lo = max(0, min(amin, last - P.dmax));
-        hi = min(L - 1, max(bmax, last + P.dmax));
+        publish(new_last);
       }
-      int vmax, pstar, nb, na, base, wend;
-      int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
-      const LocalBook io{book, L};
-      if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, nb, na); }
-      else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, nb, na); }
-      else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, nb, na); }
-      else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, nb, na); }
-      if (MODEL == 2) {
-        // the mid price needs the EXACT best quotes: a side with no depth inside the window is
-        // searched outside it (rare: the window was emptied on that side)
-        if (nb < base) nb = best_bid_below(io, L, base, lane);
-        if (na >= wend) na = best_ask_from(io, L, wend, lane);
-      }
-      bmax = nb; amin = na;
-      if (lane == 0) {
-        int new_last;
-        update_record(s_rec, last, vmax, pstar, new_last);
-        if (MODEL == 2) {
-          s_rec[F_PREV] = rc.mid2;
-          publish_paper(new_last, nb, na, rc.mid2);
-          s_mkt[0] = 0; s_mkt[1] = 0;
-        } else {
-          publish(new_last);
+    }
+    if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)P.S, s, P.S, lane,
+                            vmax > 0 ? pstar : last, vmax);
+  };
+  // ---- S steps, all on-chip
+  if constexpr (PIPE) {
+    // per-thread draws of ONE step: the offset index o = mulhi(w1, n), and q with the side bit of
+    // w0 in its top bit (q <= 2^20 + 1).  At most kPipeEvents events per thread (host plan).
+    uint32_t dr_o[kPipeEvents], dr_q[kPipeEvents];
+    const int n_mine = (int)gplan.cls[0].n_uniform + (gplan.cls[0].extra ? 1 : 0);
+    auto draw = [&](uint32_t t) {
+      const StepUniform u = step_uniform(P, mu, t);
+      uint64_t p0 = gplan.cls[0].p0;
+#pragma unroll
+      for (int e = 0; e < kPipeEvents; ++e) {
+        if (e < n_mine) {
+          uint32_t w0, w1, w2;
+          philox_from_p0<true>(P, mu, u, p0, w0, w1, w2);
+          dr_o[e] = __umulhi(w1, (uint32_t)P.noise_n);
+          dr_q[e] = hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend) | (w0 & 0x80000000u);
+          p0 = add64_alu(p0, gplan.p0_inc.inc);
         }
       }
-      if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)P.S, s, P.S, lane,
-                              vmax > 0 ? pstar : last, vmax);
+    };
+    if (P.S > 0) draw(t0);
+    for (long long s = 0; s < P.S; ++s) {
+      const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
+      last = ctl.x;
+      RuleCtx rc;
+      rc.last = last; rc.L = L; rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
+      rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
+      rc.bid_last = 0; rc.ask_last = 0;
+      // a2: the orders drawn during the previous clearing go to their ticks
+#pragma unroll
+      for (int e = 0; e < kPipeEvents; ++e) {
+        if (e < n_mine) {
+          const uint32_t m = (uint32_t)((int32_t)dr_q[e] >> 31), o = dr_o[e];
+          const int q = (int)(dr_q[e] & 0x7fffffffu);
+          if (rc.noclamp) {
+            const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
+            book_add_at<ATOM>(bref, (rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top))) + ((o ^ m) << 2), q, sink);
+          } else {
+            const bool buy = m != 0u;
+            const int tick = clamp_tick(buy ? (last + P.noise_delta) - (int)o : (last - P.noise_delta) + (int)o, L);
+            book_add<ATOM>(bref, 4u * (uint32_t)(buy ? tick : tick + L), q, sink);
+          }
+        }
+      }
+      __syncthreads();                                   // B1: the combined book is complete
+      if (warp == 0) clear_step(s, rc);                  // a3-a6 ...
+      else if (s + 1 < P.S) draw(t0 + (uint32_t)s + 1u); // ... while the other warps draw the next step (a1)
+      __syncthreads();                                   // B2: residual book and new price visible
+      prev = last;
     }
-    __syncthreads();                                   // B2: residual book and new price visible
-    prev = last;
+  } else {
+    for (long long s = 0; s < P.S; ++s) {
+      const uint32_t t = t0 + (uint32_t)s;
+      const StepUniform u = step_uniform(P, mu, t);
+      const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
+      last = ctl.x;
+      RuleCtx rc;
+      rc.last = last; rc.L = L;
+      if constexpr (MODEL == 2) {
+        rc.mid2 = ctl.y; rc.dp = ctl.z; rc.noclamp = false; rc.bid_lo = 0; rc.ask_lo = 0; rc.mkt_flags = s_mkt;
+        generate_step_paper<ATOM>(P, bref, mu, u, rc, gplan, tid, t, sink);
+      } else {
+        rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
+        rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
+        rc.bid_last = rc.bid_lo + 4u * (uint32_t)P.noise_delta; rc.ask_last = rc.ask_lo + 4u * (uint32_t)P.noise_delta;
+        // a1 + a2: order generation and aggregation
+        generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+      }
+      __syncthreads();                                   // B1: the combined book is complete
+
+      if (warp == 0) clear_step(s, rc);
+      __syncthreads();                                   // B2: residual book and new price visible
+      prev = last;
+    }
+
   }
 
   // ---- a7: write-back (shared -> HBM), 16-byte vectors, plus the totals for sub_buy/sub_sell

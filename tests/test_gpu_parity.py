@@ -95,6 +95,35 @@ def test_block_sizes_atomic_modes_and_clear_paths_give_identical_bytes(ks, oracl
                 assert_rows_equal(b, r, ids, eb, er, "T=%d atom=%d clear=%d" % (T, atom, clear))
 
 
+def test_pipelined_step_loop_gives_identical_bytes(ks, oracle):
+    """KS_OPT_PIPELINE: the next step's Philox draws overlap the clearing (warp 0 holds no agents).
+    Forced on (2) and off (1) for several block sizes and ragged agent counts, prices pinned to the
+    grid edges (clamp path), split and launch-per-step runs, the trace: always the oracle's bytes."""
+    import torch
+    L, seed, S = 128, 2, 150
+    p = zi_params(8, 10)
+    for M, A, T in [(5, 512, 512), (5, 500, 256), (3, 97, 64), (4, 33, 96), (2, 0, 128), (3, 1900, 512), (2, 1984, 1024)]:
+        ids = np.arange(M)
+        eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+        for pipe in (2, 1):
+            b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, pipe)])
+            assert_rows_equal(b, r, ids, eb, er, "pipeline=%d A=%d T=%d" % (pipe, A, T))
+    M, A, T = 4, 480, 256
+    ids = np.arange(M)
+    for init in (0, L - 1, 4):
+        q = dict(p, init_price=init)
+        eb, er, et = oracle.run_markets_traced(q, L, A, seed, ids, 60)
+        for kw in (dict(), dict(split=[1, 29, 30]), dict(stepwise=True)):
+            b, r = _gpu(ks, M, L, A, q, seed, 60, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, 2)], **kw)
+            assert_rows_equal(b, r, ids, eb, er, "pipeline init=%d %r" % (init, kw))
+        sim = ks.KsSim(M, L, A, q, seed)
+        sim.ks_set_option(ks.KS_OPT_BLOCK_THREADS, T); sim.ks_set_option(ks.KS_OPT_PIPELINE, 2)
+        tr = torch.empty((M, 60, 2), dtype=torch.int32, device="cuda")
+        sim.ks_run_traced(60, tr)
+        assert np.array_equal(tr.cpu().numpy(), et)
+        sim.ks_destroy()
+
+
 def test_split_run_and_stepwise_ablation_are_bit_identical(ks, oracle):
     """ks_run(S1); ks_run(S2) == ks_run(S1+S2); the launch-per-step ablation (a8) == persistent."""
     c = CONFIGS["C3"]
