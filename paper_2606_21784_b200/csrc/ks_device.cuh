@@ -276,23 +276,22 @@ struct RuleCtx {
 };
 
 // a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; sell tick = (last - delta) + o, buy tick =
-// last - (o - delta) = (last - delta) + (n-1-o) = (last - delta + n) + ~o.  q = 1 + mulhi(w2, qmax)
-// is the high word of w2*qmax + 2^32: one IMAD.HI with the +1 folded into its 64-bit addend.
-// No-clamp path: m = w0 >> 31 (arithmetic) is all-ones for a buy, and
-//   addr = base(m) + 4*(o ^ m),  base = &ask[last-delta] or &bid[last-delta+n]
-// -- SHF + 2 LOP3 + one shift-add beside the two multiplies.  The kernel is bound by the number of
-// math instructions it dispatches (~1 % of run time per instruction per event), so
-// the rule is written for the fewest instructions, whichever pipe runs them.
+// last - (o - delta) = (last + delta) - o.  q = 1 + mulhi(w2, qmax) is the high word of
+// w2*qmax + 2^32: one IMAD.HI with the +1 folded into its 64-bit addend.
+// No-clamp path: addr = buy ? &bid[last+delta] - 4*o : &ask[last-delta] + 4*o, which compiles to
+// ISETP + IMAD(o, -4, bid_hi) + @P IMAD(o, 4, ask_lo).  The kernel is bound by the number of math
+// instructions it dispatches (~1 % of run time per instruction per event), so the
+// rule is written for the fewest instructions, whichever pipe runs them (mask-and-xor forms of
+// the same address need four or five).
 template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                             uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
   const int q = (int)hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend);
   if (!CLAMP) {
-    const uint32_t m = (uint32_t)((int32_t)w0 >> 31);
+    // three instructions: one compare and two multiply-adds of which one is predicated off
     const uint32_t o = __umulhi(w1, (uint32_t)P.noise_n);
-    const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
-    const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top));
-    const uint32_t addr = base + ((o ^ m) << 2);
+    const uint32_t bid_hi = rc.bid_lo + (uint32_t)P.noise_n4 - 4u;            // &bid[last + delta]
+    const uint32_t addr = (int32_t)w0 < 0 ? bid_hi - (o << 2) : rc.ask_lo + (o << 2);
     book_add_at<ATOM>(book, addr, q, sink);
   } else {
     const bool buy = (int32_t)w0 < 0;
@@ -340,9 +339,9 @@ __device__ __forceinline__ void momentum_order(const KernelParams& P, const Book
 // adds when the multiplier is a uniform register, so the +1 of q is a plain add.)
 // No-clamp noise path: m = coin mask (all-ones for a buy); sell tick = (last-delta) + o, buy tick
 // = (last-delta) + (n-1-o) = (last-delta+n) + ~o, so addr = base(m) + 4*(o ^ m) with base =
-// &ask[last-delta] or &bid[last-delta+n]: SHF + 2 LOP3 + one shift-add -- four instructions
-// beside the two multiplies; what bounds the kernel is the number of math instructions dispatched
-// (DESIGN.md 7.2), so the count is what matters, not which pipe runs them.
+// &ask[last-delta] or &bid[last-delta+n]: SHF + 2 LOP3 + one shift-add.  (The compare-and-
+// predicate form that wins in the literal rule measures 8 % SLOWER here: the predicate comes
+// out of the second multiply, at the end of the dependency chain.)
 template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order_packed(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                                    uint32_t w, int& sink) {
