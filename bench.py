@@ -448,7 +448,7 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 26604288 + 239055616,            # profiles/r1g_persistent_full.md
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 25261312 + 237688320,            # profiles/r1h_persistent_full.md
                                   "C4_packed4": 23691008 + 254493952}    # profiles/r1g_packed_persistent_full.md
 
 if __name__ == "__main__":
