@@ -387,29 +387,45 @@ __device__ __forceinline__ void packed_agent(const KernelParams& P, const BookRe
 // 1 momentum, 2 maker.  `parity` = (a + t) & 1 of this thread's agents (T is even, so it is the
 // same for all of them).  Marketable orders go to the grid boundary and raise a flag so that the
 // clearing warp widens its window to that boundary.
-template <int ATOM, int KIND>
+template <int ATOM, int KIND, bool CLAMP>
 __device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                             const uint32_t (&w)[4], uint32_t parity, int& sink) {
-  bool buy; int p2, q;
-  if (KIND == 0) {
-    buy = (int32_t)w[0] < 0;
-    p2 = rc.mid2 + 2 * ((int)__umulhi(w[1], (uint32_t)P.noise_n) - P.noise_delta);
-    q = 1 + (int)__umulhi(w[2], (uint32_t)P.noise_qmax);
-  } else if (KIND == 1) {
-    buy = rc.dp > 0 ? true : (rc.dp < 0 ? false : ((int32_t)w[0] < 0));
-    p2 = rc.mid2 + (buy ? 2 : -2);
-    q = 1 + (int)__umulhi(w[2], (uint32_t)P.mom_qmax);
+  const uint32_t qmax = KIND == 0 ? (uint32_t)P.noise_qmax : (KIND == 1 ? (uint32_t)P.mom_qmax : (uint32_t)P.maker_qty);
+  const int q = (int)hi32((uint64_t)w[2] * qmax + P.q_addend);
+  const bool buy = KIND == 0 ? (int32_t)w[0] < 0
+                 : KIND == 1 ? (rc.dp > 0 ? true : (rc.dp < 0 ? false : ((int32_t)w[0] < 0)))
+                             : parity == 0u;
+  const bool mkt = KIND != 2 && (int)(w[3] >> 16) < P.paper_pmkt_q16;
+  if (!CLAMP) {
+    // round(mid + k) = midr + k for an integer k, midr = (mid2 + 1) >> 1 (2k is even), and no
+    // price can leave the grid: rc.bid_lo / rc.ask_lo are &bid / &ask[midr - delta], rc.bid_last /
+    // rc.ask_last are &bid / &ask[midr]
+    uint32_t addr;
+    if (KIND == 0) {
+      const uint32_t o4 = __umulhi(w[1], (uint32_t)P.noise_n) << 2;
+      addr = buy ? rc.bid_lo + o4 : rc.ask_lo + o4;
+    } else if (KIND == 1) {
+      addr = buy ? rc.bid_last + 4u : rc.ask_last - 4u;
+    } else {
+      addr = buy ? rc.bid_last - 4u * (uint32_t)P.maker_spread_max : rc.ask_last + 4u * (uint32_t)P.maker_spread_max;
+    }
+    if (mkt) {
+      addr = buy ? book.saddr + 4u * (uint32_t)(rc.L - 1) : book.saddr + 4u * (uint32_t)rc.L;   // bid[L-1] / ask[0]
+      rc.mkt_flags[buy ? 0 : 1] = 1;
+    }
+    book_add_at<ATOM>(book, addr, q, sink);
   } else {
-    buy = parity == 0u;
-    p2 = rc.mid2 + (buy ? -2 : 2) * P.maker_spread_max;
-    q = 1 + (int)__umulhi(w[2], (uint32_t)P.maker_qty);
+    int p2;
+    if (KIND == 0)      p2 = rc.mid2 + 2 * ((int)__umulhi(w[1], (uint32_t)P.noise_n) - P.noise_delta);
+    else if (KIND == 1) p2 = rc.mid2 + (buy ? 2 : -2);
+    else                p2 = rc.mid2 + (buy ? -2 : 2) * P.maker_spread_max;
+    int tick = clamp_tick((p2 + 1) >> 1, rc.L);
+    if (mkt) {
+      tick = buy ? rc.L - 1 : 0;
+      rc.mkt_flags[buy ? 0 : 1] = 1;
+    }
+    book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
   }
-  int tick = clamp_tick((p2 + 1) >> 1, rc.L);
-  if (KIND != 2 && (int)(w[3] >> 16) < P.paper_pmkt_q16) {
-    tick = buy ? rc.L - 1 : 0;
-    rc.mkt_flags[buy ? 0 : 1] = 1;
-  }
-  book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
 }
 
 // The agents of one class that a thread visits: first, first + a_step, ... < a_end.  p0 = M0*first;
@@ -545,14 +561,14 @@ __device__ __forceinline__ GenPlan<MODEL> gen_plan(uint32_t count, int tid, int 
   return g;
 }
 
-template <int ATOM, int KIND>
+template <int ATOM, int KIND, bool CLAMP>
 __device__ __forceinline__ void generate_class_paper(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                                      const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
                                                      const P0Step& p0_inc, uint32_t parity, int& sink) {
   auto one = [&](uint64_t p0) {
     uint32_t w[4];
     philox_block_from_p0(P, mu, u, p0, w);
-    paper_order<ATOM, KIND>(P, book, rc, w, parity, sink);
+    paper_order<ATOM, KIND, CLAMP>(P, book, rc, w, parity, sink);
   };
   uint64_t p0 = pl.p0;
 #pragma unroll kGenUnroll
@@ -578,9 +594,16 @@ __device__ __forceinline__ void generate_step_paper(const KernelParams& P, const
                                                     const StepUniform& u, const RuleCtx& rc, const GenPlan<2>& g,
                                                     int tid, uint32_t t, int& sink) {
   const uint32_t maker_first = (uint32_t)P.paper_n_noise + (uint32_t)P.paper_n_mom + (uint32_t)tid;
-  generate_class_paper<ATOM, 0>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, sink);
-  generate_class_paper<ATOM, 1>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, sink);
-  generate_class_paper<ATOM, 2>(P, book, mu, u, rc, g.cls[2], g.p0_inc, (maker_first + t) & 1u, sink);
+  const uint32_t par = (maker_first + t) & 1u;
+  if (rc.noclamp) {
+    generate_class_paper<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, sink);
+    generate_class_paper<ATOM, 1, false>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, sink);
+    generate_class_paper<ATOM, 2, false>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, sink);
+  } else {
+    generate_class_paper<ATOM, 0, true>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, sink);
+    generate_class_paper<ATOM, 1, true>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, sink);
+    generate_class_paper<ATOM, 2, true>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, sink);
+  }
 }
 
 // The highest tick < `from` with bid depth (-1 if none) / the lowest tick >= `from` with ask depth

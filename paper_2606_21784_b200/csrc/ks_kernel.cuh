@@ -254,7 +254,13 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
       RuleCtx rc;
       rc.last = last; rc.L = L;
       if constexpr (MODEL == 2) {
-        rc.mid2 = ctl.y; rc.dp = ctl.z; rc.noclamp = false; rc.bid_lo = 0; rc.ask_lo = 0; rc.mkt_flags = s_mkt;
+        rc.mid2 = ctl.y; rc.dp = ctl.z; rc.mkt_flags = s_mkt;
+      {                                                // no-clamp path: midr +- dmax inside the grid
+        const int midr = (rc.mid2 + 1) >> 1;
+        rc.noclamp = midr - P.dmax >= 0 && midr + P.dmax <= L - 1;
+        rc.bid_last = bref.saddr + 4u * (uint32_t)midr; rc.ask_last = rc.bid_last + 4u * (uint32_t)L;
+        rc.bid_lo = rc.bid_last - 4u * (uint32_t)P.noise_delta; rc.ask_lo = rc.ask_last - 4u * (uint32_t)P.noise_delta;
+      }
         generate_step_paper<ATOM>(P, bref, mu, u, rc, gplan, tid, t, sink);
       } else {
         rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
