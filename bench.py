@@ -300,6 +300,10 @@ def main():
                 "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name if args.rng == "literal" else cfg.name + "_packed4"),
                 "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "avg_launch_ms": avg_kern_s * 1e3,
                 "executed_mults_per_event": EXEC_MULTS_PER_EVENT[model], "fmaheavy_pipe_frac_from_executed": executed / peak,
+                "frac_note": "achieved counts the ALGORITHMIC multiplies (SURVEY.md S8(d)); the kernel executes fewer "
+                             "(hoisted / strength-reduced rounds, w3 skipped), so frac can reach or pass 1.0 -- the pipe's own "
+                             "utilisation is fmaheavy_pipe_frac_from_executed (ncu: 95.8 % with the address multiply-adds, "
+                             "profiles/r1h_persistent_full.md)",
                 "peak_source": "derived (DESIGN.md 7.2): %d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
                                % (sms, sm_max_mhz, "MEASURED_PEAKS.json sm_max_mhz" if peaks else "NVML max clock"),
                 "hbm": {"algorithmic_bytes": M * (8 * L + 128), "achieved_GBps": M * (8 * L + 128) / avg_kern_s / 1e9,
