@@ -35,8 +35,13 @@
  * best-bid/best-ask matching, closed forms, per-step invariants, a numpy return
  * series for the derived statistics; for the PACKED4 draw contract (models 2, 3) the
  * first four orders by hand from KAT #1 and the exact mixed-radix identity
- * (tests/test_oracle_packed.py).  Parity unpinned: the paper's own aggregate
- * numbers (Table II, Fig.7) -- its agent parameters and its RNG hash are not given.
+ * (tests/test_oracle_packed.py); for model 4 (ko_gen_orders_paper) one hand-derived
+ * order per class and branch from KAT #1 -- noise, momentum rising / falling / flat,
+ * integer and half-tick mids, marketable both ways, maker -- and the momentum rule seen
+ * through the run loop on a book whose mid differs from the last price
+ * (tests/golden/paper_model_first_order.txt, tests/test_oracle_paper_model.py).
+ * Parity unpinned: the paper's own aggregate numbers (Table II, Fig.7) -- its agent
+ * parameters and its RNG hash are not given.
  */
 #include <stdint.h>
 #include <stddef.h>

@@ -14,12 +14,52 @@ REC = {n: i for i, n in enumerate(
 
 
 def test_first_order_by_hand_from_kat1(oracle):
-    """tests/golden/paper_model_first_order.txt: agent 0, step 0, market 0, seed 0 -> Philox KAT #1."""
+    """tests/golden/paper_model_first_order.txt: agent 0, step 0, market 0, seed 0 -> Philox KAT #1.
+    One record per class: noise (half-tick / integer mid, marketable), momentum (rising, falling,
+    flat -> coin, half-tick mids, marketable both ways, the threshold itself), maker (never marketable)."""
+    seen = set()
     for g in read_golden("paper_model_first_order.txt"):
-        p = paper_params(100, 0.0, 0.0, delta=int(g["delta"][0]), qmax=int(g["qmax"][0]), p_mkt=0.0)
+        cls = g.get("class", ["noise"])[0]
+        seen.add(cls)
+        A = 100
+        p = paper_params(A, 1.0 if cls == "momentum" else 0.0, 1.0 if cls == "maker" else 0.0,
+                         delta=int(g["delta"][0]), qmax=int(g["qmax"][0]), half_spread=3, p_mkt=0.0)
         p["paper_pmkt_q16"] = int(g["pmkt_q16"][0])
-        got = oracle.gen_orders_paper(p, int(g["L"][0]), int(g["mid2"][0]), int(g["mid2"][0]), 0, 0, 0, 0, 100)
+        mid2 = int(g["mid2"][0])
+        prev2 = int(g.get("prev2", g["mid2"])[0])
+        got = oracle.gen_orders_paper(p, int(g["L"][0]), mid2, prev2, 0, 0, 0, 0, A)
         assert got == (0 if g["order"][0] == "B" else 1, int(g["order"][1]), int(g["order"][2])), g["name"]
+    assert seen == {"noise", "momentum", "maker"}
+
+
+def test_momentum_follows_the_mid_not_the_last_price(oracle):
+    """PAPER.md:139 through the run loop: ret_t = sgn(mid_t - mid_{t-1}) with mid from Eq.3 on the
+    RESTING book, p = round(mid + side).  A momentum-only population on an injected book whose mid
+    (12.5) is far from the last price (30 resp. 5): every order of the step lands on ONE tick, and
+    that tick is round(mid -/+ 1), not last -/+ 1.  Worked by hand:
+      market 0: last 30 -> f[13] = 60 (doubled opening mid); bb 10, ba 15 -> mid2 25 < 60 -> all SELL
+                at round(12.5 - 1) = round(11.5) = 12; best bid 10 < 12: no trade
+      market 1: last 5  -> f[13] = 10; mid2 25 > 10 -> all BUY at round(12.5 + 1) = round(13.5) = 14;
+                best ask 15 > 14: no trade"""
+    L, A = 64, 50
+    p = paper_params(A, 1.0, 0.0, qmax=5, p_mkt=0.0)
+    for init, side, tick in ((30, 1, 12), (5, 0, 14)):
+        books = np.zeros((1, 2, L), dtype=np.int32)
+        books[0, 0, 10] = 7; books[0, 0, 4] = 9; books[0, 1, 15] = 3; books[0, 1, 40] = 1
+        _, recs = oracle.init_state(1, L, init, model=4)
+        assert recs[0, REC["prev"]] == 2 * init
+        b, r = oracle.run_markets(dict(p, init_price=init), L, A, 3, [0], 1, books, recs)
+        d = b.astype(np.int64) - books
+        assert set(np.flatnonzero(d[0, side])) == {tick} and not d[0, 1 - side].any()
+        assert r[0, REC["n_trades"]] == 0 and r[0, REC["prev"]] == 25 and r[0, REC["last"]] == init
+        assert d[0, side, tick] == r[0, REC["sub_sell" if side else "sub_buy"]]
+    # second step of market 0: the book now rests bb 10 / ba 12 -> mid2 22 < 25 -> SELL at
+    # round(11 - 1) = 10, which crosses the 7 lots bid at tick 10: p* = 10, Vmax = 7
+    books = np.zeros((1, 2, L), dtype=np.int32)
+    books[0, 0, 10] = 7; books[0, 0, 4] = 9; books[0, 1, 15] = 3; books[0, 1, 40] = 1
+    _, recs = oracle.init_state(1, L, 30, model=4)
+    b, r = oracle.run_markets(dict(p, init_price=30), L, A, 3, [0], 2, books, recs)
+    assert r[0, REC["prev"]] == 22 and r[0, REC["last"]] == 10 and r[0, REC["sum_vol"]] == 7 and b[0, 0, 10] == 0
 
 
 def test_mid_price_retrieval_eq3(oracle):
