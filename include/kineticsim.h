@@ -49,7 +49,8 @@ typedef enum {
   KS_ERR_UNSUPPORTED = -2, /* L > 32768 (p* must fit the 16-bit field of the trajectory hash), or a book
                               that does not fit this device's shared memory.  16384 < L <= 32768 runs on a
                               thread-block cluster (DSMEM), see KS_OPT_CLUSTER_SIZE                        */
-  KS_ERR_OVERFLOW = -3,    /* a per-side depth sum or a statistic could leave its integer type            */
+  KS_ERR_OVERFLOW = -3,    /* a per-side depth sum could leave int32 (refused before the run), or a
+                              statistic DID leave int64 during an earlier run (sticky, see ks_run)        */
   KS_ERR_CUDA = -4,        /* a CUDA call failed; text in ks_last_error()                                 */
   KS_ERR_NOMEM = -5        /* host allocation failed                                                      */
 } ks_status;
@@ -141,9 +142,11 @@ KS_API size_t ks_state_bytes(int32_t M, int32_t L);
  *   out      HOST: receives the handle (freed by ks_destroy).
  *   p        HOST: agent parameters, copied.
  *   seed     Philox key.
- *   d_state  DEVICE: caller-owned buffer of ks_state_bytes(M, L) bytes, 16-byte aligned; the
- *            library never allocates or frees device memory and never frees d_state.  It IS the
- *            checkpoint: books, prices, step counter and accumulators live there between calls.
+ *   d_state  DEVICE: caller-owned buffer of ks_state_bytes(M, L) bytes, 16-byte aligned, on the
+ *            CURRENT device (the handle remembers that device and makes it current inside every
+ *            later call); the library never allocates or frees device memory and never frees
+ *            d_state.  It IS the checkpoint: books, prices, step counter and accumulators live
+ *            there between calls, and ks_attach resumes from a saved copy of it.
  * Enqueues the initialisation on `stream`: empty books, last = prev = init price, zero sums
  * (Alg.1 l.2-3; opening quotes per BASELINE.json: empty book, price L/2).
  * ks_create_ex additionally takes the global id of this shard's first market: Philox is keyed by
@@ -156,12 +159,35 @@ KS_API ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, con
                               uint64_t seed, uint32_t market_base, void* d_state, void* stream);
 
 /*
+ * Resume from a checkpoint (the "final order book and clearing statistics in global memory" of
+ * Alg.1 "Ensure", fed back in): a new handle over a d_state that ALREADY holds the
+ * bytes an earlier handle left there (same M, L; the caller passes the same A, parameters, seed
+ * and market_base to continue the same trajectory).  Nothing is initialised: books, prices, step
+ * counter, sums and hash are taken as they are, so
+ *     ks_run(S1) -> save d_state -> ... -> restore -> ks_attach -> ks_run(S2)
+ * leaves the bytes of one uninterrupted ks_run(S1+S2).  Unlike the other calls this one
+ * SYNCHRONISES `stream`: it reads the step counter and the largest per-side depth back from the
+ * device for the overflow guards of ks_run.  Arguments and errors as ks_create_ex, plus
+ * KS_ERR_INVALID_ARG when d_state holds a negative depth or an impossible step counter.
+ */
+KS_API ks_status ks_attach(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p,
+                           uint64_t seed, uint32_t market_base, void* d_state, void* stream);
+
+/*
  * Advance every market by S steps with ONE launch of the persistent kernel,
  * continuing from the state in d_state: the Philox step index is steps_done + i, so
  * ks_run(S1); ks_run(S2) leaves the same bytes as ks_run(S1+S2).  S = 0 is a no-op.
  * KS_ERR_OVERFLOW (nothing enqueued) when (steps_done+S) x per-step per-side inflow bound, plus
- * the depth injected by ks_write_books, could reach 2^31, or (L-1)^4 x (steps_done+S) >= 2^63.
- * After a ks_write_books this call first waits (host-side) for that call's depth check.
+ * the depth injected by ks_write_books, could reach 2^31 (int32 book), or steps_done+S >= 2^32.
+ * Deferred errors.  (1) If the depth check of a preceding ks_write_books has not finished yet, the
+ * call does NOT wait for it: the kernel reads the check's result on the device and, when the bound
+ * is violated (or a negative depth was stored), the whole launch returns without changing a byte
+ * of d_state.  (2) The int64 sums of r^3 and r^4 (f[8], f[9]) can only overflow on wide grids
+ * after very large price moves ((L-1)^4 x steps >= 2^63 at the earliest); the kernel detects the
+ * signed overflow exactly when it happens.  Either event sets a sticky flag that the kernel writes
+ * into host memory: every later ks_run* / ks_read_* / ks_write_books on this handle -- in
+ * particular the first ks_read_* after the caller has synchronised the stream -- returns
+ * KS_ERR_OVERFLOW (KS_ERR_INVALID_ARG for the negative depth), and the handle must be destroyed.
  */
 KS_API ks_status ks_run(ks_sim* s, int64_t S, void* stream);
 
@@ -192,26 +218,38 @@ KS_API ks_status ks_run_traced(ks_sim* s, int64_t S, int32_t* d_trace, void* str
 KS_API ks_status ks_trace_stats(const int32_t* d_trace, int32_t M, int64_t S, int32_t K, double* d_out,
                                 void* stream);
 
+/* HOST-only, never blocks: KS_OK, or the sticky deferred error of this handle (see ks_run).  A
+ * caller that has synchronised the stream after a run learns here whether that run was refused on
+ * the device or overflowed a statistic. */
+KS_API ks_status ks_error_state(ks_sim* s);
+
 /* Copy the books / the records out of d_state.  dst: HOST or DEVICE pointer (cudaMemcpyDefault),
  * int32 [M][2][L] resp. ks_market_stats [M]; a host destination must stay valid until the stream
  * work is done (pinned memory makes the copy asynchronous).  Alg.1 "Ensure". */
 KS_API ks_status ks_read_books(ks_sim* s, int32_t* dst, void* stream);
 KS_API ks_status ks_read_stats(ks_sim* s, ks_market_stats* dst, void* stream);
 
-/* Replace the resting books (test / checkpoint-restore hook: "seeds the opening quotes",
- * PAPER.md:126).  src: HOST or DEVICE pointer, int32 [M][2][L], every entry >= 0.  Records are
- * left as they are.  Also enqueues a depth check whose result the next ks_run waits for. */
+/* Replace the resting books (test hook: "seeds the opening quotes").  src: HOST or
+ * DEVICE pointer, int32 [M][2][L], every entry >= 0.  Records are left as they are.  Also enqueues
+ * a depth check (one small kernel) whose result the next ks_run uses -- on the host if it has
+ * finished by then, else on the device (see ks_run, deferred errors). */
 KS_API ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream);
 
 /* Tuning / ablation switches; none of them changes a single output byte.  Returns
  * KS_ERR_INVALID_ARG for an unknown option or value. */
 typedef enum {
-  KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 64..1024, multiple of 32          */
+  KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 32..1024, multiple of 32          */
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
   KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
-  KS_OPT_PIPELINE = 4,      /* software pipeline for few markets (the next step's draws overlap the clearing):
-                               0 = automatic, 1 = never, 2 = whenever legal (zero-intelligence model, plain
-                               atomics, >= 64 threads, at most 4 agents per generating thread)               */
+  KS_OPT_PIPELINE = 4,      /* the decoupled kernel (generating warps fill a price-independent relative order
+                               histogram up to two steps ahead; one clearing warp per market, holding no
+                               agents, merges it at the step's price and clears): 0 = automatic (when the
+                               grid underfills the GPU, i.e. step latency is what counts), 1 = never,
+                               2 = whenever legal (KS_MODEL_ZI / KS_MODEL_ZI_PACKED4, plain atomics,
+                               >= 64 threads, L <= 16384, book + two histograms fit shared memory)          */
+  KS_OPT_REL_COLUMNS = 5,   /* decoupled kernel only: 0 = one int32 per histogram bin, 1 = 32 lane columns per
+                               bin (column = lane = bank: a warp's atomics never conflict) -- the
+                               aggregation ablation of north_star (3)                                       */
   KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
                                i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
                                book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and

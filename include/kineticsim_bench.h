@@ -1,7 +1,9 @@
 /*
- * kineticsim_bench.h -- ablation and roofline-microbenchmark entry points of the library.
- * Not part of the product ABI (include/kineticsim.h); used by bench.py, the tests and DESIGN.md's
- * measurement section.  Same conventions as kineticsim.h.  The ks_bench_* calls are SYNCHRONOUS:
+ * kineticsim_bench.h -- ablation and roofline-microbenchmark entry points, exported by a SEPARATE
+ * library (libkineticsim_bench.so, linked against libkineticsim.so).  Not part of the product ABI
+ * (include/kineticsim.h); used by bench.py, the tests and DESIGN.md's measurement section.  Same
+ * conventions as kineticsim.h, except that the ks_bench_* calls allocate a few bytes of device
+ * scratch for themselves (the product library never allocates device memory) and are SYNCHRONOUS:
  * they time their own kernel with CUDA events on `stream` (after `warmup` untimed launches) and
  * return the best of `reps` timed launches.
  */
@@ -16,7 +18,8 @@ extern "C" {
 
 /* a8 ablation (SIII-F "naive" traffic): the same step as ks_run, but ONE LAUNCH
  * PER STEP with the book stored to and re-loaded from HBM between launches, so global traffic is
- * Theta(S*M*L) instead of Theta(M*L).  Leaves bit-identical state to ks_run(S). */
+ * Theta(S*M*L) instead of Theta(M*L).  Leaves bit-identical state to ks_run(S).  Implemented as S
+ * calls of the product's public ks_run(s, 1, stream). */
 KS_API ks_status ks_run_stepwise(ks_sim* s, int64_t S, void* stream);
 
 /* Shared-memory atomic ceilings (BASELINE.json `metric`: "% of smem-atomic roofline").
@@ -44,7 +47,9 @@ KS_API ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int
 /* Raw issue rates of the two instructions Philox is made of.  kind 0: IMAD.WIDE.U32 (u32 x u32 ->
  * u64), kind 1: LOP3 (three-input xor), kind 2: one of each, interleaved (the Philox round
  * pattern), kind 3 / 4: one IMAD.WIDE with two / three LOP3 (what every further alu-pipe instruction
- * costs the multiply stream).  Each thread runs 8 independent dependency chains.  *thread_ops_per_s receives thread-level operations per second
+ * costs the multiply stream), kind 5: a pure stream of mul.wide.u32 with no addend (IMAD.WIDE.U32
+ * only) -- the measured peak of the pipe that bounds the hot loop (roofline.peak in bench.py).
+ * Each thread runs 8 independent dependency chains.  *thread_ops_per_s receives thread-level operations per second
  * over the whole GPU (divide by 32 x SMs x 4 x clock for warp instructions per cycle per
  * scheduler). */
 KS_API ks_status ks_bench_int_pipe(int32_t kind, int32_t threads, int32_t ctas_per_sm, int32_t iters,

@@ -1,7 +1,7 @@
 // ks_api.cu -- host side of the C ABI declared in include/kineticsim.h.
 #include "../../include/kineticsim.h"
-#include "../../include/kineticsim_bench.h"
 #include "ks_cluster.cuh"
+#include "ks_decoupled.cuh"
 #include "ks_trace.cuh"
 
 #include <atomic>
@@ -44,69 +44,102 @@ struct ks_sim {
   uint32_t market_base;
   void* d_state;
   int64_t steps_done;
-  int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books
+  int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books / found by ks_attach
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe;
+  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe, opt_cols;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
-  // ks_write_books depth check
-  unsigned long long* h_bound;   // pinned host
+  unsigned long long* h_words;   // pinned, mapped host memory: [0] depth bound of ks_write_books (copied),
+                                 // [1] sticky error flags written by the kernels themselves (ks::kFlag*)
+  unsigned long long* d_flags;   // device alias of &h_words[1]
   cudaEvent_t bound_event;
-  int32_t bound_pending;
+  int32_t bound_pending;         // a ks_write_books depth check whose result the host has not seen yet
   int32_t dev_smem_optin;
   int32_t num_sms;
+  int32_t device;                // the CUDA device d_state lives on (the current one at creation)
 };
 
-static int32_t* books_ptr(const ks_sim* s) { return reinterpret_cast<int32_t*>(s->d_state); }
-static long long* recs_ptr(const ks_sim* s) {
+namespace {
+
+// Makes the handle's device current for the duration of a call (a process may hold several GPUs).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+// Sticky device-raised errors.  The kernels write them into mapped host memory; a caller that can
+// see a run's results has synchronised the stream and therefore cannot miss the flag.
+ks_status check_flags(const ks_sim* s, const char* who) {
+  const unsigned long long f = *reinterpret_cast<volatile unsigned long long*>(&s->h_words[1]);
+  if (f == 0) return KS_OK;
+  if (f & ks::kFlagNegativeDepth) { set_err("%s: ks_write_books stored a negative depth; the following run was not executed", who); return KS_ERR_INVALID_ARG; }
+  if (f & ks::kFlagDepthOverflow) { set_err("%s: per-side depth could reach 2^31; the run was not executed", who); return KS_ERR_OVERFLOW; }
+  set_err("%s: a statistic (sum of r^3 or r^4) left int64 during an earlier run", who);
+  return KS_ERR_OVERFLOW;
+}
+
+int32_t* books_ptr(const ks_sim* s) { return reinterpret_cast<int32_t*>(s->d_state); }
+long long* recs_ptr(const ks_sim* s) {
   return reinterpret_cast<long long*>(reinterpret_cast<char*>(s->d_state) + (size_t)s->M * 8 * (size_t)s->L);
 }
-static unsigned long long* scratch_ptr(const ks_sim* s) {
+unsigned long long* scratch_ptr(const ks_sim* s) {
   return reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(s->d_state) +
                                                (size_t)s->M * (8 * (size_t)s->L + 128));
 }
 
-static bool shape_ok(int32_t M, int32_t L) { return M >= 1 && is_pow2(L) && L >= 32 && L <= 32768; }
+bool shape_ok(int32_t M, int32_t L) { return M >= 1 && is_pow2(L) && L >= 32 && L <= 32768; }
 
-extern "C" {
-
-size_t ks_state_bytes(int32_t M, int32_t L) {
-  if (!shape_ok(M, L)) return 0;
-  return (size_t)M * (8 * (size_t)L + 128) + 256;
+void free_sim(ks_sim* s) {
+  if (!s) return;
+  if (s->h_words) cudaFreeHost(s->h_words);
+  if (s->bound_event) cudaEventDestroy(s->bound_event);
+  delete s;
 }
 
-const char* ks_last_error(void) { return g_err; }
-int64_t ks_launch_count(void) { return g_launches.load(); }
-
-ks_status ks_create(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
-                    void* d_state, void* stream) {
-  return ks_create_ex(out, M, L, A, p, seed, 0u, d_state, stream);
+// Enqueue the depth check of the books in d_state: max over markets and sides of the total depth
+// -> scratch word -> h_words[0]; bound_event marks its completion.
+ks_status enqueue_depth_check(ks_sim* s, cudaStream_t st) {
+  KS_CUDA(cudaMemsetAsync(scratch_ptr(s), 0, sizeof(unsigned long long), st));
+  ks::ks_depth_bound_kernel<<<2 * s->M, 128, 0, st>>>(books_ptr(s), s->L, scratch_ptr(s));
+  KS_CUDA(cudaGetLastError());
+  g_launches++;
+  KS_CUDA(cudaMemcpyAsync(&s->h_words[0], scratch_ptr(s), sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  KS_CUDA(cudaEventRecord(s->bound_event, st));
+  s->bound_pending = 1;
+  return KS_OK;
 }
 
-ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
-                       uint32_t market_base, void* d_state, void* stream) {
-  if (!out || !p || !d_state) { set_err("ks_create: NULL argument"); return KS_ERR_INVALID_ARG; }
+// ks_create_ex (attach = false: enqueue the initialisation) and ks_attach (attach = true: adopt
+// the state already in d_state).
+ks_status create_common(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
+                        uint32_t market_base, void* d_state, void* stream, bool attach) {
+  const char* who = attach ? "ks_attach" : "ks_create";
+  if (!out || !p || !d_state) { set_err("%s: NULL argument", who); return KS_ERR_INVALID_ARG; }
   *out = nullptr;
-  if (M < 1 || A < 0 || !is_pow2(L) || L < 32) { set_err("ks_create: need M >= 1, A >= 0, L a power of two >= 32"); return KS_ERR_INVALID_ARG; }
-  if (L > kMaxL) { set_err("ks_create: L > 32768 is not supported (p* must fit 16 bits of the trajectory hash)"); return KS_ERR_UNSUPPORTED; }
-  if ((reinterpret_cast<uintptr_t>(d_state) & 15) != 0) { set_err("ks_create: d_state must be 16-byte aligned"); return KS_ERR_INVALID_ARG; }
-  if (p->model < KS_MODEL_ZI || p->model > KS_MODEL_PAPER) { set_err("ks_create: unknown model"); return KS_ERR_INVALID_ARG; }
+  if (M < 1 || A < 0 || !is_pow2(L) || L < 32) { set_err("%s: need M >= 1, A >= 0, L a power of two >= 32", who); return KS_ERR_INVALID_ARG; }
+  if (L > kMaxL) { set_err("%s: L > 32768 is not supported (p* must fit 16 bits of the trajectory hash)", who); return KS_ERR_UNSUPPORTED; }
+  if ((reinterpret_cast<uintptr_t>(d_state) & 15) != 0) { set_err("%s: d_state must be 16-byte aligned", who); return KS_ERR_INVALID_ARG; }
+  if (p->model < KS_MODEL_ZI || p->model > KS_MODEL_PAPER) { set_err("%s: unknown model", who); return KS_ERR_INVALID_ARG; }
   if (p->noise_delta < 0 || p->noise_delta >= L || p->noise_qmax < 1 || p->noise_qmax > kMaxQty || p->init_price >= L) {
-    set_err("ks_create: bad noise parameters or init_price"); return KS_ERR_INVALID_ARG;
+    set_err("%s: bad noise parameters or init_price", who); return KS_ERR_INVALID_ARG;
   }
   if (p->model == KS_MODEL_PAPER) {
     if (p->maker_spread_max < 0 || p->maker_spread_max >= L || p->maker_qty < 1 || p->maker_qty > kMaxQty ||
         p->mom_qmax < 1 || p->mom_qmax > kMaxQty || p->paper_n_mom < 0 || p->paper_n_maker < 0 ||
         (int64_t)p->paper_n_mom + p->paper_n_maker > A || p->paper_pmkt_q16 < 0 || p->paper_pmkt_q16 > 65536) {
-      set_err("ks_create: bad parameters of the paper agent model"); return KS_ERR_INVALID_ARG;
+      set_err("%s: bad parameters of the paper agent model", who); return KS_ERR_INVALID_ARG;
     }
-    if (L > kMaxLPerCta) { set_err("ks_create: the paper agent model has no cluster path (L <= 16384)"); return KS_ERR_UNSUPPORTED; }
+    if (L > kMaxLPerCta) { set_err("%s: the paper agent model has no cluster path (L <= 16384)", who); return KS_ERR_UNSUPPORTED; }
   } else if ((p->model & 1) == KS_MODEL_MIX3 &&
       (p->maker_spread_max < 1 || p->maker_spread_max > L || p->maker_qty < 1 || p->maker_qty > kMaxQty ||
        p->mom_delta < 0 || p->mom_delta >= L || p->mom_qmax < 1 || p->mom_qmax > kMaxQty)) {
-    set_err("ks_create: bad maker/momentum parameters"); return KS_ERR_INVALID_ARG;
+    set_err("%s: bad maker/momentum parameters", who); return KS_ERR_INVALID_ARG;
   }
-  if ((uint64_t)market_base + (uint64_t)M > 0x100000000ull) { set_err("ks_create: market ids exceed 32 bits"); return KS_ERR_INVALID_ARG; }
+  if ((uint64_t)market_base + (uint64_t)M > 0x100000000ull) { set_err("%s: market ids exceed 32 bits", who); return KS_ERR_INVALID_ARG; }
 
   int dev = 0, optin = 0, sms = 0;
   KS_CUDA(cudaGetDevice(&dev));
@@ -114,16 +147,16 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   KS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   {
     const int32_t Lc = L > kMaxLPerCta ? kMaxLPerCta : L;           // larger books are split across a cluster
-    if ((size_t)8 * Lc + 2048 > (size_t)optin) { set_err("ks_create: book does not fit this device's shared memory"); return KS_ERR_UNSUPPORTED; }
+    if ((size_t)8 * Lc + 2048 > (size_t)optin) { set_err("%s: book does not fit this device's shared memory", who); return KS_ERR_UNSUPPORTED; }
   }
 
   ks_sim* s = new (std::nothrow) ks_sim();
-  if (!s) { set_err("ks_create: out of host memory"); return KS_ERR_NOMEM; }
+  if (!s) { set_err("%s: out of host memory", who); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
-  s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0;
-  s->dev_smem_optin = optin; s->num_sms = sms;
-  s->bound_pending = 0; s->h_bound = nullptr; s->bound_event = nullptr;
+  s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = attach ? 0 : 1;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0; s->opt_cols = 0;
+  s->dev_smem_optin = optin; s->num_sms = sms; s->device = dev;
+  s->bound_pending = 0; s->h_words = nullptr; s->d_flags = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_PAPER) {
     s->n_mom = p->paper_n_mom; s->n_maker = 0; s->n_noise = A - p->paper_n_mom - p->paper_n_maker;
     s->inflow_per_step = (int64_t)s->n_noise * p->noise_qmax + (int64_t)p->paper_n_mom * p->mom_qmax +
@@ -138,39 +171,87 @@ ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_a
   }
   if (s->p.init_price < 0) s->p.init_price = L / 2;
 
-  cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&s->h_bound), sizeof(unsigned long long), cudaHostAllocDefault);
+  cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&s->h_words), 2 * sizeof(unsigned long long), cudaHostAllocMapped);
+  if (e == cudaSuccess) { s->h_words[0] = 0; s->h_words[1] = 0; }
+  if (e == cudaSuccess) {
+    void* dp = nullptr;
+    e = cudaHostGetDevicePointer(&dp, &s->h_words[1], 0);
+    s->d_flags = reinterpret_cast<unsigned long long*>(dp);
+  }
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->bound_event, cudaEventDisableTiming);
   if (e != cudaSuccess) {
-    set_err("ks_create: %s", cudaGetErrorString(e));
-    if (s->h_bound) cudaFreeHost(s->h_bound);
-    delete s;
+    set_err("%s: %s", who, cudaGetErrorString(e));
+    free_sim(s);
     return KS_ERR_CUDA;
   }
-  *s->h_bound = 0;
 
-  size_t nvec = (size_t)M * 2 * (size_t)L / 4;
-  int blocks = (int)((nvec + 255) / 256);
-  if (blocks > sms * 16) blocks = sms * 16;
-  if (blocks < 1) blocks = 1;
-  ks::ks_init_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<int4*>(books_ptr(s)), nvec, recs_ptr(s), M,
-                                                              s->p.init_price,
-                                                              p->model == KS_MODEL_PAPER ? 2 * s->p.init_price : s->p.init_price);
-  e = cudaGetLastError();
-  if (e != cudaSuccess) {
-    set_err("ks_create: init launch failed: %s", cudaGetErrorString(e));
-    cudaFreeHost(s->h_bound); cudaEventDestroy(s->bound_event); delete s;
-    return KS_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!attach) {
+    size_t nvec = (size_t)M * 2 * (size_t)L / 4;
+    int blocks = (int)((nvec + 255) / 256);
+    if (blocks > sms * 16) blocks = sms * 16;
+    if (blocks < 1) blocks = 1;
+    ks::ks_init_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<int4*>(books_ptr(s)), nvec, recs_ptr(s), M, s->p.init_price,
+                                               p->model == KS_MODEL_PAPER ? 2 * s->p.init_price : s->p.init_price);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) {
+      set_err("%s: init launch failed: %s", who, cudaGetErrorString(e));
+      free_sim(s);
+      return KS_ERR_CUDA;
+    }
+    g_launches++;
+  } else {
+    // adopt the checkpoint: the step counter (for the overflow guards) and the resting depth bound
+    // come back from the device; this call synchronises `stream`
+    long long steps0 = 0;
+    ks_status r = enqueue_depth_check(s, st);
+    if (r == KS_OK) {
+      e = cudaMemcpyAsync(&steps0, recs_ptr(s), sizeof(long long), cudaMemcpyDeviceToHost, st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+      if (e != cudaSuccess) { set_err("%s: %s", who, cudaGetErrorString(e)); r = KS_ERR_CUDA; }
+    }
+    if (r == KS_OK && (steps0 < 0 || steps0 >= 4294967296LL)) { set_err("%s: d_state does not hold a valid record (step counter)", who); r = KS_ERR_INVALID_ARG; }
+    if (r == KS_OK && s->h_words[0] == 0xffffffffffffffffull) { set_err("%s: d_state holds a negative depth", who); r = KS_ERR_INVALID_ARG; }
+    if (r != KS_OK) { free_sim(s); return r; }
+    s->bound_pending = 0;
+    s->steps_done = steps0;
+    s->resting_bound = (int64_t)s->h_words[0];
   }
-  g_launches++;
   *out = s;
   return KS_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+size_t ks_state_bytes(int32_t M, int32_t L) {
+  if (!shape_ok(M, L)) return 0;
+  return (size_t)M * (8 * (size_t)L + 128) + 256;
+}
+
+const char* ks_last_error(void) { return g_err; }
+int64_t ks_launch_count(void) { return g_launches.load(); }
+
+ks_status ks_create(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
+                    void* d_state, void* stream) {
+  return create_common(out, M, L, A, p, seed, 0u, d_state, stream, false);
+}
+
+ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
+                       uint32_t market_base, void* d_state, void* stream) {
+  return create_common(out, M, L, A, p, seed, market_base, d_state, stream, false);
+}
+
+ks_status ks_attach(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p, uint64_t seed,
+                    uint32_t market_base, void* d_state, void* stream) {
+  return create_common(out, M, L, A, p, seed, market_base, d_state, stream, true);
+}
+
 void ks_destroy(ks_sim* s) {
   if (!s) return;
-  if (s->h_bound) cudaFreeHost(s->h_bound);
-  if (s->bound_event) cudaEventDestroy(s->bound_event);
-  delete s;
+  DeviceGuard g(s->device);
+  free_sim(s);
 }
 
 ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
@@ -190,6 +271,9 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_PIPELINE:
       if (value != 0 && value != 1 && value != 2) break;
       s->opt_pipe = value; return KS_OK;
+    case KS_OPT_REL_COLUMNS:
+      if (value != 0 && value != 1) break;
+      s->opt_cols = value; return KS_OK;
     case KS_OPT_CLUSTER_SIZE:
       if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break;
       if (value > 1 && (s->L / value < 32 || s->opt_atomic || s->p.model == KS_MODEL_PAPER)) break;
@@ -212,13 +296,21 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 // T = 32 beats 64/128 on C4).  A book so large that 32-thread CTAs would leave the SM short of
 // warps -> widen until ~1024 threads are resident; few markets -> widen so the whole GPU is used,
 // but never beyond the agents.
-struct LaunchPlan { int T; size_t smem; };
+struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
+
+// Bytes of one side (sell or buy bins) of one relative histogram of ks_decoupled_kernel: 2*delta+1
+// bins of one int32 (padded to 128 bytes) or of 32 lane columns.  One buffer = two sides.
+static uint32_t rel_side_for(const ks_sim* s) {
+  const uint32_t n = 2u * (uint32_t)s->p.noise_delta + 1u;
+  return s->opt_cols ? n * 128u : ((n * 4u + 127u) / 128u) * 128u;
+}
 
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
   pl.smem = (size_t)8 * (size_t)s->L;
+  pl.decoupled = false; pl.rel_side = 0;
   int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
   if (k < 1) k = 1;
   if (k > 32) k = 32;
@@ -226,21 +318,49 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   if (s->opt_threads) {
     T = s->opt_threads;
   } else {
-    // few markets: widen until the grid brings ~16 warps to every SM (measured: C2, M = 1024, runs
-    // 288 G events/s at T = 128 against 250 at T = 256 and 259 at T = 32 -- wider CTAs pay more at
-    // the two barriers than their extra warps hide)
+    // few markets: widen until the grid brings ~16 warps to every SM (wider CTAs pay more at the
+    // two barriers than their extra warps hide)
     const long long want_threads = (long long)s->num_sms * 512;
     const int a_cap = s->A > 32 ? s->A : 32;
     while (T < 1024 && (long long)s->M * T < want_threads && T * 2 <= a_cap) T *= 2;
     while (T < 1024 && (long long)k * T < 1024 && T * 2 <= a_cap) T *= 2;
   }
   pl.T = T;
+  // ks_decoupled_kernel: legal for the zero-intelligence rules (literal or PACKED4) with plain
+  // atomics when book + two relative histograms fit the CTA's shared memory; automatic when the
+  // grid leaves the GPU underfilled, i.e. the step latency is what counts (C1, C3).  Block size for
+  // it: one clearing warp + the smallest power-of-two-minus... generating threads holding <= 3 events.
+  const bool zi = s->p.model == KS_MODEL_ZI || s->p.model == KS_MODEL_ZI_PACKED4;
+  if (zi && !s->opt_atomic && s->opt_pipe != 1) {
+    const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
+    const uint32_t side = rel_side_for(s);
+    const bool fits = pl.smem + 4 * (size_t)side + 2048 <= (size_t)s->dev_smem_optin;
+    if (fits && (s->opt_pipe == 2 || underfilled)) {
+      int Td = pl.T;
+      if (!s->opt_threads) {
+        Td = 64;
+        while (Td < 1024 && (long long)(Td - 32) * 3 < s->A) Td *= 2;
+      }
+      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.smem += 4 * (size_t)side; }
+    }
+  }
   return pl;
 }
 
-template <int MODEL, int ATOM, bool PACKED, bool PIPE = false>
+template <int MODEL, int ATOM, bool PACKED>
 static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_persistent_kernel<MODEL, ATOM, PACKED, PIPE>;
+  auto kern = ks::ks_persistent_kernel<MODEL, ATOM, PACKED>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e != cudaSuccess) return e;
+  kern<<<P.M, T, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+template <bool PACKED, int COLS>
+static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
+  auto kern = ks::ks_decoupled_kernel<PACKED, COLS>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -273,21 +393,29 @@ static cudaError_t launch_cluster(const ks::KernelParams& P, int C, int T, cudaS
 static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, int32_t* d_trace = nullptr) {
   if (!s) { set_err("%s: NULL handle", who); return KS_ERR_INVALID_ARG; }
   if (S < 0) { set_err("%s: S < 0", who); return KS_ERR_INVALID_ARG; }
+  {
+    ks_status f = check_flags(s, who);
+    if (f != KS_OK) return f;
+  }
   if (S == 0) return KS_OK;
+  DeviceGuard guard(s->device);
+  // The depth bound of the last ks_write_books: taken from the host copy if the check has finished,
+  // otherwise the kernel reads the device word itself (never a host-side wait).
   if (s->bound_pending) {
-    KS_CUDA(cudaEventSynchronize(s->bound_event));
-    s->bound_pending = 0;
-    if (*s->h_bound == 0xffffffffffffffffull) { set_err("%s: ks_write_books stored a negative depth", who); return KS_ERR_INVALID_ARG; }
-    s->resting_bound = (int64_t)*s->h_bound;
+    const cudaError_t q = cudaEventQuery(s->bound_event);
+    if (q == cudaSuccess) {
+      s->bound_pending = 0;
+      if (s->h_words[0] == 0xffffffffffffffffull) { set_err("%s: ks_write_books stored a negative depth", who); return KS_ERR_INVALID_ARG; }
+      s->resting_bound = (int64_t)s->h_words[0];
+    } else if (q != cudaErrorNotReady) {
+      set_err("%s: %s", who, cudaGetErrorString(q)); return KS_ERR_CUDA;
+    }
   }
   const long double total_steps = (long double)s->steps_done + (long double)S;
-  if ((long double)s->resting_bound + total_steps * (long double)s->inflow_per_step >= 2147483648.0L) {
-    set_err("%s: per-side depth could reach 2^31", who); return KS_ERR_OVERFLOW;
-  }
-  const long double lm1 = (long double)(s->L - 1);
-  if (lm1 * lm1 * lm1 * lm1 * total_steps >= 9223372036854775808.0L || total_steps >= 4294967296.0L) {
-    set_err("%s: a statistic or the step counter could overflow", who); return KS_ERR_OVERFLOW;
-  }
+  const long double inflow = total_steps * (long double)s->inflow_per_step;
+  const long double known_resting = s->bound_pending ? 0.0L : (long double)s->resting_bound;
+  if (known_resting + inflow >= 2147483648.0L) { set_err("%s: per-side depth could reach 2^31", who); return KS_ERR_OVERFLOW; }
+  if (total_steps >= 4294967296.0L) { set_err("%s: the step counter would pass 2^32", who); return KS_ERR_OVERFLOW; }
 
   ks::KernelParams P;
   memset(&P, 0, sizeof(P));
@@ -315,6 +443,11 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
   P.trace = reinterpret_cast<int2*>(d_trace);
   P.S = S;
   P.orders_per_step = (long long)s->A + s->n_maker;
+  P.host_flags = s->d_flags;
+  if (s->bound_pending) {
+    P.depth_word = scratch_ptr(s);
+    P.depth_limit = (unsigned long long)(2147483647.0L - inflow);   // inflow < 2^31 was checked above
+  }
 
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
@@ -335,24 +468,12 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     if (!packed) e = mix ? launch_cluster<1, false>(P, C, T, st) : launch_cluster<0, false>(P, C, T, st);
     else         e = mix ? launch_cluster<1, true>(P, C, T, st) : launch_cluster<0, true>(P, C, T, st);
   } else {
-    // software pipeline (kernel template PIPE): legal for the literal zero-intelligence contract
-    // with plain atomics when every generating thread (warps >= 1) holds at most kPipeEvents events;
-    // automatic when the grid leaves the GPU underfilled, i.e. the step latency is what counts (C3).
-    // Block size for it: the smallest power of two whose generating threads hold <= 3 events each
-    // (measured on C3: T = 256 -> 7.4 ms, T = 512 -> 8.0 ms, unpipelined 8.9 ms).
-    LaunchPlan pl = plan_launch(s);
-    const bool pipe_model = !paper && !mix && !packed && !s->opt_atomic;
-    const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
-    if (pipe_model && !s->opt_threads && s->opt_pipe != 1 && (s->opt_pipe == 2 || underfilled)) {
-      int Tp = 64;
-      while (Tp < 1024 && (long long)(Tp - 32) * 3 < s->A) Tp *= 2;
-      if ((long long)(Tp - 32) * ks::kPipeEvents >= s->A) pl.T = Tp;
-    }
-    const bool pipe_legal = pipe_model && pl.T >= 64 && (long long)(pl.T - 32) * ks::kPipeEvents >= s->A;
-    const bool pipe = pipe_legal && s->opt_pipe != 1 && (s->opt_pipe == 2 || underfilled);
-    if (pipe)
-      e = launch_persistent<0, 0, false, true>(P, pl.T, pl.smem, st);
-    else if (paper)
+    const LaunchPlan pl = plan_launch(s);
+    P.rel_side = pl.rel_side; P.rel_stride = 2 * pl.rel_side;
+    if (pl.decoupled) {
+      if (s->opt_cols) e = packed ? launch_decoupled<true, 32>(P, pl.T, pl.smem, st) : launch_decoupled<false, 32>(P, pl.T, pl.smem, st);
+      else             e = packed ? launch_decoupled<true, 1>(P, pl.T, pl.smem, st) : launch_decoupled<false, 1>(P, pl.T, pl.smem, st);
+    } else if (paper)
       e = launch_persistent<2, 0, false>(P, pl.T, pl.smem, st);
     else if (packed)
       e = mix ? launch_persistent<1, 0, true>(P, pl.T, pl.smem, st) : launch_persistent<0, 0, true>(P, pl.T, pl.smem, st);
@@ -388,42 +509,38 @@ ks_status ks_trace_stats(const int32_t* d_trace, int32_t M, int64_t S, int32_t K
   return KS_OK;
 }
 
-// a8 ablation: the same kernel, one launch per step, book through HBM between launches.
-ks_status ks_run_stepwise(ks_sim* s, int64_t S, void* stream) {
-  if (!s) { set_err("ks_run_stepwise: NULL handle"); return KS_ERR_INVALID_ARG; }
-  if (S < 0) { set_err("ks_run_stepwise: S < 0"); return KS_ERR_INVALID_ARG; }
-  for (int64_t i = 0; i < S; ++i) {
-    ks_status r = run_impl(s, 1, stream, "ks_run_stepwise");
-    if (r != KS_OK) return r;
-  }
-  return KS_OK;
+ks_status ks_error_state(ks_sim* s) {
+  if (!s) { set_err("ks_error_state: NULL handle"); return KS_ERR_INVALID_ARG; }
+  return check_flags(s, "ks_error_state");
 }
 
 ks_status ks_read_books(ks_sim* s, int32_t* dst, void* stream) {
   if (!s || !dst) { set_err("ks_read_books: NULL argument"); return KS_ERR_INVALID_ARG; }
+  ks_status f = check_flags(s, "ks_read_books");
+  if (f != KS_OK) return f;
+  DeviceGuard guard(s->device);
   KS_CUDA(cudaMemcpyAsync(dst, books_ptr(s), (size_t)s->M * 8 * (size_t)s->L, cudaMemcpyDefault, (cudaStream_t)stream));
   return KS_OK;
 }
 
 ks_status ks_read_stats(ks_sim* s, ks_market_stats* dst, void* stream) {
   if (!s || !dst) { set_err("ks_read_stats: NULL argument"); return KS_ERR_INVALID_ARG; }
+  ks_status f = check_flags(s, "ks_read_stats");
+  if (f != KS_OK) return f;
+  DeviceGuard guard(s->device);
   KS_CUDA(cudaMemcpyAsync(dst, recs_ptr(s), (size_t)s->M * 128, cudaMemcpyDefault, (cudaStream_t)stream));
   return KS_OK;
 }
 
 ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream) {
   if (!s || !src) { set_err("ks_write_books: NULL argument"); return KS_ERR_INVALID_ARG; }
+  ks_status f = check_flags(s, "ks_write_books");
+  if (f != KS_OK) return f;
+  DeviceGuard guard(s->device);
   cudaStream_t st = (cudaStream_t)stream;
   KS_CUDA(cudaMemcpyAsync(books_ptr(s), src, (size_t)s->M * 8 * (size_t)s->L, cudaMemcpyDefault, st));
-  KS_CUDA(cudaMemsetAsync(scratch_ptr(s), 0, sizeof(unsigned long long), st));
-  ks::ks_depth_bound_kernel<<<2 * s->M, 128, 0, st>>>(books_ptr(s), s->L, scratch_ptr(s));
-  KS_CUDA(cudaGetLastError());
-  g_launches++;
-  KS_CUDA(cudaMemcpyAsync(s->h_bound, scratch_ptr(s), sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-  KS_CUDA(cudaEventRecord(s->bound_event, st));
-  s->bound_pending = 1;
   s->fresh = 0;
-  return KS_OK;
+  return enqueue_depth_check(s, st);
 }
 
 void ks_derive_stats(const ks_market_stats* rec, ks_derived_stats* out, int64_t n) {

@@ -72,6 +72,8 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
   __shared__ int s_ctl[4];                            // [0] = price at the start of the step (written by rank 0)
   __shared__ long long s_ctot[8][2];                  // rank 0 only: per-rank (sum_bid, sum_ask)
   __shared__ int s_cext[8][2];                        // rank 0 only: per-rank (bmax, amin), global ticks
+  __shared__ int s_abort;
+  __shared__ int s_ovf;
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
   const int L = P.L, log2C = P.log2C, C = 1 << log2C;
@@ -92,6 +94,23 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
   const uint32_t ctot_saddr = (uint32_t)__cvta_generic_to_shared(&s_ctot[rank][0]);
   const uint32_t cext_saddr = (uint32_t)__cvta_generic_to_shared(&s_cext[rank][0]);
   const int tick_base = (int)rank * Lc;
+
+  // deferred depth check of ks_write_books (as in ks_persistent_kernel): a uniform decision of the
+  // whole grid, taken before any cluster barrier
+  if (P.depth_word) {
+    if (tid == 0) {
+      const unsigned long long b = *P.depth_word;
+      s_abort = b > P.depth_limit;
+      if (b > P.depth_limit && blockIdx.x == 0) {
+        *P.host_flags = b == 0xffffffffffffffffull ? kFlagNegativeDepth : kFlagDepthOverflow;
+        __threadfence_system();
+      }
+    }
+    __syncthreads();
+    if (s_abort) return;
+  }
+  // every CTA of the cluster must be running before its shared memory is written remotely
+  cluster_sync();
 
   // ---- a0: every CTA loads its own ticks
   long long sb0 = 0, sa0 = 0;
@@ -130,7 +149,7 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
   int last = (int)s_rec[F_LAST], prev = (int)s_rec[F_PREV];
   const uint32_t t0 = (uint32_t)s_rec[F_STEPS];
   const long long vol0 = s_rec[F_SUMVOL];
-  if (tid == 0) s_ctl[0] = last;
+  if (tid == 0) { s_ctl[0] = last; s_ovf = 0; }
   cluster_sync();
   long long tot0_bid = 0, tot0_ask = 0;
   bmax = -1; amin = L;
@@ -155,18 +174,17 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
     if (rank == 0 && warp == 0) {
       int lo = max(0, min(amin, last - P.dmax));
       int hi = min(L - 1, max(bmax, last + P.dmax));
-      int vmax, pstar, nb, na;
+      int vmax, pstar, nb, na, base, wend;
+      LaneBounds lbnd;
       int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
-      if (P.force_generic || width8 > 256) clear_generic(io, L, lo & ~3, hi, lane, vmax, pstar, nb, na);
-      else if (hi - lo < 32)               clear_window1(io, L, lo, lane, vmax, pstar, nb, na);
-      else if (width4 <= 128)              clear_window<4>(io, L, lo & ~3, lane, vmax, pstar, nb, na);
-      else                                 clear_window<8>(io, L, lo & ~7, lane, vmax, pstar, nb, na);
+      if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, lbnd); }
+      else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, lbnd); }
+      else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, lbnd); }
+      else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, lbnd); }
+      reduce_bounds(lbnd, base, wend, nb, na);
       bmax = nb; amin = na;
-      if (lane == 0) {
-        int new_last;
-        update_record(s_rec, last, vmax, pstar, new_last);
-        for (int r = 0; r < C; ++r) st_cluster_s32(mapa_shared(ctl_saddr, (uint32_t)r), new_last);
-      }
+      if (lane < C) st_cluster_s32(mapa_shared(ctl_saddr, (uint32_t)lane), vmax > 0 ? pstar : last);
+      update_record_lanes(s_rec, &s_ovf, lane, last, vmax, pstar, last);
       if (P.trace) trace_step(s_trace, P.trace + (size_t)cluster_id * (size_t)P.S, s, P.S, lane,
                               vmax > 0 ? pstar : last, vmax);
     }
@@ -201,6 +219,7 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
       s_rec[F_SUBBUY] += (tot1_bid - tot0_bid) + dvol;
       s_rec[F_SUBSELL] += (tot1_ask - tot0_ask) + dvol;
       s_rec[F_NORDERS] += P.S * P.orders_per_step;
+      if (s_ovf) { *P.host_flags = kFlagStatOverflow; __threadfence_system(); }
     }
     __syncthreads();
     if (tid < 16) grec[tid] = s_rec[tid];

@@ -68,7 +68,18 @@ struct KernelParams {
   int32_t paper_n_noise, paper_n_mom, paper_pmkt_q16;
   long long S;                                    // steps to run
   long long orders_per_step;                      // A + number of makers
+  // deferred checks (ks_api.cu): the depth bound of a ks_write_books whose result the host has not
+  // seen yet (DEVICE word, or NULL), the largest resting depth this run tolerates, and the sticky
+  // error flags in MAPPED HOST memory (written on an overflow only)
+  const unsigned long long* depth_word;
+  unsigned long long depth_limit;
+  unsigned long long* host_flags;
+  uint32_t rel_stride, rel_side;                  // ks_decoupled_kernel: bytes of ONE relative histogram buffer
+                                                  // (sell bins then buy bins) and of one side of it
 };
+
+// sticky error flags raised by the kernels (host_flags)
+enum : unsigned long long { kFlagStatOverflow = 1ull, kFlagDepthOverflow = 2ull, kFlagNegativeDepth = 4ull };
 
 // u32 x u32 -> u64 as ONE mul.wide.u32 (IMAD.WIDE.U32).  Written as PTX because the compiler,
 // given (uint64_t)a * b with a loop-invariant b, hoists the zero-extension of b and then emits a
@@ -273,7 +284,24 @@ struct RuleCtx {
   uint32_t bid_last, ask_last;   // shared addresses of bid[last], ask[last] (MIX3 no-clamp paths)
   int mid2;              // model 4: doubled mid price of the resting book (Eq.3); dp = sgn(mid2 - previous mid2)
   int* mkt_flags;        // model 4: shared int[2], set when a marketable buy [0] / sell [1] was generated
+  uint32_t rel_s, rel_b; // ATOM 4 / 5: shared addresses of sell bin 0 and of buy bin n-1 of the relative order
+                         // histogram being filled (plus 4*lane for the lane-columned layout)
 };
+
+// ATOM 4 / 5 (ks_decoupled_kernel): a noise order goes into a PRICE-INDEPENDENT relative histogram
+// instead of the book: with o = the offset draw in [0, n), a sell adds to sell[o] and a buy to
+// buy[n-1-o], so that for BOTH sides bin i means tick (last - delta) + i (sell tick = last - delta
+// + o; buy tick = last + delta - o = last - delta + (n-1-o)).  Only the clearing warp turns bins
+// into ticks, when it merges the histogram into the book at the step's price (clamping to the
+// grid there).  Integer adds commute, so the combined book is the one the direct path builds.
+// ATOM 4: one int32 per bin (byte stride 4); ATOM 5: 32 lane columns per bin (byte stride 128,
+// column = lane = bank): the 32 atomics of a warp instruction never share a bank (SURVEY.md S7
+// "lane-columned relative histogram").  Same three instructions as the direct no-clamp path.
+template <int ATOM>
+__device__ __forceinline__ uint32_t rel_bin_addr(const RuleCtx& rc, uint32_t side_word, uint32_t o) {
+  constexpr int sh = ATOM == 4 ? 2 : 7;
+  return (int32_t)side_word < 0 ? rc.rel_b - (o << sh) : rc.rel_s + (o << sh);
+}
 
 // a1 noise rule.  o = mulhi(w1, n), n = 2*delta+1; sell tick = (last - delta) + o, buy tick =
 // last - (o - delta) = (last + delta) - o.  q = 1 + mulhi(w2, qmax) is the high word of
@@ -287,7 +315,9 @@ template <int ATOM, bool CLAMP>
 __device__ __forceinline__ void noise_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
                                             uint32_t w0, uint32_t w1, uint32_t w2, int& sink) {
   const int q = (int)hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend);
-  if (!CLAMP) {
+  if (ATOM == 4 || ATOM == 5) {
+    book_add_at<0>(book, rel_bin_addr<ATOM>(rc, w0, __umulhi(w1, (uint32_t)P.noise_n)), q, sink);
+  } else if (!CLAMP) {
     // three instructions: one compare and two multiply-adds of which one is predicated off
     const uint32_t o = __umulhi(w1, (uint32_t)P.noise_n);
     const uint32_t bid_hi = rc.bid_lo + (uint32_t)P.noise_n4 - 4u;            // &bid[last + delta]
@@ -349,7 +379,9 @@ __device__ __forceinline__ void noise_order_packed(const KernelParams& P, const 
   const uint64_t p2 = mul_wide_u32(lo32(p1), (uint32_t)P.noise_qmax);
   const int q = (int)hi32(p2) + 1;
   const uint32_t o = hi32(p1);
-  if (!CLAMP) {
+  if (ATOM == 4 || ATOM == 5) {
+    book_add_at<0>(book, rel_bin_addr<ATOM>(rc, lo32(p2), o), q, sink);
+  } else if (!CLAMP) {
     const uint32_t m = (uint32_t)((int32_t)lo32(p2) >> 31);
     const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
     const uint32_t base = rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top));
@@ -490,6 +522,31 @@ __device__ __forceinline__ void generate_class(const KernelParams& P, const Book
 #pragma unroll kGenUnroll
   for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, p0_inc.inc, p0_inc.a_step); }
   if (pl.extra) one(p0);
+}
+
+// The same for threads that own at most N <= 4 agents of the class, written for LATENCY (the
+// decoupled kernel on an underfilled GPU, where a generating thread holds 1-3 agents and the loop
+// above would run its dependent Philox chains one after the other): the N chains are computed
+// side by side, unconditionally, and only the atomic is predicated on the agent existing.
+template <int ATOM, int N>
+__device__ __forceinline__ void generate_class_rel_few(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                                       const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
+                                                       const P0Step& p0_inc, int& sink) {
+  const uint32_t n_mine = pl.n_uniform + (pl.extra ? 1u : 0u);
+  uint64_t p0 = pl.p0;
+  uint32_t addr[N];
+  int q[N];
+#pragma unroll
+  for (uint32_t e = 0; e < N; ++e) {
+    uint32_t w0, w1, w2;
+    philox_from_p0<true>(P, mu, u, p0, w0, w1, w2);
+    q[e] = (int)hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend);
+    addr[e] = rel_bin_addr<ATOM>(rc, w0, __umulhi(w1, (uint32_t)P.noise_n));
+    p0 = add64_alu(p0, p0_inc.inc);
+  }
+#pragma unroll
+  for (uint32_t e = 0; e < N; ++e)
+    if (e < n_mine) book_add_at<0>(book, addr[e], q[e], sink);
 }
 
 // PACKED4: one class of BLOCKS of four agents.  MIX = false: all noise.  MIX = true: the blocks of
@@ -716,12 +773,28 @@ struct LocalBook {
 //   S[p] = (asks of lower lanes)  + (own asks at ticks <= p)      Eq.1, prefix
 //   V = min(D, S); Vmax by REDUX max; p* = lowest tick attaining it
 //   residual: bid <- min(bid, max(0, D - Vmax)), ask <- min(ask, max(0, S - Vmax))
-// Also returns conservative bounds of the residual book inside the window (bmax: highest tick
-// with bid depth, else base-1; amin: lowest tick with ask depth, else base+32K).
+// Also returns, per lane, the candidates for the bounds of the residual book inside the window
+// (LaneBounds; reduce_bounds turns them into bmax: highest tick with bid depth, else base-1, and
+// amin: lowest tick with ask depth, else the end of the window).  The two reductions are kept out
+// of these functions so that the caller can publish the new price first (ks_kernel.cuh): nothing
+// on the step's critical path needs them.
 // ---------------------------------------------------------------------------------------------
-template <int K, class IO>
+struct LaneBounds { int lb, la; };     // highest own tick with bid depth (-1) / lowest with ask depth (INT_MAX)
+
+__device__ __forceinline__ void reduce_bounds(const LaneBounds& c, int base, int wend, int& bmax_new, int& amin_new) {
+  bmax_new = __reduce_max_sync(0xffffffffu, c.lb);
+  amin_new = __reduce_min_sync(0xffffffffu, c.la);
+  if (bmax_new < 0) bmax_new = base - 1;
+  if (amin_new == 0x7fffffff) amin_new = wend;
+}
+
+// INC: ib[j] / ia[j] are added to the loaded bid / ask depth of the lane's j-th tick before the
+// clearing (the decoupled kernel's incoming orders, fused into the scan instead of being merged
+// into the book first); the residual is then stored even when nothing traded.
+template <int K, class IO, bool INC = false>
 __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int lane,
-                                             int& vmax, int& pstar, int& bmax_new, int& amin_new) {
+                                             int& vmax, int& pstar, LaneBounds& lbnd,
+                                             const int* ib = nullptr, const int* ia = nullptr) {
   static_assert(K % 4 == 0, "K must be a multiple of 4 (16-byte shared-memory vectors)");
   const unsigned FULL = 0xffffffffu;
   const int tick0 = base + lane * K;
@@ -736,6 +809,10 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
     }
     b[4 * v] = vb.x; b[4 * v + 1] = vb.y; b[4 * v + 2] = vb.z; b[4 * v + 3] = vb.w;
     a[4 * v] = va.x; a[4 * v + 1] = va.y; a[4 * v + 2] = va.z; a[4 * v + 3] = va.w;
+  }
+  if (INC) {
+#pragma unroll
+    for (int j = 0; j < K; ++j) { b[j] += ib[j]; a[j] += ia[j]; }
   }
   int tb = 0, ta = 0;
 #pragma unroll
@@ -764,15 +841,17 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
   vmax = __reduce_max_sync(FULL, bestV);
   pstar = __reduce_min_sync(FULL, bestV == vmax ? bestp : 0x7fffffff);
   int lb = -1, la = 0x7fffffff;
-  if (vmax > 0) {
-    int Drun = D0 - vmax, Srun = S0 - vmax;
+  if (vmax > 0 || INC) {
+    if (vmax > 0) {
+      int Drun = D0 - vmax, Srun = S0 - vmax;
 #pragma unroll
-    for (int j = 0; j < K; ++j) {
-      Srun += a[j];
-      int nbid = min(b[j], max(0, Drun));
-      Drun -= b[j];
-      b[j] = nbid;
-      a[j] = min(a[j], max(0, Srun));
+      for (int j = 0; j < K; ++j) {
+        Srun += a[j];
+        int nbid = min(b[j], max(0, Drun));
+        Drun -= b[j];
+        b[j] = nbid;
+        a[j] = min(a[j], max(0, Srun));
+      }
     }
     if (in) {
 #pragma unroll
@@ -787,10 +866,7 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
     if (b[j] > 0) lb = tick0 + j;                      // ascending: the highest wins
     if (a[K - 1 - j] > 0) la = tick0 + K - 1 - j;      // descending: the lowest wins
   }
-  bmax_new = __reduce_max_sync(FULL, lb);
-  amin_new = __reduce_min_sync(FULL, la);
-  if (bmax_new < 0) bmax_new = base - 1;
-  if (amin_new == 0x7fffffff) amin_new = min(L, base + 32 * K);
+  lbnd.lb = lb; lbnd.la = la;
 }
 
 // a3-a5 for a window of at most 32 ticks starting at `base` (any alignment): one tick per lane, no
@@ -798,11 +874,12 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
 // chain is what bounds the step.  Same definitions as clear_window.
 template <class IO>
 __device__ __forceinline__ void clear_window1(const IO& io, int L, int base, int lane,
-                                              int& vmax, int& pstar, int& bmax_new, int& amin_new) {
+                                              int& vmax, int& pstar, LaneBounds& lbnd, int inc_b = 0, int inc_a = 0) {
   const unsigned FULL = 0xffffffffu;
   const int tick = base + lane;
   const bool in = tick < L;
-  int b = in ? io.ld1(0, tick) : 0, a = in ? io.ld1(1, tick) : 0;
+  const int b0 = in ? io.ld1(0, tick) : 0, a0 = in ? io.ld1(1, tick) : 0;
+  int b = b0 + inc_b, a = a0 + inc_a;   // inc: incoming orders fused into the scan (decoupled kernel), else 0
   int D = b, S = a;                     // inclusive suffix of bids / prefix of asks over lanes
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
@@ -815,15 +892,13 @@ __device__ __forceinline__ void clear_window1(const IO& io, int L, int base, int
   vmax = __reduce_max_sync(FULL, V);
   pstar = __reduce_min_sync(FULL, (V == vmax && vmax > 0) ? tick : 0x7fffffff);
   if (vmax > 0) {
-    const int nbid = min(b, max(0, D - vmax)), nask = min(a, max(0, S - vmax));
-    if (in && nbid != b) io.st1(0, tick, nbid);
-    if (in && nask != a) io.st1(1, tick, nask);
-    b = nbid; a = nask;
+    b = min(b, max(0, D - vmax));
+    a = min(a, max(0, S - vmax));
   }
-  bmax_new = __reduce_max_sync(FULL, b > 0 ? tick : -1);
-  amin_new = __reduce_min_sync(FULL, a > 0 ? tick : 0x7fffffff);
-  if (bmax_new < 0) bmax_new = base - 1;
-  if (amin_new == 0x7fffffff) amin_new = min(L, base + 32);
+  if (in && b != b0) io.st1(0, tick, b);
+  if (in && a != a0) io.st1(1, tick, a);
+  lbnd.lb = b > 0 ? tick : -1;
+  lbnd.la = a > 0 ? tick : 0x7fffffff;
 }
 
 // General window of any width: chunks of 128 ticks, three passes (total bid depth; profiles and
@@ -831,7 +906,7 @@ __device__ __forceinline__ void clear_window1(const IO& io, int L, int base, int
 // than 256 ticks.  Same definitions as clear_window.
 template <class IO>
 static __device__ __noinline__ void clear_generic(const IO& io, int L, int base, int top, int lane,
-                                           int& vmax, int& pstar, int& bmax_new, int& amin_new) {
+                                           int& vmax, int& pstar, LaneBounds& lbnd) {
   const unsigned FULL = 0xffffffffu;
   // pass 0: total bid depth of the window
   int tbsum = 0;
@@ -888,10 +963,7 @@ static __device__ __noinline__ void clear_generic(const IO& io, int L, int base,
       pstar = __reduce_min_sync(FULL, bestV == vmax ? bestp : 0x7fffffff);
     }
   }
-  bmax_new = __reduce_max_sync(FULL, lb);
-  amin_new = __reduce_min_sync(FULL, la);
-  if (bmax_new < 0) bmax_new = base - 1;
-  if (amin_new == 0x7fffffff) amin_new = min(L, top + 1);
+  lbnd.lb = lb; lbnd.la = la;
 }
 
 }  // namespace ks

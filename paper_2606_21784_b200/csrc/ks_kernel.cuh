@@ -29,33 +29,52 @@ __device__ __forceinline__ BookTotals block_reduce_totals(long long sb, long lon
   return r;
 }
 
-// a6: price state, statistics and trajectory hash -- executed by lane 0 of warp 0 on the
-// shared-memory copy of the record (include/kineticsim.h, ks_market_stats).
-__device__ __forceinline__ void update_record(long long* rec, int last, int vmax, int pstar, int& new_last) {
-  long long before = last;
-  unsigned long long x;
-  new_last = last;
-  if (vmax > 0) {
-    new_last = pstar;
-    rec[F_NTRADES] += 1;
-    rec[F_SUMVOL] += vmax;
-    rec[F_SUMPX] += pstar;
-    rec[F_SUMPX2] += (long long)pstar * pstar;
-    rec[F_SUMPXVOL] += (long long)pstar * vmax;
-    x = ((unsigned long long)(unsigned)vmax << 16) | (unsigned long long)(unsigned)pstar;
-  } else {
-    x = 0xFFFFull;
+// a6: price state, statistics and trajectory hash -- all sixteen fields of the record
+// (include/kineticsim.h, ks_market_stats) updated IN PARALLEL, lane f (f < 16) of the clearing warp
+// owning field f: one LDS.64, a handful of warp instructions with a dependency depth of ~8, one
+// STS.64 -- instead of fifteen dependent read-modify-writes by one lane.  The record stays in
+// shared memory between steps (holding it in registers across the generation loop costs that
+// loop four registers of its 64 and measured 2-7 % slower on C4 / C5).  Every additive field's
+// per-step increment is a product X*Y of two of {0, 1, traded, Vmax, pt, r, r^2} (pt = p* on a
+// trading step, else 0; r = last_after - last_before):
+//   steps 1*1   n_trades 1*traded   sum_vol 1*Vmax   sum_px 1*pt   sum_px2 pt*pt   sum_pxvol pt*Vmax
+//   sum_ret 1*r   sum_ret2 r*r   sum_ret3 r*r^2   sum_ret4 r^2*r^2   (others 0*0)
+// so a lane picks its two factors by a constant 3-bit code and does ONE 32x32->64 multiply-add.
+// f[12] last, f[13] prev and f[14] the trajectory hash are set, not added.  Signed overflow of any
+// additive field (only sum_ret3 / sum_ret4 can get there: (L-1)^4 * steps may pass 2^63 on a wide
+// grid) is detected exactly and raised as a sticky flag (KS_ERR_OVERFLOW, ks_api.cu).
+__device__ __forceinline__ int rec_pick(int code, int tr, int vmax, int pt, int r, int r2) {
+  // code: 0 zero, 1 one, 2 traded, 3 Vmax, 4 pt, 5 r, 6 r^2
+  const bool b0 = code & 1, b1 = code & 2, b2 = code & 4;
+  const int v01 = b0 ? 1 : 0, v23 = b0 ? vmax : tr, v45 = b0 ? r : pt;
+  const int lo = b1 ? v23 : v01, hi = b1 ? r2 : v45;
+  return b2 ? hi : lo;
+}
+
+// One step's record update by all lanes of the clearing warp.  prev_value is what f[13] receives
+// (the price before the step; model 4: the doubled mid the step started from).  *ovf_flag (shared)
+// is set when an additive field leaves int64.
+__device__ __forceinline__ void update_record_lanes(long long* rec, int* ovf_flag, int lane, int last, int vmax, int pstar,
+                                                    int prev_value) {
+  //                         field: 15 14 13 12 11 10  9  8  7  6  5  4  3  2  1  0
+  const unsigned long long XC = 0x0000006551441111ull;
+  const unsigned long long YC = 0x0000006655344321ull;
+  const int f = lane & 15;
+  const int xc = (int)((XC >> (4 * f)) & 7ull), yc = (int)((YC >> (4 * f)) & 7ull);
+  const int tr = vmax > 0 ? 1 : 0;
+  const int new_last = tr ? pstar : last;
+  const int pt = tr ? pstar : 0;
+  const int r = new_last - last, r2 = r * r;            // |r| < 2^15, r^2 < 2^30
+  const long long old = rec[f];
+  const long long inc = (long long)rec_pick(xc, tr, vmax, pt, r, r2) * (long long)rec_pick(yc, tr, vmax, pt, r, r2);
+  const long long sum = (long long)((unsigned long long)old + (unsigned long long)inc);
+  const unsigned long long x = tr ? (((unsigned long long)(unsigned)vmax << 16) | (unsigned long long)(unsigned)pstar) : 0xFFFFull;
+  const long long hash = (long long)(((unsigned long long)old ^ x) * kHashPrime);
+  const long long nv = f == F_HASH ? hash : (f == F_LAST ? (long long)new_last : (f == F_PREV ? (long long)prev_value : sum));
+  if (lane < 16) {
+    rec[f] = nv;
+    if (((old ^ sum) & (inc ^ sum)) < 0) *ovf_flag = 1;  // both operands of one sign, the sum of the other
   }
-  long long r = (long long)new_last - before;
-  long long r2 = r * r;
-  rec[F_SUMRET] += r;
-  rec[F_SUMRET2] += r2;
-  rec[F_SUMRET3] += r2 * r;
-  rec[F_SUMRET4] += r2 * r2;
-  rec[F_HASH] = (long long)(((unsigned long long)rec[F_HASH] ^ x) * kHashPrime);
-  rec[F_STEPS] += 1;
-  rec[F_PREV] = before;
-  rec[F_LAST] = new_last;
 }
 
 // The per-thread generation plan of a launch (MODEL 2 = the paper's agent model has its own).
@@ -68,22 +87,121 @@ __device__ __forceinline__ GenPlan<2> make_gen_plan<2>(const KernelParams& P, bo
   return gen_plan_paper(P, tid, T);
 }
 
-constexpr int kPipeEvents = 4;     // PIPE kernels: events per generating thread held in registers
-
 __device__ __forceinline__ int sign_of(int x) { return (x > 0) - (x < 0); }
+
+// Split-phase named barriers (PTX bar.arrive / bar.sync on barrier `id`, `n` participating
+// threads): the producer side of a phase only ARRIVES and goes on, the consumer side waits
+// (producer/consumer use as in the PTX ISA's bar.arrive example).  Used by ks_decoupled_kernel
+// only: inside ks_persistent_kernel's step loop they sit in a branch the compiler must treat as
+// divergent, and ptxas then stops keeping the Philox keys in uniform registers across the
+// generation loops (measured: +5 % instructions on C5) -- that kernel keeps __syncthreads().
+// The barrier id is an immediate: with an id in a register ptxas reserves all 16 hardware barriers
+// for the CTA (4 resident CTAs per SM at most).
+template <int ID> __device__ __forceinline__ void bar_sync(int n) { asm volatile("bar.sync %0, %1;" ::"n"(ID), "r"(n) : "memory"); }
+template <int ID> __device__ __forceinline__ void bar_arrive(int n) { asm volatile("bar.arrive %0, %1;" ::"n"(ID), "r"(n) : "memory"); }
+
+// ---- pieces shared by the kernels of this file ------------------------------------------------
+// Deferred depth check of ks_write_books (ks_api.cu): every CTA reads the same device word and
+// takes the same decision, so an unsafe run changes nothing at all.  Returns true = abort.
+__device__ __forceinline__ bool depth_check_aborts(const KernelParams& P, int* s_abort) {
+  if (!P.depth_word) return false;
+  if (threadIdx.x == 0) {
+    const unsigned long long b = *P.depth_word;
+    *s_abort = b > P.depth_limit;
+    if (b > P.depth_limit && blockIdx.x == 0) {
+      *P.host_flags = b == 0xffffffffffffffffull ? kFlagNegativeDepth : kFlagDepthOverflow;
+      __threadfence_system();
+    }
+  }
+  __syncthreads();
+  return *s_abort != 0;
+}
+
+// a0: state load (HBM -> shared) of one market's [2][L] book, skipped for a fresh (all-zero) book;
+// per-thread partial depth totals and extents of what was loaded.
+__device__ __forceinline__ void load_book(const KernelParams& P, int32_t* book, const int32_t* gbook, int L,
+                                          long long& sb0, long long& sa0, int& bmax, int& amin) {
+  const int tid = threadIdx.x, T = blockDim.x;
+  const int nvec = L / 2;                              // int4 vectors in the whole book
+  int4* sbook4 = reinterpret_cast<int4*>(book);
+  sb0 = 0; sa0 = 0; bmax = -1; amin = 0x7fffffff;
+  if (P.fresh) {
+    for (int i = tid; i < nvec; i += T) sbook4[i] = make_int4(0, 0, 0, 0);
+  } else {
+    const int4* gbook4 = reinterpret_cast<const int4*>(gbook);
+    const int nside = L / 4;
+    for (int i = tid; i < nvec; i += T) {
+      int4 v = __ldg(gbook4 + i);
+      sbook4[i] = v;
+      int vals[4] = {v.x, v.y, v.z, v.w};
+      if (i < nside) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { sb0 += vals[j]; if (vals[j] > 0) bmax = max(bmax, 4 * i + j); }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { sa0 += vals[j]; if (vals[j] > 0) amin = min(amin, 4 * (i - nside) + j); }
+      }
+    }
+  }
+}
+
+// a7: write-back (shared -> HBM) of the book with 16-byte vectors and of the 128-byte record; the
+// depth totals give sub_buy / sub_sell by conservation: submitted = (resting after - resting
+// before) + executed during this run (the oracle counts the same quantity order by order).
+// keep[3] = resting bid total, resting ask total, executed volume at the start of the run.
+__device__ __forceinline__ void store_state(const KernelParams& P, const int32_t* book, int32_t* gbook, long long* grec, int L,
+                                            long long* s_rec, const long long* keep, const int* s_ovf,
+                                            long long* s_red64, int* s_red32) {
+  const int tid = threadIdx.x, T = blockDim.x;
+  long long sb1 = 0, sa1 = 0;
+  {
+    const int nvec = L / 2, nside = L / 4;
+    const int4* sbook4 = reinterpret_cast<const int4*>(book);
+    int4* gbook4 = reinterpret_cast<int4*>(gbook);
+    for (int i = tid; i < nvec; i += T) {
+      int4 v = sbook4[i];
+      gbook4[i] = v;
+      long long sum = (long long)v.x + v.y + v.z + v.w;
+      if (i < nside) sb1 += sum; else sa1 += sum;
+    }
+  }
+  BookTotals tot1 = block_reduce_totals(sb1, sa1, -1, 0x7fffffff, s_red64, s_red32);
+  if (tid == 0) {
+    long long dvol = s_rec[F_SUMVOL] - keep[2];
+    s_rec[F_SUBBUY] += (tot1.sum_bid - keep[0]) + dvol;
+    s_rec[F_SUBSELL] += (tot1.sum_ask - keep[1]) + dvol;
+    s_rec[F_NORDERS] += P.S * P.orders_per_step;
+    if (*s_ovf) { *P.host_flags = kFlagStatOverflow; __threadfence_system(); }
+  }
+  __syncthreads();
+  if (tid < 16) grec[tid] = s_rec[tid];
+}
+
+// a3-a5 on the active window [lo, hi] of a book in this CTA's shared memory, by one warp: picks
+// the scan by the window's width.  base / wend = the tick range the chosen scan covered.
+__device__ __forceinline__ void clear_active_window(const LocalBook& io, int L, int lo, int hi, bool force_generic, int lane,
+                                                    int& vmax, int& pstar, LaneBounds& lbnd, int& base, int& wend) {
+  const int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
+  if (force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, lbnd); }
+  else if (hi - lo < 32)             { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, lbnd); }
+  else if (width4 <= 128)            { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, lbnd); }
+  else                               { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, lbnd); }
+}
 
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
 // dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3, 2 = the paper's agent
 // model (mid-price reference, A24).  ATOM: see book_add.
 // PACKED: the PACKED4 draw contract (one Philox block per four agents, A22).
-// PIPE (MODEL 0, ATOM 0, literal contract, few markets): software pipeline for the latency-bound
-// regime (C3).  The Philox words of a step do not depend on the price, only the address does: warp 0
-// holds no agents and only clears; while it clears step s, the other warps draw (offset, side,
-// quantity) of step s+1 into registers (at most 4 events per thread), and after the barrier they
-// only compute addresses and issue the atomics.  Same orders, same bytes.
+//
+// Step structure (Alg.1 phases): a1+a2 by all warps | barrier | a3-a6 by ONE
+// clearing warp | barrier.  The clearing warp is warp (blockIdx mod #warps): warps map to the SM's
+// four schedulers by index, so a fixed warp 0 would pile every resident market's clearing on one
+// scheduler.  This is the throughput kernel (many markets per SM hide each other's clearing; the
+// automatic plan runs it with ONE warp per market on C4); when the grid underfills the GPU the
+// step latency counts and ks_decoupled_kernel takes over.
 // ---------------------------------------------------------------------------------------------
-template <int MODEL, int ATOM, bool PACKED, bool PIPE = false>
+template <int MODEL, int ATOM, bool PACKED>
 __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_constant__ KernelParams P) {
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask
   __shared__ long long s_rec[16];
@@ -93,50 +211,35 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   __shared__ __align__(16) int s_ctl[4];              // per-step broadcast: last, &bid[last-delta], &ask[last-delta], noclamp
                                                       // (MODEL 2: last, mid2, sgn(mid2 - previous mid2), 0)
   __shared__ int s_mkt[2];                            // MODEL 2: a marketable buy / sell was generated this step
+  __shared__ int s_abort;
+  __shared__ int s_ovf;                               // an int64 statistic overflowed (sticky)
+  __shared__ long long s_keep[3];                     // resting totals and executed volume at the start of the run:
+                                                      // parked here so that they hold no registers during the S steps
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5;
   const int L = P.L;
+  const bool clearing = warp == (int)(blockIdx.x % (unsigned)(T >> 5));   // the clearing warp of this market
   const uint32_t market = P.market_base + blockIdx.x;
   int32_t* gbook = P.books + (size_t)blockIdx.x * 2 * (size_t)L;
   long long* grec = P.recs + (size_t)blockIdx.x * 16;
+  if (depth_check_aborts(P, &s_abort)) return;
   const MarketUniform mu = market_uniform(P, market);
-
-  const GenPlan<MODEL> gplan = PIPE ? gen_plan<MODEL>(warp > 0 ? (uint32_t)P.A : 0u, tid >= 32 ? tid - 32 : 0, T - 32)
-                                    : make_gen_plan<MODEL>(P, PACKED, tid, T);
+  const GenPlan<MODEL> gplan = make_gen_plan<MODEL>(P, PACKED, tid, T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
 
-  // ---- a0: state load (HBM -> shared), skipped for a fresh (all-zero) book
-  long long sb0 = 0, sa0 = 0;
-  int bmax = -1, amin = 0x7fffffff;
-  {
-    const int nvec = L / 2;                            // int4 vectors in the whole book
-    int4* sbook4 = reinterpret_cast<int4*>(book);
-    if (P.fresh) {
-      for (int i = tid; i < nvec; i += T) sbook4[i] = make_int4(0, 0, 0, 0);
-    } else {
-      const int4* gbook4 = reinterpret_cast<const int4*>(gbook);
-      const int nside = L / 4;
-      for (int i = tid; i < nvec; i += T) {
-        int4 v = __ldg(gbook4 + i);
-        sbook4[i] = v;
-        int vals[4] = {v.x, v.y, v.z, v.w};
-        if (i < nside) {
-#pragma unroll
-          for (int j = 0; j < 4; ++j) { sb0 += vals[j]; if (vals[j] > 0) bmax = max(bmax, 4 * i + j); }
-        } else {
-#pragma unroll
-          for (int j = 0; j < 4; ++j) { sa0 += vals[j]; if (vals[j] > 0) amin = min(amin, 4 * (i - nside) + j); }
-        }
-      }
-    }
-    if (tid < 16) s_rec[tid] = grec[tid];
-  }
+  // ---- a0
+  long long sb0, sa0;
+  int bmax, amin;
+  load_book(P, book, gbook, L, sb0, sa0, bmax, amin);
+  if (tid < 16) s_rec[tid] = grec[tid];
+  if (tid == 0) s_ovf = 0;
   BookTotals tot0 = block_reduce_totals(sb0, sa0, bmax, amin, s_red64, s_red32);   // has barriers
-  bmax = tot0.bmax;                       // only warp 0 keeps these up to date below
+  bmax = tot0.bmax;                       // only the clearing warp keeps these up to date below
   amin = min(tot0.amin, L);
   int last = (int)s_rec[F_LAST], prev = (int)s_rec[F_PREV];
   const uint32_t t0 = (uint32_t)s_rec[F_STEPS];
-  const long long vol0 = s_rec[F_SUMVOL];
+  const uint32_t S = (uint32_t)P.S;                   // ks_run guarantees steps_done + S < 2^32
+  if (tid == 0) { s_keep[0] = tot0.sum_bid; s_keep[1] = tot0.sum_ask; s_keep[2] = s_rec[F_SUMVOL]; }
 
   int sink = 0;                           // only used by the ATOM == 2 microbenchmark variant
   auto publish = [&](int new_last) {      // one thread: the rule context of the next step
@@ -154,12 +257,12 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
     else publish(last);
   }
   __syncthreads();
-  // a3-a6: clearing by warp 0 on the active window (called by warp 0 only)
-  auto clear_step = [&](long long s, const RuleCtx& rc) {
+  // a3-a6: clearing by the clearing warp on the active window
+  auto clear_step = [&](uint32_t s, int mid2_now) {
     int lo, hi;
     if (MODEL == 2) {
-      lo = max(0, min(amin, (rc.mid2 >> 1) - P.dmax));
-      hi = min(L - 1, max(bmax, ((rc.mid2 + 1) >> 1) + P.dmax));
+      lo = max(0, min(amin, (mid2_now >> 1) - P.dmax));
+      hi = min(L - 1, max(bmax, ((mid2_now + 1) >> 1) + P.dmax));
       if (s_mkt[0]) hi = L - 1;                      // marketable buys sit at tick L-1,
       if (s_mkt[1]) lo = 0;                          // marketable sells at tick 0
       __syncwarp();
@@ -167,141 +270,57 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
       lo = max(0, min(amin, last - P.dmax));
       hi = min(L - 1, max(bmax, last + P.dmax));
     }
-    int vmax, pstar, nb, na, base, wend;
-    int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
+    int vmax, pstar, base, wend, nb, na;
+    LaneBounds lbnd;
     const LocalBook io{book, L};
-    if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, nb, na); }
-    else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, nb, na); }
-    else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, nb, na); }
-    else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, nb, na); }
+    clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
+    reduce_bounds(lbnd, base, wend, nb, na);
     if (MODEL == 2) {
       // the mid price needs the EXACT best quotes: a side with no depth inside the window is
       // searched outside it (rare: the window was emptied on that side)
       if (nb < base) nb = best_bid_below(io, L, base, lane);
       if (na >= wend) na = best_ask_from(io, L, wend, lane);
+      if (lane == 0) { publish_paper(vmax > 0 ? pstar : last, nb, na, mid2_now); s_mkt[0] = 0; s_mkt[1] = 0; }
+    } else {
+      if (lane == 0) publish(vmax > 0 ? pstar : last);
     }
     bmax = nb; amin = na;
-    if (lane == 0) {
-      int new_last;
-      update_record(s_rec, last, vmax, pstar, new_last);
-      if (MODEL == 2) {
-        s_rec[F_PREV] = rc.mid2;
-        publish_paper(new_last, nb, na, rc.mid2);
-        s_mkt[0] = 0; s_mkt[1] = 0;
-      } else {
-        publish(new_last);
-      }
-    }
-    if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)P.S, s, P.S, lane,
+    update_record_lanes(s_rec, &s_ovf, lane, last, vmax, pstar, MODEL == 2 ? mid2_now : last);
+    if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)s, (long long)S, lane,
                             vmax > 0 ? pstar : last, vmax);
   };
   // ---- S steps, all on-chip
-  if constexpr (PIPE) {
-    // per-thread draws of ONE step: the offset index o = mulhi(w1, n), and q with the side bit of
-    // w0 in its top bit (q <= 2^20 + 1).  At most kPipeEvents events per thread (host plan).
-    uint32_t dr_o[kPipeEvents], dr_q[kPipeEvents];
-    const int n_mine = (int)gplan.cls[0].n_uniform + (gplan.cls[0].extra ? 1 : 0);
-    auto draw = [&](uint32_t t) {
-      const StepUniform u = step_uniform(P, mu, t);
-      uint64_t p0 = gplan.cls[0].p0;
-#pragma unroll
-      for (int e = 0; e < kPipeEvents; ++e) {
-        if (e < n_mine) {
-          uint32_t w0, w1, w2;
-          philox_from_p0<true>(P, mu, u, p0, w0, w1, w2);
-          dr_o[e] = __umulhi(w1, (uint32_t)P.noise_n);
-          dr_q[e] = hi32((uint64_t)w2 * (uint32_t)P.noise_qmax + P.q_addend) | (w0 & 0x80000000u);
-          p0 = add64_alu(p0, gplan.p0_inc.inc);
-        }
-      }
-    };
-    if (P.S > 0) draw(t0);
-    for (long long s = 0; s < P.S; ++s) {
-      const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
-      last = ctl.x;
-      RuleCtx rc;
-      rc.last = last; rc.L = L; rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
-      rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
-      rc.bid_last = 0; rc.ask_last = 0;
-      // a2: the orders drawn during the previous clearing go to their ticks
-#pragma unroll
-      for (int e = 0; e < kPipeEvents; ++e) {
-        if (e < n_mine) {
-          const uint32_t m = (uint32_t)((int32_t)dr_q[e] >> 31), o = dr_o[e];
-          const int q = (int)(dr_q[e] & 0x7fffffffu);
-          if (rc.noclamp) {
-            const uint32_t bid_top = rc.bid_lo + (uint32_t)P.noise_n4;
-            book_add_at<ATOM>(bref, (rc.ask_lo ^ (m & (rc.ask_lo ^ bid_top))) + ((o ^ m) << 2), q, sink);
-          } else {
-            const bool buy = m != 0u;
-            const int tick = clamp_tick(buy ? (last + P.noise_delta) - (int)o : (last - P.noise_delta) + (int)o, L);
-            book_add<ATOM>(bref, 4u * (uint32_t)(buy ? tick : tick + L), q, sink);
-          }
-        }
-      }
-      __syncthreads();                                   // B1: the combined book is complete
-      if (warp == 0) clear_step(s, rc);                  // a3-a6 ...
-      else if (s + 1 < P.S) draw(t0 + (uint32_t)s + 1u); // ... while the other warps draw the next step (a1)
-      __syncthreads();                                   // B2: residual book and new price visible
-      prev = last;
-    }
-  } else {
-    for (long long s = 0; s < P.S; ++s) {
-      const uint32_t t = t0 + (uint32_t)s;
-      const StepUniform u = step_uniform(P, mu, t);
-      const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
-      last = ctl.x;
-      RuleCtx rc;
-      rc.last = last; rc.L = L;
-      if constexpr (MODEL == 2) {
-        rc.mid2 = ctl.y; rc.dp = ctl.z; rc.mkt_flags = s_mkt;
+  for (uint32_t s = 0; s < S; ++s) {
+    const uint32_t t = t0 + s;
+    const StepUniform u = step_uniform(P, mu, t);
+    const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
+    last = ctl.x;
+    RuleCtx rc;
+    rc.last = last; rc.L = L;
+    if constexpr (MODEL == 2) {
+      rc.mid2 = ctl.y; rc.dp = ctl.z; rc.mkt_flags = s_mkt;
       {                                                // no-clamp path: midr +- dmax inside the grid
         const int midr = (rc.mid2 + 1) >> 1;
         rc.noclamp = midr - P.dmax >= 0 && midr + P.dmax <= L - 1;
         rc.bid_last = bref.saddr + 4u * (uint32_t)midr; rc.ask_last = rc.bid_last + 4u * (uint32_t)L;
         rc.bid_lo = rc.bid_last - 4u * (uint32_t)P.noise_delta; rc.ask_lo = rc.ask_last - 4u * (uint32_t)P.noise_delta;
       }
-        generate_step_paper<ATOM>(P, bref, mu, u, rc, gplan, tid, t, sink);
-      } else {
-        rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
-        rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
-        rc.bid_last = rc.bid_lo + 4u * (uint32_t)P.noise_delta; rc.ask_last = rc.ask_lo + 4u * (uint32_t)P.noise_delta;
-        // a1 + a2: order generation and aggregation
-        generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
-      }
-      __syncthreads();                                   // B1: the combined book is complete
-
-      if (warp == 0) clear_step(s, rc);
-      __syncthreads();                                   // B2: residual book and new price visible
-      prev = last;
+      generate_step_paper<ATOM>(P, bref, mu, u, rc, gplan, tid, t, sink);
+    } else {
+      rc.dp = last - prev; rc.mid2 = 0; rc.mkt_flags = nullptr;
+      rc.bid_lo = (uint32_t)ctl.y; rc.ask_lo = (uint32_t)ctl.z; rc.noclamp = ctl.w != 0;
+      rc.bid_last = rc.bid_lo + 4u * (uint32_t)P.noise_delta; rc.ask_last = rc.ask_lo + 4u * (uint32_t)P.noise_delta;
+      // a1 + a2: order generation and aggregation
+      generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
     }
-
+    __syncthreads();                                   // B1: the combined book is complete
+    if (clearing) clear_step(s, rc.mid2);
+    __syncthreads();                                   // B2: residual book and new price visible
+    prev = last;
   }
 
-  // ---- a7: write-back (shared -> HBM), 16-byte vectors, plus the totals for sub_buy/sub_sell
-  long long sb1 = 0, sa1 = 0;
-  {
-    const int nvec = L / 2, nside = L / 4;
-    const int4* sbook4 = reinterpret_cast<const int4*>(book);
-    int4* gbook4 = reinterpret_cast<int4*>(gbook);
-    for (int i = tid; i < nvec; i += T) {
-      int4 v = sbook4[i];
-      gbook4[i] = v;
-      long long sum = (long long)v.x + v.y + v.z + v.w;
-      if (i < nside) sb1 += sum; else sa1 += sum;
-    }
-  }
-  BookTotals tot1 = block_reduce_totals(sb1, sa1, -1, 0x7fffffff, s_red64, s_red32);
-  if (tid == 0) {
-    // submitted = (resting after - resting before) + executed during this run (conservation;
-    // the oracle counts the same quantity order by order)
-    long long dvol = s_rec[F_SUMVOL] - vol0;
-    s_rec[F_SUBBUY] += (tot1.sum_bid - tot0.sum_bid) + dvol;
-    s_rec[F_SUBSELL] += (tot1.sum_ask - tot0.sum_ask) + dvol;
-    s_rec[F_NORDERS] += P.S * P.orders_per_step;
-  }
-  __syncthreads();
-  if (tid < 16) grec[tid] = s_rec[tid];
+  // ---- a7
+  store_state(P, book, gbook, grec, L, s_rec, s_keep, &s_ovf, s_red64, s_red32);
 }
 
 // ks_create: empty books, opening price, zero accumulators (Alg.1 l.2-3).

@@ -1,4 +1,8 @@
-// ks_microbench.cu -- roofline microbenchmarks declared in include/kineticsim_bench.h.
+// ks_microbench.cu -- libkineticsim_bench.so: the ablation entry point and the roofline
+// microbenchmarks declared in include/kineticsim_bench.h.  A separate library from the product
+// (libkineticsim.so, which never allocates device memory): these calls allocate a few bytes of
+// device scratch for themselves and time their own kernels.
+// (0) the launch-per-step ablation, through the product's public ks_run,
 // (1) shared-memory atomic ceilings, (2) generation-only (Philox + rule) ceiling built from the
 // library's own device templates, (3) raw IMAD.WIDE / LOP3 issue rates.
 #include "../../include/kineticsim_bench.h"
@@ -98,6 +102,30 @@ __global__ void int_pipe_kernel(int iters, uint32_t seed, uint32_t* out) {
   if (acc == 0x12345678u) out[0] = acc;
 }
 
+// KIND 5: a pure stream of mul.wide.u32 (IMAD.WIDE.U32 with no addend), 8 independent chains per
+// thread, each feeding the high word of its product back in -- nothing but 32x32->64 multiplies
+// on the fmaheavy pipe: the MEASURED peak the hot loop's multiplies are reported against.
+__global__ void mul_wide_kernel(int iters, uint32_t seed, uint32_t* out) {
+  uint32_t c[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) c[j] = seed + threadIdx.x * 8u + j;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        uint64_t p;
+        asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(c[j]), "r"(ks::kPhiloxM0));
+        c[j] = (uint32_t)(p >> 32);
+      }
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) acc ^= c[j];
+  if (acc == 0x12345678u) out[0] = acc;
+}
+
 template <typename F>
 ks_status time_best(F launch, int warmup, int reps, cudaStream_t st, double* seconds) {
   cudaEvent_t e0, e1;
@@ -129,6 +157,16 @@ int num_sms() {
 }  // namespace
 
 extern "C" {
+
+// a8 ablation: the product's own ks_run, one launch per step, book through HBM between launches.
+ks_status ks_run_stepwise(ks_sim* s, int64_t S, void* stream) {
+  if (!s || S < 0) return KS_ERR_INVALID_ARG;
+  for (int64_t i = 0; i < S; ++i) {
+    ks_status r = ks_run(s, 1, stream);
+    if (r != KS_OK) return r;
+  }
+  return KS_OK;
+}
 
 ks_status ks_bench_smem_atomic(int32_t mode, int32_t delta, int32_t L, int32_t threads, int32_t ctas_per_sm,
                                int32_t iters, int32_t warmup, int32_t reps, void* stream, double* lane_ops_per_s,
@@ -201,7 +239,7 @@ ks_status ks_bench_generate_only(const ks_agent_params* p, int32_t M, int32_t L,
 
 ks_status ks_bench_int_pipe(int32_t kind, int32_t threads, int32_t ctas_per_sm, int32_t iters, int32_t warmup,
                             int32_t reps, void* stream, double* thread_ops_per_s, double* seconds) {
-  if (!thread_ops_per_s || !seconds || kind < 0 || kind > 4 || threads < 32 || threads > 1024 || threads % 32 ||
+  if (!thread_ops_per_s || !seconds || kind < 0 || kind > 5 || threads < 32 || threads > 1024 || threads % 32 ||
       ctas_per_sm < 1 || iters < 1 || reps < 1)
     return KS_ERR_INVALID_ARG;
   const int sms = num_sms();
@@ -215,12 +253,13 @@ ks_status ks_bench_int_pipe(int32_t kind, int32_t threads, int32_t ctas_per_sm, 
     else if (kind == 1) int_pipe_kernel<1><<<grid, threads, 0, st>>>(iters, 7u, d_out);
     else if (kind == 2) int_pipe_kernel<2><<<grid, threads, 0, st>>>(iters, 7u, d_out);
     else if (kind == 3) int_pipe_kernel<3><<<grid, threads, 0, st>>>(iters, 7u, d_out);
-    else                int_pipe_kernel<4><<<grid, threads, 0, st>>>(iters, 7u, d_out);
+    else if (kind == 4) int_pipe_kernel<4><<<grid, threads, 0, st>>>(iters, 7u, d_out);
+    else                mul_wide_kernel<<<grid, threads, 0, st>>>(iters, 7u, d_out);
   };
   ks_status rc = time_best(launch, warmup, reps, st, seconds);
   cudaFree(d_out);
   if (rc != KS_OK) return rc;
-  const double per_iter = (kind == 0 ? 1.0 : (kind <= 2 ? 2.0 : (kind == 3 ? 3.0 : 4.0))) * 32.0;   // ops per thread per iteration
+  const double per_iter = (kind == 0 || kind == 5 ? 1.0 : (kind <= 2 ? 2.0 : (kind == 3 ? 3.0 : 4.0))) * 32.0;   // ops per thread per iteration
   *thread_ops_per_s = (double)grid * threads * (double)iters * per_iter / *seconds;
   return KS_OK;
 }

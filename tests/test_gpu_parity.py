@@ -87,7 +87,7 @@ def test_block_sizes_atomic_modes_and_clear_paths_give_identical_bytes(ks, oracl
     for T in (32, 64, 96, 128, 256, 512, 1024):
         for atom in (0, 1):
             for clear in (0, 1):
-                if T not in (96, 256) and (atom or clear):
+                if T not in (32, 96, 256, 1024) and (atom or clear):
                     continue
                 b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T),
                                                             (ks.KS_OPT_ATOMIC_MODE, atom),
@@ -95,33 +95,58 @@ def test_block_sizes_atomic_modes_and_clear_paths_give_identical_bytes(ks, oracl
                 assert_rows_equal(b, r, ids, eb, er, "T=%d atom=%d clear=%d" % (T, atom, clear))
 
 
-def test_pipelined_step_loop_gives_identical_bytes(ks, oracle):
-    """KS_OPT_PIPELINE: the next step's Philox draws overlap the clearing (warp 0 holds no agents).
-    Forced on (2) and off (1) for several block sizes and ragged agent counts, prices pinned to the
-    grid edges (clamp path), split and launch-per-step runs, the trace: always the oracle's bytes."""
+def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
+    """KS_OPT_PIPELINE: ks_decoupled_kernel -- generating warps fill a price-independent relative
+    order histogram (double-buffered, up to two steps ahead), one clearing warp per market merges
+    it at the step's price.  Forced on (2) and off (1) for several block sizes and ragged agent
+    counts, plain bins and the 32-lane-column layout, literal and PACKED4 draws, prices pinned to the
+    grid edges (the clamp happens at the merge), split and launch-per-step runs, S = 1, 2, 3 (the
+    double buffer's corner cases), the trace: always the oracle's bytes."""
     import torch
     L, seed, S = 128, 2, 150
     p = zi_params(8, 10)
-    for M, A, T in [(5, 512, 512), (5, 500, 256), (3, 97, 64), (4, 33, 96), (2, 0, 128), (3, 1900, 512), (2, 1984, 1024)]:
+    # M > #warps makes every warp index the clearing warp of some market (clearing warp = market mod #warps)
+    for M, A, T in [(5, 512, 512), (5, 500, 256), (3, 97, 64), (4, 33, 96), (2, 0, 128), (3, 1900, 512), (2, 1984, 1024),
+                    (7, 1024, 160), (6, 1024, 128), (9, 1000, 96), (5, 3000, 224), (11, 4096, 1024), (3, 4096, 288)]:
         ids = np.arange(M)
         eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
-        for pipe in (2, 1):
-            b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, pipe)])
-            assert_rows_equal(b, r, ids, eb, er, "pipeline=%d A=%d T=%d" % (pipe, A, T))
+        for pipe, cols in ((2, 0), (2, 1), (1, 0)):
+            b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, pipe),
+                                                        (ks.KS_OPT_REL_COLUMNS, cols)])
+            assert_rows_equal(b, r, ids, eb, er, "decoupled=%d cols=%d A=%d T=%d" % (pipe, cols, A, T))
+    pk = packed4(zi_params(16, 100))
+    for M, A, T in [(6, 1001, 128), (5, 3, 64), (7, 4096, 288)]:
+        eb, er = oracle_rows(oracle, pk, 256, A, 9, np.arange(M), 70)
+        for cols in (0, 1):
+            b, r = _gpu(ks, M, 256, A, pk, 9, 70, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, 2),
+                                                        (ks.KS_OPT_REL_COLUMNS, cols)])
+            assert_rows_equal(b, r, np.arange(M), eb, er, "decoupled packed4 cols=%d A=%d T=%d" % (cols, A, T))
     M, A, T = 4, 480, 256
     ids = np.arange(M)
     for init in (0, L - 1, 4):
         q = dict(p, init_price=init)
         eb, er, et = oracle.run_markets_traced(q, L, A, seed, ids, 60)
-        for kw in (dict(), dict(split=[1, 29, 30]), dict(stepwise=True)):
-            b, r = _gpu(ks, M, L, A, q, seed, 60, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, 2)], **kw)
-            assert_rows_equal(b, r, ids, eb, er, "pipeline init=%d %r" % (init, kw))
+        for kw in (dict(), dict(split=[1, 29, 30]), dict(split=[2, 3, 55]), dict(stepwise=True)):
+            for cols in (0, 1):
+                b, r = _gpu(ks, M, L, A, q, seed, 60, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, 2),
+                                                            (ks.KS_OPT_REL_COLUMNS, cols)], **kw)
+                assert_rows_equal(b, r, ids, eb, er, "decoupled init=%d cols=%d %r" % (init, cols, kw))
         sim = ks.KsSim(M, L, A, q, seed)
         sim.ks_set_option(ks.KS_OPT_BLOCK_THREADS, T); sim.ks_set_option(ks.KS_OPT_PIPELINE, 2)
         tr = torch.empty((M, 60, 2), dtype=torch.int32, device="cuda")
         sim.ks_run_traced(60, tr)
         assert np.array_equal(tr.cpu().numpy(), et)
         sim.ks_destroy()
+    # injected crossed books + a wide offset range (2 x 257 bins, several merge rounds)
+    M, L2, A = 5, 1024, 700
+    pw = zi_params(128, 30)
+    books = random_books(M, L2, seed=11, max_qty=40, fill=0.2)
+    eb0, er0 = oracle.init_state(M, L2, -1)
+    eb, er = oracle_rows(oracle, pw, L2, A, 3, np.arange(M), 25, books=books, recs=er0)
+    for cols in (0, 1):
+        b, r = _gpu(ks, M, L2, A, pw, 3, 25, books=books, opts=[(ks.KS_OPT_BLOCK_THREADS, 192), (ks.KS_OPT_PIPELINE, 2),
+                                                                (ks.KS_OPT_REL_COLUMNS, cols)])
+        assert_rows_equal(b, r, np.arange(M), eb, er, "decoupled injected cols=%d" % cols)
 
 
 def test_split_run_and_stepwise_ablation_are_bit_identical(ks, oracle):
@@ -184,24 +209,171 @@ def test_cluster_path_gives_identical_bytes(ks, oracle, model):
 def test_book_larger_than_one_sm(ks, oracle):
     """L = 32768: 256 KB of book per market, more than one SM's shared memory -> the automatic
     plan runs a 2-CTA cluster.  Opening price at the CTA boundary (L/2), so orders and the
-    clearing window straddle both CTAs' shared memory.  (The conservative int64 guard on the
-    fourth return moment, (L-1)^4 * steps < 2^63, allows 8 steps per record at this L.)"""
-    M, L, A, S, seed = 6, 32768, 3000, 8, 21
+    clearing window straddle both CTAs' shared memory.  S = 1000 steps: the a-priori
+    (L-1)^4 * steps < 2^63 guard of round 1 (8 steps at this L) is gone -- the int64 sums are
+    checked exactly on the device, and these runs stay far inside them."""
+    M, L, A, S, seed = 4, 32768, 300, 1000, 21
     p = zi_params(64, 50)
     ids = np.arange(M)
     eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
-    b, r = _gpu(ks, M, L, A, p, seed, S)
-    assert_rows_equal(b, r, ids, eb, er, "L=32768 auto cluster")
+    b, r = _gpu(ks, M, L, A, p, seed, S, split=[400, 600])
+    assert_rows_equal(b, r, ids, eb, er, "L=32768 auto cluster, S=1000")
     pm = mix3_params()
     books = random_books(M, L, seed=5, max_qty=30, fill=0.05)
     eb0, er0 = oracle.init_state(M, L, -1)
-    eb, er = oracle_rows(oracle, pm, L, 900, seed, ids, 5, books=books, recs=er0)
-    b, r = _gpu(ks, M, L, 900, pm, seed, 5, books=books, split=[2, 3])
+    eb, er = oracle_rows(oracle, pm, L, 900, seed, ids, 40, books=books, recs=er0)
+    b, r = _gpu(ks, M, L, 900, pm, seed, 40, books=books, split=[2, 38])
     assert_rows_equal(b, r, ids, eb, er, "L=32768 mix3 injected")
-    sim = ks.KsSim(1, L, 10, p, 0)
-    with pytest.raises(ks.KsError):
-        sim.ks_run(9)                                  # KS_ERR_OVERFLOW, nothing enqueued
+
+
+def test_large_price_moves_reach_the_int64_limit_exactly(ks, oracle):
+    """The sum of r^4 (f[9]) is the statistic that can leave int64 on a wide grid.  A = 0 and
+    injected crossed quotes (ks_write_books before every step) make the price jump between tick 10
+    and tick 32700 of an L = 32768 grid: the first jump from L/2 adds 16374^4, each later one
+    32690^4 = 1.142e18.  After 1 + 8 jumps the sum is 9.208e18 < 2^63 = 9.223e18 and every byte
+    still equals the oracle's (whose int64 sums have not overflowed either); the next jump leaves
+    int64, the kernel raises the sticky flag and the handle returns KS_ERR_OVERFLOW from then on."""
+    import torch
+    M, L, seed, p = 3, 32768, 1, zi_params(8, 10)
+    ids = np.arange(M)
+
+    def quotes(k):
+        b = np.zeros((M, 2, L), dtype=np.int32)
+        lo, hi = (10, 32700) if k % 2 == 0 else (32700, 32750)     # ask at lo, bid at hi: V = q on [lo, hi], p* = lo
+        b[:, 1, lo] = 5 + np.arange(M); b[:, 0, hi] = 5 + np.arange(M)
+        return b
+
+    sim = ks.KsSim(M, L, 0, p, seed)
+    eb, er = oracle.init_state(M, L, -1)
+    for k in range(9):
+        sim.ks_write_books(torch.from_numpy(quotes(k)).cuda())
+        sim.ks_run(1)
+        eb, er = oracle.run_markets(p, L, 0, seed, ids.astype(np.uint32), 1, quotes(k), er)
+    torch.cuda.synchronize()
+    sim.ks_error_state()
+    assert_rows_equal(sim.books_to_host(), sim.stats_to_host(), ids, eb, er, "nine jumps")
+    assert (er[:, 12] == 10).all() and (er[:, 9] == 16374 ** 4 + 8 * 32690 ** 4).all() and (er[:, 9] > 0.998 * 2 ** 63).all()
+    sim.ks_write_books(torch.from_numpy(quotes(9)).cuda())
+    sim.ks_run(1)
+    torch.cuda.synchronize()
+    for call in (sim.ks_error_state, lambda: sim.ks_run(1), sim.stats_to_host):
+        with pytest.raises(ks.KsError) as e:
+            call()
+        assert e.value.status == ks.KS_ERR_OVERFLOW
     sim.ks_destroy()
+
+
+def test_single_cta_maximum_grid_long_run(ks, oracle):
+    """L = 16384 (the single-CTA maximum), S = 1000 (round 1's guard allowed 128 steps)."""
+    M, L, A, S, seed = 3, 16384, 400, 1000, 8
+    p = zi_params(100, 20)
+    eb, er = oracle_rows(oracle, p, L, A, seed, np.arange(M), S)
+    b, r = _gpu(ks, M, L, A, p, seed, S)
+    assert_rows_equal(b, r, np.arange(M), eb, er, "L=16384, S=1000")
+
+
+# ------------------------------------------------------------------ checkpoint / deferred errors
+@pytest.mark.parametrize("case", ["zi", "mix3", "paper", "cluster", "decoupled"])
+def test_checkpoint_attach_resumes_bit_exactly(ks, oracle, case):
+    """include/kineticsim.h: d_state IS the checkpoint.  Save its bytes after S1 steps, destroy the
+    handle, scribble over the buffer, restore the bytes, ks_attach a NEW handle, run S2 more steps:
+    the result equals one uninterrupted run of S1 + S2 steps (and the oracle)."""
+    import torch
+    opts = []
+    if case == "zi":
+        M, L, A, seed, p = 11, 256, 700, 9, zi_params(16, 100)
+    elif case == "mix3":
+        M, L, A, seed, p = 7, 1024, 900, 4, mix3_params()
+    elif case == "paper":
+        M, L, A, seed, p = 9, 128, 200, 5, paper_params(200, 0.15, 0.15, p_mkt=0.05)
+    elif case == "cluster":
+        M, L, A, seed, p = 5, 512, 600, 8, zi_params(32, 50)
+        opts = [(ks.KS_OPT_CLUSTER_SIZE, 4)]
+    else:
+        M, L, A, seed, p = 6, 128, 512, 2, zi_params(8, 10)
+        opts = [(ks.KS_OPT_BLOCK_THREADS, 256), (ks.KS_OPT_PIPELINE, 2)]      # ks_decoupled_kernel
+    S1, S2 = 37, 55
+    ids = np.arange(M)
+    eb, er = oracle_rows(oracle, p, L, A, seed, ids, S1 + S2)
+    sim = ks.KsSim(M, L, A, p, seed)
+    for o, v in opts:
+        sim.ks_set_option(o, v)
+    sim.ks_run(S1)
+    torch.cuda.synchronize()
+    saved = sim.state.clone()
+    sim.ks_destroy()
+    state = torch.full_like(saved, 0x5A)                # a different buffer with garbage in it
+    state.copy_(saved)
+    sim2 = ks.KsSim(M, L, A, p, seed, state=state, attach=True)
+    for o, v in opts:
+        sim2.ks_set_option(o, v)
+    sim2.ks_run(S2)
+    b, r = sim2.books_to_host(), sim2.stats_to_host()
+    sim2.ks_destroy()
+    assert_rows_equal(b, r, ids, eb, er, "attach " + case)
+    # the guards of the new handle start from the restored step counter and depth, not from zero
+    sim3 = ks.KsSim(M, L, A, p, seed, state=state, attach=True)
+    with pytest.raises(ks.KsError) as e:
+        sim3.ks_run(2 ** 32 - (S1 + S2))
+    assert e.value.status == ks.KS_ERR_OVERFLOW
+    sim3.ks_destroy()
+
+
+def test_statistic_overflow_is_detected_on_the_device(ks):
+    """The int64 sum of r^4 (f[9]) is checked exactly where it is formed: a record restored with
+    f[9] just below 2^63 overflows at the first price move, the kernel raises the sticky flag, and
+    every later call on the handle returns KS_ERR_OVERFLOW.  The same state with f[9] = 0 runs."""
+    import torch
+    M, L, A, seed, p = 3, 64, 256, 0, zi_params(8, 10)
+    sim = ks.KsSim(M, L, A, p, seed)
+    sim.ks_run(5)
+    torch.cuda.synchronize()
+    state = sim.state.clone()
+    sim.ks_destroy()
+    recs = state[M * 8 * L: M * (8 * L + 128)].view(torch.int64).view(M, 16)
+    ok = ks.KsSim(M, L, A, p, seed, state=state.clone(), attach=True)
+    ok.ks_run(200); torch.cuda.synchronize(); ok.ks_error_state()
+    moved = ok.stats_to_host()[:, 7] > 0                      # sum r^2 > 0: the price moved
+    ok.ks_destroy()
+    assert moved[1]
+    recs[1, 9] = 2 ** 63 - 1                                   # market 1 only
+    bad = ks.KsSim(M, L, A, p, seed, state=state, attach=True)
+    bad.ks_error_state()
+    bad.ks_run(200)
+    torch.cuda.synchronize()
+    for call in (bad.ks_error_state, lambda: bad.ks_run(1), bad.stats_to_host, bad.books_to_host):
+        with pytest.raises(ks.KsError) as e:
+            call()
+        assert e.value.status == ks.KS_ERR_OVERFLOW
+    bad.ks_destroy()
+
+
+def test_deferred_depth_check_refuses_the_run_on_the_device(ks, oracle):
+    """ks_run right after ks_write_books does not wait for the depth check: when the injected depth
+    plus the run's inflow could reach 2^31 the kernel itself refuses, nothing changes, and the
+    error surfaces as a sticky KS_ERR_OVERFLOW; a negative depth gives KS_ERR_INVALID_ARG.  A legal
+    injected book runs exactly as before (every other injected-book test takes this path too)."""
+    import torch
+    M, L, A, seed, p = 4, 64, 100, 3, zi_params(8, 10)
+    for poison, status in ((2 ** 31 - 1000, ks.KS_ERR_OVERFLOW), (-1, ks.KS_ERR_INVALID_ARG)):
+        books = random_books(M, L, seed=1, max_qty=20, fill=0.3)
+        books[2, 1, 7] = poison
+        d_books = torch.from_numpy(books).cuda()
+        sim = ks.KsSim(M, L, A, p, seed)
+        sim.ks_write_books(d_books)
+        try:
+            sim.ks_run(10)                                 # usually enqueued: the check is still in flight
+            torch.cuda.synchronize()
+            with pytest.raises(ks.KsError) as e:
+                sim.ks_error_state()
+            assert e.value.status == status
+        except ks.KsError as e2:                           # the host already had the result
+            assert e2.status == status
+        torch.cuda.synchronize()
+        raw = sim.state[: M * 8 * L].view(torch.int32).view(M, 2, L).cpu().numpy()
+        rec = sim.state[M * 8 * L: M * (8 * L + 128)].view(torch.int64).view(M, 16).cpu().numpy()
+        assert np.array_equal(raw, books) and (rec[:, 0] == 0).all()     # not a byte of the run happened
+        sim.ks_destroy()
 
 
 # ------------------------------------------------------------------ PACKED4 draw contract

@@ -21,25 +21,41 @@ def lib():
     return binding.load()
 
 
-def _declared():
-    names = []
-    for h in ("kineticsim.h", "kineticsim_bench.h"):
-        src = open(os.path.join(ROOT, "include", h)).read()
-        names += re.findall(r"KS_API\s+[\w\s\*]+?\b(ks_\w+)\s*\(", src)
-    return names
+def _declared(header):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    return re.findall(r"KS_API\s+[\w\s\*]+?\b(ks_\w+)\s*\(", src)
+
+
+def _exported(path):
+    out = subprocess.check_output(["nm", "-D", "--defined-only", path]).decode()
+    return {l.split()[-1] for l in out.splitlines() if " T " in l and l.split()[-1].startswith("ks_")}
 
 
 def test_headers_declare_what_the_binding_lists():
-    assert sorted(_declared()) == sorted(binding.EXPORTS)
+    assert sorted(_declared("kineticsim.h")) == sorted(binding.EXPORTS)
+    assert sorted(_declared("kineticsim_bench.h")) == sorted(binding.BENCH_EXPORTS)
 
 
-def test_library_exports_every_declared_symbol(lib):
-    out = subprocess.check_output(["nm", "-D", "--defined-only", binding.LIB_PATH]).decode()
-    exported = {l.split()[-1] for l in out.splitlines() if " T " in l}
-    ks = {s for s in exported if s.startswith("ks_")}
-    assert ks == set(_declared())
-    for n in _declared():
+def test_libraries_export_every_declared_symbol(lib):
+    """The product library exports exactly include/kineticsim.h, the bench library exactly
+    include/kineticsim_bench.h (ablation + microbenchmarks live OUTSIDE the product)."""
+    assert _exported(binding.LIB_PATH) == set(_declared("kineticsim.h"))
+    assert _exported(binding.BENCH_LIB_PATH) == set(_declared("kineticsim_bench.h"))
+    for n in _declared("kineticsim.h"):
         assert getattr(lib, n) is not None
+    bench = binding.load_bench()
+    for n in _declared("kineticsim_bench.h"):
+        assert getattr(bench, n) is not None
+
+
+def test_product_library_never_allocates_device_memory():
+    """include/kineticsim.h: the state buffer is the caller's; the product library holds no
+    cudaMalloc / cudaFree call (the bench library may, and says so)."""
+    for f in ("ks_api.cu", "ks_kernel.cuh", "ks_device.cuh", "ks_cluster.cuh", "ks_trace.cuh"):
+        src = open(os.path.join(ROOT, "paper_2606_21784_b200", "csrc", f)).read()
+        assert not re.search(r"\bcudaMalloc\w*\s*\(|\bcudaFree\s*\(", src), f
+    out = subprocess.check_output(["nm", "-D", "--undefined-only", binding.LIB_PATH]).decode()
+    assert "cudaMalloc" not in out
 
 
 def test_library_is_sm100a_with_shared_atomics():
@@ -75,6 +91,9 @@ def test_argument_validation_precedes_cuda(lib):
     assert lib.ks_run(None, 1, None) == binding.KS_ERR_INVALID_ARG
     assert lib.ks_read_books(None, None, None) == binding.KS_ERR_INVALID_ARG
     assert lib.ks_set_option(None, 0, 0) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_error_state(None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_attach(C.byref(h), 1, 48, 256, C.byref(P), 0, 0, fake, None) == binding.KS_ERR_INVALID_ARG
+    assert lib.ks_attach(C.byref(h), 1, 64, 256, C.byref(P), 0, 0, None, None) == binding.KS_ERR_INVALID_ARG
     assert b"NULL" in lib.ks_last_error()
     lib.ks_destroy(None)
 
@@ -88,7 +107,7 @@ def test_no_cpu_fallback_without_a_device(lib):
     assert lib.ks_create(C.byref(h), 1, 64, 256, C.byref(P), 0, 0x1000, None) == binding.KS_ERR_CUDA
     assert h.value is None and len(lib.ks_last_error()) > 0
     ops, sec = C.c_double(0), C.c_double(0)
-    assert lib.ks_bench_int_pipe(0, 256, 1, 1, 0, 1, None, C.byref(ops), C.byref(sec)) == binding.KS_ERR_CUDA
+    assert binding.load_bench().ks_bench_int_pipe(0, 256, 1, 1, 0, 1, None, C.byref(ops), C.byref(sec)) == binding.KS_ERR_CUDA
 
 
 def test_derive_stats_matches_oracle_on_equal_integers(lib, oracle):
