@@ -2,19 +2,25 @@
 """bench.py -- agent events/s of the call-auction hot path on B200 (BASELINE.json `metric`).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
+                    [--scaling weak|strong] [--rng literal|packed4] [--no-extras]
+    python bench.py --case NAME [--S n] [--M m] [--mode persistent|stepwise|traced]   # one run, for ncu
 
 A "step" is one pass of the whole hot path over one batch: ks_create (state init) + ONE ks_run of
-all S steps of the workload (a0-a7), on M markets per GPU.  Workload: BASELINE.json configs[3]
-("throughput scale", C4: M=65536, L=512, A=4096, S=1000, seed 3), the largest config and the one
-the metric's roofline clause is quoted on.  For N > 1 each rank runs its own M markets with
-market_base = rank*M (weak scaling, no data-path collective: markets are independent).
-Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+all S steps of the workload (a0-a7).  Workload: BASELINE.json configs[3] ("throughput scale", C4:
+M=65536, L=512, A=4096, S=1000, seed 3), the largest config and the one the metric's roofline
+clause is quoted on.  N > 1: one process per GPU (the driver launches torchrun; a plain
+`python bench.py --gpus N` re-executes itself under torch.distributed.run), markets sharded by
+market_base, no data-path collective.  Prints ONE JSON line (rank 0).  DESIGN.md 7 explains every
+field.
 """
 from __future__ import annotations
 
 import argparse
+import dataclasses
 import json
 import os
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -25,23 +31,39 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-import dataclasses  # noqa: E402
-
-from paper_2606_21784_b200.workloads import CONFIGS, KS_MODEL_ZI, packed4, paper_params, sampled_markets  # noqa: E402
+from paper_2606_21784_b200.workloads import (CONFIGS, KS_MODEL_PAPER, KS_MODEL_ZI, packed4, paper_params,  # noqa: E402
+                                             sampled_markets, shard_markets, zi_params)
 
 # Roofline of ks_persistent_kernel: the fmaheavy pipe that executes the 32x32->64
 # multiplies.  Algorithmic multiplies per agent event: 20 of Philox4x32-10 + the
 # mulhi draws of the rule (noise/momentum: offset and quantity; maker: spread only).
 ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0,
                        # PACKED4 (A22): a Philox block per 4 agents + the rule's multiply-extract draws
-                       "zi_packed4": 20.0 / 4 + 2.0, "mix3_packed4": 20.0 / 4 + (2.0 + 1.0 + 2.0) / 3.0}
-# Multiplies the kernel actually issues per event (IMAD.WIDE.U32 + IMAD.HI.U32 in the hot loop,
-# from cuobjdump -sass): hoisting of (market, step)-uniform products, round 0's M0*agent carried as
-# a running 64-bit sum, w3 never computed.
-EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 17.0 + 19.0) / 3.0,
-                        "zi_packed4": 17.0 / 4 + 2.0, "mix3_packed4": 17.0 / 4 + (2.0 + 1.0 + 2.0) / 3.0}
-# a 32-lane IMAD.WIDE/IMAD.HI occupies an SMSP's fmaheavy pipe for 4 cycles -> 8 lanes/clk/SMSP
+                       "zi_packed4": 20.0 / 4 + 2.0, "mix3_packed4": 20.0 / 4 + (2.0 + 1.0 + 2.0) / 3.0,
+                       # model 4 (A24): 20 of Philox + offset and quantity (momentum / maker: quantity only)
+                       "paper": 0.70 * 22.0 + 0.30 * 21.0}
+# Multiplies the kernel actually issues per event (IMAD.WIDE.U32 + IMAD.HI.U32 per ATOMS in the
+# hot loops).  tests/test_library_host.py counts them in the SASS of the built library, so these
+# constants cannot go stale silently.
+EXEC_MULTS_PER_CLASS = {"noise": 19.0, "maker": 14.0, "momentum": 19.0,                 # literal contract (a%3 classes)
+                        "paper_noise": 19.0, "paper_momentum": 18.0, "paper_maker": 16.0,   # model 4 (all four words)
+                        "packed_block": 17.0}                                               # one Philox block of 4 agents
+EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 14.0 + 19.0) / 3.0,
+                        "zi_packed4": 17.0 / 4 + 2.0, "mix3_packed4": 17.0 / 4 + (2.0 + 1.0 + 2.0) / 3.0,
+                        # model 4 at the mix bench.py times (case model4_C4shape: 70 % noise, 15 % momentum, 15 % makers)
+                        "paper": 0.70 * 19.0 + 0.15 * 18.0 + 0.15 * 16.0}
+# derived peak: a 32-lane IMAD.WIDE/IMAD.HI occupies an SMSP's fmaheavy pipe for 4 cycles -> 8 lanes/clk/SMSP
 WIDE_MUL_LANES_PER_SM_PER_CLK = 4 * 8
+# dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
+# `ncu --set full` capture summarised under profiles/ (None until measured for that config).
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 25261312 + 237688320,            # profiles/r1h_persistent_full.md
+                                  "C4_packed4": 23691008 + 254493952}    # profiles/r1g_packed_persistent_full.md
+
+
+def model_key(params: dict) -> str:
+    if params["model"] == KS_MODEL_PAPER:
+        return "paper"
+    return ("zi" if (params["model"] & 1) == KS_MODEL_ZI else "mix3") + ("_packed4" if params["model"] >= 2 else "")
 
 
 class ClockSampler(threading.Thread):
@@ -97,6 +119,51 @@ def physical_gpu_index(local_rank: int) -> int:
     return local_rank
 
 
+# ---------------------------------------------------------------------------------------------
+# Multi-GPU launch logic: one process per GPU.  Pure function of the arguments
+# and the environment so that tests/test_bench_launch.py can check it without a GPU.
+# ---------------------------------------------------------------------------------------------
+def launch_plan(gpus: int, env: dict, n_visible, argv, impl: str = "ours"):
+    """-> ("run", rank, local_rank, world) when this process is a rank (or the single-GPU run),
+          ("spawn", cmd) when `--gpus N > 1` was given WITHOUT torchrun: re-execute under
+          torch.distributed.run with N ranks on 127.0.0.1,
+          ("error", message) when the request cannot be honoured -- bench.py then exits non-zero
+          instead of printing a line whose n_gpus differs from --gpus."""
+    if gpus < 1:
+        return ("error", "--gpus must be >= 1")
+    if "WORLD_SIZE" in env:
+        world = int(env["WORLD_SIZE"])
+        rank, local_rank = int(env.get("RANK", "0")), int(env.get("LOCAL_RANK", env.get("RANK", "0")))
+        if world != gpus:
+            return ("error", "WORLD_SIZE=%d but --gpus %d: launch torchrun with --nproc-per-node %d" % (world, gpus, gpus))
+        if not 0 <= rank < world:
+            return ("error", "RANK=%d outside [0, %d)" % (rank, world))
+        if impl == "ours" and n_visible is not None and local_rank >= n_visible:
+            return ("error", "LOCAL_RANK=%d but only %d CUDA device(s) are visible" % (local_rank, n_visible))
+        return ("run", rank, local_rank, world)
+    if gpus == 1 or impl == "reference":       # the reference arm is CPU-only: rank 0 alone does the work
+        return ("run", 0, 0, 1 if impl == "ours" else gpus)
+    if n_visible is not None and n_visible < gpus:
+        return ("error", "--gpus %d but only %d CUDA device(s) are visible" % (gpus, n_visible))
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return ("spawn", cmd)
+
+
+def rank_markets(cfg_M: int, rank: int, world: int, scaling: str):
+    """(market_base, markets of this rank, markets of the whole job).  weak: every GPU runs the
+    config's M markets, rank r keyed from r*M; strong: the config's M markets are cut into
+    contiguous shards (workloads.shard_markets)."""
+    if scaling == "strong":
+        base, count = shard_markets(cfg_M, rank, world)
+        return base, count, cfg_M
+    return rank * cfg_M, cfg_M, world * cfg_M
+
+
 def time_oracle(cfg, n_markets: int, S: int):
     """The oracle as it stands, one thread, on the first n sampled markets of cfg for S steps."""
     from oracle import ks_oracle
@@ -105,6 +172,25 @@ def time_oracle(cfg, n_markets: int, S: int):
     ks_oracle.run_markets(cfg.params, cfg.L, cfg.A, cfg.seed, ids, S)
     dt = time.perf_counter() - t0
     return len(ids) * cfg.A * S / dt, dt, len(ids)
+
+
+def workload_config(cfg, n_gpus, scaling="weak"):
+    if scaling == "strong":
+        par = "strong: the %d markets cut into %d contiguous shards (workloads.shard_markets), market_base = shard start, no collective" % (cfg.M, n_gpus)
+    else:
+        par = "weak: %d markets on each of %d GPU(s), market_base = rank*M, no collective" % (cfg.M, n_gpus)
+    kind = "paper agent model (model 4)" if cfg.params["model"] == KS_MODEL_PAPER else \
+        ("zero-intelligence" if (cfg.params["model"] & 1) == KS_MODEL_ZI else "noise/maker/momentum by a%3") + \
+        (", PACKED4 draw contract (NOT the BASELINE.json one; DESIGN.md A22)" if cfg.params["model"] >= 2 else "")
+    return {"workload": "%s: BASELINE.json configs[%d] -- M=%d markets%s, L=%d ticks, A=%d agents, S=%d steps, seed=%d, %s"
+                        % (cfg.name, int(cfg.name[1]) - 1, cfg.M, "/GPU" if scaling == "weak" else " in all", cfg.L, cfg.A, cfg.S,
+                           cfg.seed, kind),
+            "M": cfg.M, "L": cfg.L, "A": cfg.A, "S": cfg.S, "seed": cfg.seed, "parallelism": par,
+            "l2": ("state buffer %.0f MB per GPU exceeds the 126 MB L2; every timed step (ks_create + ks_run) rewrites all of it"
+                   if cfg.M * (8 * cfg.L + 128) > 126e6 else
+                   "state buffer %.1f MB per GPU fits the L2, but a fresh ks_run never READS it (ks_create zeroes it, the kernel "
+                   "skips the load of an all-zero book): there is no input to keep warm")
+                  % (cfg.M * (8 * cfg.L + 128) / 1e6)}
 
 
 def run_reference(args, cfg, rank: int):
@@ -128,8 +214,8 @@ def run_reference(args, cfg, rank: int):
     line = {
         "impl": "reference", "metric": "agent_events_per_s", "value": value, "unit": "events/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-        "config": workload_config(cfg, args.gpus),
+        "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": workload_config(cfg, args.gpus, args.scaling),
         "cpu_baseline": {"value": value, "unit": "events/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -137,14 +223,94 @@ def run_reference(args, cfg, rank: int):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg, n_gpus):
-    return {"workload": "%s: BASELINE.json configs[%d] -- M=%d markets/GPU, L=%d ticks, A=%d agents, S=%d steps, seed=%d, %s"
-                        % (cfg.name, int(cfg.name[1]) - 1, cfg.M, cfg.L, cfg.A, cfg.S, cfg.seed,
-                           ("zero-intelligence" if (cfg.params["model"] & 1) == KS_MODEL_ZI else "noise/maker/momentum by a%3")
-                           + (", PACKED4 draw contract (NOT the BASELINE.json one; DESIGN.md A22)" if cfg.params["model"] >= 2 else "")),
-            "M_per_gpu": cfg.M, "L": cfg.L, "A": cfg.A, "S": cfg.S, "seed": cfg.seed,
-            "parallelism": "markets sharded across %d GPU(s), market_base = rank*M, no collective" % n_gpus,
-            "l2": "state buffer %.0f MB per GPU exceeds the 126 MB L2; written once per step" % (cfg.M * (8 * cfg.L + 128) / 1e6)}
+# ---------------------------------------------------------------------------------------------
+# One named case, timed with CUDA events (extras of the default line and the `--case` mode that
+# the ncu / compute-sanitizer commands under profiles/ run).
+# ---------------------------------------------------------------------------------------------
+def case_config(name: str):
+    """Named cases: C1..C5, C4_packed4, C5_packed4, model4_C4shape (the paper's own agent model on
+    the C4 shape, alpha_mom = alpha_maker = 0.15, P_mkt = 0.02), table4 / latency (the paper's own
+    shapes with zero-intelligence agents: context), cluster (L = 32768 on a 2-CTA cluster)."""
+    from paper_2606_21784_b200.workloads import Config, mix3_params
+    if name in CONFIGS:
+        return CONFIGS[name]
+    if name.endswith("_packed4") and name[:-8] in CONFIGS:
+        c = CONFIGS[name[:-8]]
+        return dataclasses.replace(c, name=name, params=packed4(c.params))
+    if name == "model4_C4shape":
+        c = CONFIGS["C4"]
+        return dataclasses.replace(c, name=name, params=paper_params(c.A, 0.15, 0.15, delta=32, qmax=100, half_spread=2, p_mkt=0.02))
+    if name == "table4":
+        return Config(name, 8192, 128, 256, 500, 5, zi_params(8, 10))
+    if name == "latency":
+        return Config(name, 4096, 128, 256, 500, 5, zi_params(8, 10))
+    if name == "cluster":
+        return Config(name, 64, 32768, 4096, 200, 6, mix3_params())
+    raise SystemExit("bench.py: unknown case %r" % name)
+
+
+def time_case(ks, torch, dev, c, *, reps=3, mode="persistent", S=None, M=None, opts=(), warm=1):
+    """Median device time (ms) of ks_run(S) on config c (ks_create outside the events)."""
+    M = M or c.M
+    S = S or c.S
+    st = torch.empty(ks.ks_state_bytes(M, c.L), dtype=torch.uint8, device=dev)
+    tr = torch.empty((M, S, 2), dtype=torch.int32, device=dev) if mode == "traced" else None
+    ts = []
+    for i in range(warm + reps):
+        sim = ks.KsSim(M, c.L, c.A, c.params, c.seed, state=st)
+        try:
+            for o, v in opts:
+                sim.ks_set_option(o, v)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            if mode == "stepwise":
+                sim.ks_run_stepwise(S)
+            elif mode == "traced":
+                sim.ks_run_traced(S, tr)
+            else:
+                sim.ks_run(S)
+            b.record()
+            torch.cuda.synchronize()
+            sim.ks_error_state()
+            ts.append(a.elapsed_time(b))
+        finally:
+            sim.ks_destroy()
+    ms = float(np.median(ts[warm:]))
+    return {"ms": ms, "events_per_s": float(M) * c.A * S / (ms * 1e-3), "M": M, "L": c.L, "A": c.A, "S": S, "reps": reps}
+
+
+def run_case(args):
+    """--case: ONE timed run of a named case (after one warm-up), a small JSON line."""
+    import torch
+    from paper_2606_21784_b200 import binding as ks
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    ks.load()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    c = case_config(args.case)
+    opts = []
+    if args.threads:
+        opts.append((ks.KS_OPT_BLOCK_THREADS, args.threads))
+    if args.atomic_mode:
+        opts.append((ks.KS_OPT_ATOMIC_MODE, args.atomic_mode))
+    if args.pipeline:
+        opts.append((ks.KS_OPT_PIPELINE, args.pipeline))
+    if args.rel_columns:
+        opts.append((ks.KS_OPT_REL_COLUMNS, args.rel_columns))
+    n0 = ks.ks_launch_count()
+    r = time_case(ks, torch, dev, c, reps=1, mode=args.mode, S=args.S, M=args.M, opts=opts)
+    if args.trace_stats:
+        M, S = r["M"], r["S"]
+        tr = torch.zeros((M, S, 2), dtype=torch.int32, device=dev)
+        sim = ks.KsSim(M, c.L, c.A, c.params, c.seed)
+        sim.ks_run_traced(S, tr)
+        ks.ks_trace_stats(tr, M, S, 20)
+        torch.cuda.synchronize()
+        sim.ks_destroy()
+    r.update({"case": c.name, "mode": args.mode, "gpu_launches": ks.ks_launch_count() - n0,
+              "hbm_bytes_persistent": float(r["M"]) * (8 * c.L + 128)})
+    print(json.dumps(r), flush=True)
 
 
 def main():
@@ -154,46 +320,70 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = the config's M markets on EVERY GPU (default); strong = the config's M markets "
+                         "cut into N contiguous shards (SURVEY.md S8(e))")
     ap.add_argument("--threads", type=int, default=0, help="KS_OPT_BLOCK_THREADS (0 = automatic)")
     ap.add_argument("--atomic-mode", type=int, default=0)
+    ap.add_argument("--pipeline", type=int, default=0, help="KS_OPT_PIPELINE (--case only)")
+    ap.add_argument("--rel-columns", type=int, default=0, help="KS_OPT_REL_COLUMNS (--case only)")
     ap.add_argument("--rng", default="literal", choices=["literal", "packed4"],
                     help="draw contract: literal = BASELINE.json (one Philox block per agent); packed4 = the "
                          "separately named PACKED4 contract (DESIGN.md A22), reported beside it, never instead of it")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-microbench", action="store_true")
-    ap.add_argument("--all-configs", action="store_true", help="also time C1..C5 (extra keys)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the other configs / contracts / ablation keys")
+    ap.add_argument("--all-configs", action="store_true", help="(kept for compatibility: the extras are on by default)")
+    ap.add_argument("--case", default=None, help="run ONE named case once and print a small JSON line (ncu / sanitizer helper)")
+    ap.add_argument("--mode", default="persistent", choices=["persistent", "stepwise", "traced"])
+    ap.add_argument("--trace-stats", action="store_true", help="--case: also launch ks_run_traced + ks_trace_stats once")
+    ap.add_argument("--S", type=int, default=None, help="--case: override the number of steps")
+    ap.add_argument("--M", type=int, default=None, help="--case: override the number of markets")
     args = ap.parse_args()
+    if args.case:
+        run_case(args)
+        return
     cfg = CONFIGS[args.config]
     if args.rng == "packed4":
         cfg = dataclasses.replace(cfg, params=packed4(cfg.params))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    n_visible = None
+    if args.impl == "ours":
+        import torch
+        n_visible = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if n_visible == 0:
+            raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    plan = launch_plan(args.gpus, os.environ, n_visible, sys.argv[1:], args.impl)
+    if plan[0] == "error":
+        print("bench.py: " + plan[1], file=sys.stderr)
+        sys.exit(2)
+    if plan[0] == "spawn":
+        sys.exit(subprocess.call(plan[1]))
+    _, rank, local_rank, world = plan
 
     if args.impl == "reference":
         run_reference(args, cfg, rank)
         return
 
-    import torch
     import torch.distributed as dist
     from paper_2606_21784_b200 import binding as ks
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     ks.load()
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    assert world == args.gpus or world == 1, "launch with torchrun --nproc-per-node N for --gpus N"
+        if dist.get_world_size() != args.gpus:
+            print("bench.py: process group has %d ranks, --gpus %d" % (dist.get_world_size(), args.gpus), file=sys.stderr)
+            sys.exit(2)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    M, L, A, S = cfg.M, cfg.L, cfg.A, cfg.S
-    base = rank * M
+    L, A, S = cfg.L, cfg.A, cfg.S
+    base, M, M_job = rank_markets(cfg.M, rank, world, args.scaling)
     state = torch.empty(ks.ks_state_bytes(M, L), dtype=torch.uint8, device=dev)
 
     def one_step(ev_pairs=None):
@@ -231,13 +421,15 @@ def main():
     total_ms = t_start.elapsed_time(t_end)
     kern_ms = [a.elapsed_time(b) for a, b in pairs]
     for s_ in sims:
+        s_.ks_error_state()
         s_.ks_destroy()
     if world > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
-    events_per_step = float(M) * A * S
-    value = world * events_per_step * args.steps / (total_ms * 1e-3)
+    events_per_step = float(M) * A * S                    # this rank
+    job_events_per_step = float(M_job) * A * S            # all ranks
+    value = job_events_per_step * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers: opening book H2D from pinned memory,
     #      ks_run, books + records D2H into pinned memory, all inside the timed region
@@ -270,7 +462,7 @@ def main():
         t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_ms = float(t.item())
-    e2e_value = world * events_per_step * n_e2e / (e2e_ms * 1e-3)
+    e2e_value = job_events_per_step * n_e2e / (e2e_ms * 1e-3)
     # the e2e result is the same simulation: check it against the device-resident run's records
     chk = torch.empty((M, 16), dtype=torch.int64).pin_memory()
     sim = one_step(); sim.ks_read_stats(chk); torch.cuda.synchronize(); sim.ks_destroy()
@@ -281,9 +473,11 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (ks_persistent_kernel): ALU / issue bound
-    model = ("zi" if (cfg.params["model"] & 1) == KS_MODEL_ZI else "mix3") + ("_packed4" if cfg.params["model"] >= 2 else "")
+    # ---- microbenchmarks in the same process (same clocks): the measured multiply-pipe peak, the
+    #      BASELINE.json smem-atomic roofline and the generation-only (integer ALU) ceiling
+    model = model_key(cfg.params)
     avg_kern_s = float(np.mean(kern_ms)) * 1e-3
+    kev = events_per_step / avg_kern_s
     peaks = {}
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -292,41 +486,9 @@ def main():
         pass
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
-    peak = sms * WIDE_MUL_LANES_PER_SM_PER_CLK * sm_max_mhz * 1e6 / 1e12
-    achieved = ALG_MULTS_PER_EVENT[model] * events_per_step / avg_kern_s / 1e12
-    executed = EXEC_MULTS_PER_EVENT[model] * events_per_step / avg_kern_s / 1e12
-    roofline = {"bound": "alu", "kernel": "ks_persistent_kernel", "achieved": achieved, "peak": peak,
-                "unit": "T 32x32->64-bit integer multiplies/s", "frac": achieved / peak,
-                "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name if args.rng == "literal" else cfg.name + "_packed4"),
-                "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "avg_launch_ms": avg_kern_s * 1e3,
-                "executed_mults_per_event": EXEC_MULTS_PER_EVENT[model], "fmaheavy_pipe_frac_from_executed": executed / peak,
-                "frac_note": "achieved counts the ALGORITHMIC multiplies (SURVEY.md S8(d)); the kernel executes fewer "
-                             "(hoisted / strength-reduced rounds, w3 skipped), so frac can reach or pass 1.0 -- the pipe's own "
-                             "utilisation is fmaheavy_pipe_frac_from_executed (ncu: 95.8 % with the address multiply-adds, "
-                             "profiles/r1h_persistent_full.md)",
-                "peak_source": "derived (DESIGN.md 7.2): %d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
-                               % (sms, sm_max_mhz, "MEASURED_PEAKS.json sm_max_mhz" if peaks else "NVML max clock"),
-                "hbm": {"algorithmic_bytes": M * (8 * L + 128), "achieved_GBps": M * (8 * L + 128) / avg_kern_s / 1e9,
-                        "peak_GBps": peaks.get("hbm_gbs", 6650.0),
-                        "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback (B200_PROFILING.md)"}}
-
-    line = {
-        "metric": "agent_events_per_s", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": workload_config(cfg, world),
-        "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": int(h_open.numel() * 4),
-                "d2h_bytes_per_step": int(h_books.numel() * 4 + h_recs.numel() * 8), "steps": n_e2e,
-                "ms_per_step": e2e_ms / n_e2e},
-        "gpu_launches": int(launches),
-        "roofline": roofline,
-        "kernel_events_per_s": events_per_step / avg_kern_s,
-        "paper_context": {"events_per_s": 5.47e10, "where": "RTX 5090, M=8192 A=1024 L=128 S=500, PAPER.md:313 (other GPU, other agent model)"},
-    }
-
-    # ---- microbenchmarks in the same process (same clocks): the BASELINE.json smem-atomic
-    #      roofline and the generation-only (integer ALU) ceiling
-    if not args.no_microbench and world == 1:
+    peak_derived = sms * WIDE_MUL_LANES_PER_SM_PER_CLK * sm_max_mhz * 1e6 / 1e12
+    micro, mulwide_peak = None, None
+    if not args.no_microbench:
         delta = cfg.params["noise_delta"]
         Lb = min(L, 8192)
         thr = 256
@@ -342,104 +504,72 @@ def main():
         mix, _ = ks.ks_bench_int_pipe(2)
         mix2, _ = ks.ks_bench_int_pipe(3)
         mix3, _ = ks.ks_bench_int_pipe(4)
+        mulwide, _ = ks.ks_bench_int_pipe(5)
+        mulwide_peak = mulwide / 1e12
         cyc = lambda ops_s, per: sms * 4 * sm_max_mhz * 1e6 * 32 * per / ops_s      # SMSP cycles per IMAD.WIDE
-        atomics_per_event = 1.0 if model.startswith("zi") else 4.0 / 3.0
-        kev = events_per_step / avg_kern_s
-        line["microbench"] = {
+        atomics_per_event = {"zi": 1.0, "zi_packed4": 1.0, "paper": 1.0}.get(model, 4.0 / 3.0)
+        micro = {
+            "mul_wide_u32_thread_ops_per_s": mulwide,
             "smem_atomic_peak_lane_ops_per_s": peak_ops, "smem_atomic_pattern_lane_ops_per_s": pat_ops,
             "smem_atomic_pattern_warp_aggregated_lane_ops_per_s": agg_ops, "smem_atomic_same_address_lane_ops_per_s": one_ops,
-            "generate_only_events_per_s": gen_ev, "imad_wide_thread_ops_per_s": wide, "lop3_thread_ops_per_s": lop,
+            "generate_only_events_per_s": gen_ev, "imad_wide_accumulate_thread_ops_per_s": wide, "lop3_thread_ops_per_s": lop,
             "imad_wide_lop3_mix_thread_ops_per_s": mix,
-            "smsp_cycles_per_imad_wide": {"alone": cyc(wide, 1), "with_1_lop3": cyc(mix, 2), "with_2_lop3": cyc(mix2, 3),
-                                          "with_3_lop3": cyc(mix3, 4)},
+            "smsp_cycles_per_imad_wide": {"mul_wide_alone": cyc(mulwide, 1), "accumulate_alone": cyc(wide, 1),
+                                          "with_1_lop3": cyc(mix, 2), "with_2_lop3": cyc(mix2, 3), "with_3_lop3": cyc(mix3, 4)},
             "frac_of_smem_atomic_peak": kev * atomics_per_event / peak_ops,
             "frac_of_smem_atomic_pattern": kev * atomics_per_event / pat_ops,
             "frac_of_generate_only": kev / gen_ev,
         }
 
-    if args.all_configs and world == 1:
-        extra = {}
-        for name in sorted(CONFIGS):
-            c = CONFIGS[name]
-            st = torch.empty(ks.ks_state_bytes(c.M, c.L), dtype=torch.uint8, device=dev)
-            ts = []
-            for i in range(4):
-                sim = ks.KsSim(c.M, c.L, c.A, c.params, c.seed, state=st)
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(); sim.ks_run(c.S); b.record(); torch.cuda.synchronize()
-                ts.append(a.elapsed_time(b)); sim.ks_destroy()
-            extra[name] = {"ms_median_of_3": float(np.median(ts[1:])), "events_per_s": c.events / (float(np.median(ts[1:])) * 1e-3)}
-        line["all_configs"] = extra
-        # a8 ablation on C2: one launch per step, book through HBM every step
-        c = CONFIGS["C2"]
-        st = torch.empty(ks.ks_state_bytes(c.M, c.L), dtype=torch.uint8, device=dev)
-        ts = []
-        for i in range(3):
-            sim = ks.KsSim(c.M, c.L, c.A, c.params, c.seed, state=st)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); sim.ks_run_stepwise(c.S); b.record(); torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b)); sim.ks_destroy()
-        ms = float(np.median(ts[1:]))
-        hbm_bytes = float(c.S) * c.M * 2 * (8 * c.L + 128)          # load + store of book and record, every step
-        line["ablation_launch_per_step_C2"] = {
-            "ms": ms, "events_per_s": c.events / (ms * 1e-3), "launches": c.S,
-            "slowdown_vs_persistent": ms / extra["C2"]["ms_median_of_3"],
-            "algorithmic_hbm_bytes": hbm_bytes, "hbm_GBps": hbm_bytes / (ms * 1e-3) / 1e9,
-            "persistent_hbm_bytes": float(c.M) * (8 * c.L + 128)}
+    # ---- roofline of the dominant kernel (ks_persistent_kernel): bound by the 32x32->64 multiply pipe
+    peak = mulwide_peak if mulwide_peak else peak_derived
+    achieved = ALG_MULTS_PER_EVENT[model] * kev / 1e12
+    executed = EXEC_MULTS_PER_EVENT[model] * kev / 1e12
+    roofline = {"bound": "alu", "kernel": "ks_persistent_kernel", "achieved": achieved, "peak": peak,
+                "unit": "T 32x32->64-bit integer multiplies/s", "frac": achieved / peak,
+                "frac_executed": executed / peak,
+                "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name if args.rng == "literal" else cfg.name + "_packed4"),
+                "peak_source": ("measured in this process: ks_bench_int_pipe(5), a pure mul.wide.u32 stream "
+                                "(include/kineticsim_bench.h)") if mulwide_peak else
+                               "derived (microbenchmarks skipped): see peak_derived_source",
+                "peak_derived": peak_derived, "frac_of_derived_peak": achieved / peak_derived,
+                "frac_executed_of_derived_peak": executed / peak_derived,
+                "peak_derived_source": "%d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
+                                       % (sms, sm_max_mhz, "MEASURED_PEAKS.json sm_max_mhz" if peaks else "NVML max clock"),
+                "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "executed_mults_per_event": EXEC_MULTS_PER_EVENT[model],
+                "avg_launch_ms": avg_kern_s * 1e3,
+                "frac_note": "achieved/frac count the ALGORITHMIC multiplies (SURVEY.md S8(d): 22 per event); the kernel executes "
+                             "fewer (19: hoisted / strength-reduced rounds, w3 skipped; counted in the SASS by "
+                             "tests/test_library_host.py), so frac can pass 1.0 -- the pipe's own utilisation is frac_executed "
+                             "(ncu: sm__pipe_fmaheavy_cycles_active, profiles/)",
+                "hbm": {"algorithmic_bytes": M * (8 * L + 128), "achieved_GBps": M * (8 * L + 128) / avg_kern_s / 1e9,
+                        "peak_GBps": peaks.get("hbm_gbs", 6650.0),
+                        "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback (B200_PROFILING.md)"}}
+    if micro:
+        # BASELINE.json's metric names the smem-atomic roofline: keep its two fractions beside the headline
+        roofline["frac_of_smem_atomic_peak"] = micro["frac_of_smem_atomic_peak"]
+        roofline["frac_of_smem_atomic_pattern"] = micro["frac_of_smem_atomic_pattern"]
 
-    if args.all_configs and world == 1:
-        # context runs in the paper's own shapes: Table IV's fixed workload M=8192,
-        # A=256, L=128, S=500 and the latency configuration M=4096, A=256 with
-        # zero-intelligence agents Delta=8, q<=10, seed 5 -- NOT the paper's agent model or GPU
-        from paper_2606_21784_b200.workloads import zi_params
-        ctx = {}
-        for name, Mp in (("table4_M8192_A256_L128_S500", 8192), ("latency_M4096_A256_L128_S500", 4096)):
-            st = torch.empty(ks.ks_state_bytes(Mp, 128), dtype=torch.uint8, device=dev)
-            ts = []
-            for i in range(6):
-                sim = ks.KsSim(Mp, 128, 256, zi_params(8, 10), 5, state=st)
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(); sim.ks_run(500); b.record(); torch.cuda.synchronize()
-                ts.append(a.elapsed_time(b)); sim.ks_destroy()
-            ms = float(np.median(ts[1:]))
-            ctx[name] = {"ms_median_of_5": ms, "events_per_s": Mp * 256 * 500 / (ms * 1e-3), "us_per_step": ms * 1e3 / 500}
-        ctx["paper"] = "KineticSim on RTX 5090: 20.2 ms, 5.2e10 events/s (Table IV); 22.1 us median per step at M=4096 (PAPER.md:438)"
-        line["paper_shape_context"] = ctx
+    line = {
+        "metric": "agent_events_per_s", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": args.scaling,
+        "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": workload_config(cfg, world, args.scaling),
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": int(h_open.numel() * 4),
+                "d2h_bytes_per_step": int(h_books.numel() * 4 + h_recs.numel() * 8), "steps": n_e2e,
+                "ms_per_step": e2e_ms / n_e2e},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "kernel_events_per_s": kev,
+        "paper_context": {"events_per_s": 5.47e10, "where": "RTX 5090, M=8192 A=1024 L=128 S=500, PAPER.md:313 (other GPU, other agent model)"},
+    }
+    if micro:
+        line["microbench"] = micro
 
-    if args.all_configs and world == 1:
-        # SIV-J sweep shape: alpha_mom = 0 .. 0.70 in steps of 0.05, alpha_maker
-        # = 0.15, M = 64 markets x S = 1000 steps each, the paper's own agent model (model 4), traced,
-        # statistics on the device.  A = 200 (12.8e6 events / 64 / 1000: PAPER.md:458); L, Delta,
-        # q_max, P_mkt are not given -- workloads.paper_params defaults.  Context, not a parity case.
-        Ms, Ls, As, Ss, K = 64, 128, 200, 1000, 20
-        st = torch.empty(ks.ks_state_bytes(Ms, Ls), dtype=torch.uint8, device=dev)
-        tr = torch.empty((Ms, Ss, 2), dtype=torch.int32, device=dev)
-        out = torch.empty((Ms, 4 + 2 * K), dtype=torch.float64, device=dev)
-        alphas = [round(0.05 * i, 2) for i in range(15)]
-        rows = []
+    if not args.no_extras:
+        line.update(extras(ks, torch, dev, peak, cfg))
 
-        def sweep(record):
-            for al in alphas:
-                sim = ks.KsSim(Ms, Ls, As, paper_params(As, al), 5, state=st)
-                sim.ks_run_traced(Ss, tr)
-                ks.ks_trace_stats(tr, Ms, Ss, K, out)
-                if record:
-                    o = out.cpu().numpy()
-                    rows.append({"alpha_mom": al, "volatility": float(np.nanmean(o[:, 0])), "excess_kurtosis": float(np.nanmean(o[:, 1])),
-                                 "volume_per_step": float(np.nanmean(o[:, 2])), "acf_r_lag1": float(np.nanmean(o[:, 4])),
-                                 "acf_abs_r_lag1": float(np.nanmean(o[:, 4 + K]))})
-                sim.ks_destroy()
-
-        sweep(False)
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); sweep(False); b.record(); torch.cuda.synchronize()
-        sweep(True)
-        line["sivj_sweep"] = {"configs": len(alphas), "M": Ms, "L": Ls, "A": As, "S": Ss, "agent_events": len(alphas) * Ms * As * Ss,
-                              "ms_total_device": a.elapsed_time(b), "paper": "< 250 ms for 12.8e6 events (RTX 5090, PAPER.md:458)",
-                              "mean_over_markets": rows}
-
-    if not args.no_cpu_baseline and world == 1:
+    if not args.no_cpu_baseline:
         n_mk = min(cfg.M, 64)
         ev_s, dt, n = time_oracle(cfg, n_mk, S)
         line["cpu_baseline"] = {"value": ev_s, "unit": "events/s", "cores": 1, "kind": "oracle",
@@ -450,10 +580,92 @@ def main():
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
-# `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 25261312 + 237688320,            # profiles/r1h_persistent_full.md
-                                  "C4_packed4": 23691008 + 254493952}    # profiles/r1g_packed_persistent_full.md
+# dram__bytes_read.sum + dram__bytes_write.sum summed over the launches, from the ncu captures of
+# `bench.py --case C2 --M 128 --S {100,1000} --mode {persistent,stepwise}` (profiles/r2_traffic.md):
+# measured counters, not algorithmic bytes.  Filled in when the capture exists.
+PROFILED_TRAFFIC_C2_M128 = None
+
+
+def extras(ks, torch, dev, peak_tmults, headline_cfg):
+    """The other BASELINE configs, the other contracts and the ablation, timed in the same process
+    (each a few ms to a few hundred ms of GPU time): every number DESIGN.md quotes is in the
+    driver-run line.  frac_executed = executed multiplies/s over the same measured peak as the
+    headline's roofline."""
+    out = {}
+
+    def with_frac(r, c):
+        mk = model_key(c.params)
+        r["frac_executed"] = EXEC_MULTS_PER_EVENT[mk] * r["events_per_s"] / 1e12 / peak_tmults
+        r["us_per_step"] = r["ms"] * 1e3 / r["S"]
+        return r
+
+    allc = {}
+    for name in sorted(CONFIGS):
+        if name == headline_cfg.name and headline_cfg.params == CONFIGS[name].params:
+            continue
+        c = CONFIGS[name]
+        allc[name] = with_frac(time_case(ks, torch, dev, c, reps=5 if c.events < 5e10 else 3), c)
+    out["all_configs"] = allc
+    for key, case in (("packed4_C4", "C4_packed4"), ("model4_C4shape", "model4_C4shape")):
+        c = case_config(case)
+        out[key] = with_frac(time_case(ks, torch, dev, c, reps=3), c)
+    out["packed4_C4"]["note"] = "PACKED4 draw contract (DESIGN.md A22): NOT the BASELINE.json contract, reported beside it"
+    out["model4_C4shape"]["note"] = ("the paper's own agent model (DESIGN.md A24) on the C4 shape, alpha_mom = alpha_maker = 0.15, "
+                                     "Delta = 32, q <= 100, P_mkt = 0.02 (parameter values ours: the paper gives none)")
+
+    # a8 ablation on C2: one launch per step, book through HBM every step (PAPER.md:222-224)
+    c = CONFIGS["C2"]
+    pers = allc.get("C2") or time_case(ks, torch, dev, c, reps=5)
+    sw = time_case(ks, torch, dev, c, reps=3, mode="stepwise")
+    out["ablation_launch_per_step_C2"] = {
+        "ms": sw["ms"], "events_per_s": sw["events_per_s"], "launches": c.S, "persistent_ms": pers["ms"],
+        "slowdown_vs_persistent": sw["ms"] / pers["ms"],
+        "algorithmic_hbm_bytes": float(c.S) * c.M * 2 * (8 * c.L + 128), "persistent_algorithmic_hbm_bytes": float(c.M) * (8 * c.L + 128),
+        "measured_dram_bytes": PROFILED_TRAFFIC_C2_M128}
+
+    # context runs in the paper's own shapes (SURVEY.md S8(d)): Table IV's fixed workload and the
+    # latency configuration (PAPER.md:384-394, 438) with zero-intelligence agents -- NOT the paper's
+    # agent model or GPU
+    ctx = {}
+    for name in ("table4", "latency"):
+        c = case_config(name)
+        ctx["%s_M%d_A%d_L%d_S%d" % (name, c.M, c.A, c.L, c.S)] = with_frac(time_case(ks, torch, dev, c, reps=5), c)
+    ctx["paper"] = "KineticSim on RTX 5090: 20.2 ms, 5.2e10 events/s (Table IV); 22.1 us median per step at M=4096 (PAPER.md:438)"
+    out["paper_shape_context"] = ctx
+
+    # SIV-J sweep shape (PAPER.md:442-458): alpha_mom = 0 .. 0.70 in steps of 0.05, alpha_maker =
+    # 0.15, M = 64 markets x S = 1000 steps each, the paper's own agent model (model 4), traced,
+    # statistics on the device.  A = 200 (12.8e6 events / 64 / 1000: PAPER.md:458); L, Delta, q_max,
+    # P_mkt are not given -- workloads.paper_params defaults.  Context, not a parity case.
+    Ms, Ls, As, Ss, K = 64, 128, 200, 1000, 20
+    st = torch.empty(ks.ks_state_bytes(Ms, Ls), dtype=torch.uint8, device=dev)
+    tr = torch.empty((Ms, Ss, 2), dtype=torch.int32, device=dev)
+    res = torch.empty((Ms, 4 + 2 * K), dtype=torch.float64, device=dev)
+    alphas = [round(0.05 * i, 2) for i in range(15)]
+    rows = []
+
+    def sweep(record):
+        for al in alphas:
+            sim = ks.KsSim(Ms, Ls, As, paper_params(As, al), 5, state=st)
+            sim.ks_run_traced(Ss, tr)
+            ks.ks_trace_stats(tr, Ms, Ss, K, res)
+            if record:
+                o = res.cpu().numpy()
+                rows.append({"alpha_mom": al, "volatility": float(np.nanmean(o[:, 0])), "excess_kurtosis": float(np.nanmean(o[:, 1])),
+                             "volume_per_step": float(np.nanmean(o[:, 2])), "acf_r_lag1": float(np.nanmean(o[:, 4])),
+                             "acf_abs_r_lag1": float(np.nanmean(o[:, 4 + K]))})
+            sim.ks_destroy()
+
+    sweep(False)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); sweep(False); b.record(); torch.cuda.synchronize()
+    sweep(True)
+    out["sivj_sweep"] = {"configs": len(alphas), "M": Ms, "L": Ls, "A": As, "S": Ss, "agent_events": len(alphas) * Ms * As * Ss,
+                         "ms_total_device": a.elapsed_time(b), "paper": "< 250 ms for 12.8e6 events (RTX 5090, PAPER.md:458)",
+                         "mean_over_markets": rows}
+    return out
+
 
 if __name__ == "__main__":
     main()

@@ -13,7 +13,7 @@ LIB = os.path.join(HERE, "libkineticsim.so")
 BENCH_LIB = os.path.join(HERE, "libkineticsim_bench.so")
 SOURCES = ["ks_api.cu"]
 BENCH_SOURCES = ["ks_microbench.cu"]
-HEADERS = ["ks_device.cuh", "ks_kernel.cuh", "ks_cluster.cuh", "ks_trace.cuh", os.path.join("..", "..", "include", "kineticsim.h"),
+HEADERS = ["ks_device.cuh", "ks_kernel.cuh", "ks_cluster.cuh", "ks_decoupled.cuh", "ks_trace.cuh", os.path.join("..", "..", "include", "kineticsim.h"),
            os.path.join("..", "..", "include", "kineticsim_bench.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static"]

@@ -110,3 +110,30 @@ def assert_rows_equal(gpu_books, gpu_recs, ids, exp_books, exp_recs, what=""):
         i, s, p = bad[0]
         raise AssertionError("%s: book mismatch at market %d side %d tick %d: gpu %d oracle %d (%d mismatches)"
                              % (what, ids[i], s, p, gb[i, s, p], exp_books[i, s, p], len(bad)))
+
+
+def sass_innermost_loops(sass_text, function_substring):
+    """Innermost loops of one kernel in `cuobjdump -sass` output: a loop is the address range of a
+    backward branch; -> list of dict(n=instructions, atoms=ATOMS count, mults=IMAD.WIDE.U32 +
+    IMAD.HI.U32 count, lop3=...) for the loops that contain no other loop."""
+    import re
+    bodies = [p for p in sass_text.split("Function : ") if function_substring in p.split("\n", 1)[0]]
+    assert len(bodies) == 1, "%d kernels match %r" % (len(bodies), function_substring)
+    ins = []
+    for line in bodies[0].splitlines():
+        m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(.*?);", line)
+        if m:
+            ins.append((int(m.group(1), 16), m.group(2)))
+    loops = []
+    for addr, text in ins:
+        m = re.search(r"\bBRA\b.*?0x([0-9a-f]+)", text)
+        if m and int(m.group(1), 16) <= addr:
+            loops.append((int(m.group(1), 16), addr))
+    inner = [(lo, hi) for lo, hi in loops if not any((l2, h2) != (lo, hi) and lo <= l2 and h2 <= hi for l2, h2 in loops)]
+    out = []
+    for lo, hi in inner:
+        body = [t for a, t in ins if lo <= a <= hi]
+        out.append(dict(n=len(body), atoms=sum("ATOMS" in t for t in body),
+                        mults=sum("IMAD.WIDE.U32" in t or "IMAD.HI.U32" in t for t in body),
+                        lop3=sum("LOP3" in t for t in body)))
+    return out

@@ -51,7 +51,7 @@ def test_libraries_export_every_declared_symbol(lib):
 def test_product_library_never_allocates_device_memory():
     """include/kineticsim.h: the state buffer is the caller's; the product library holds no
     cudaMalloc / cudaFree call (the bench library may, and says so)."""
-    for f in ("ks_api.cu", "ks_kernel.cuh", "ks_device.cuh", "ks_cluster.cuh", "ks_trace.cuh"):
+    for f in ("ks_api.cu", "ks_kernel.cuh", "ks_device.cuh", "ks_cluster.cuh", "ks_decoupled.cuh", "ks_trace.cuh"):
         src = open(os.path.join(ROOT, "paper_2606_21784_b200", "csrc", f)).read()
         assert not re.search(r"\bcudaMalloc\w*\s*\(|\bcudaFree\s*\(", src), f
     out = subprocess.check_output(["nm", "-D", "--undefined-only", binding.LIB_PATH]).decode()
@@ -65,6 +65,35 @@ def test_library_is_sm100a_with_shared_atomics():
     assert "sm_100a" in out
     body = out.split("ks_persistent_kernel")[1]
     assert "ATOMS" in body and "REDUX" in body and "IMAD.WIDE.U32" in body
+
+
+def test_hot_loops_execute_the_multiplies_bench_reports():
+    """bench.py turns events/s into executed multiplies/s with EXEC_MULTS_PER_EVENT; count them in
+    the SASS of the built library so that the constants cannot go stale: per unrolled hot loop (4
+    events, or 2 PACKED4 blocks of 4 agents), IMAD.WIDE.U32 + IMAD.HI.U32 per event."""
+    import bench
+    from ks_testlib import sass_innermost_loops
+    sass = subprocess.check_output(["cuobjdump", "-sass", binding.LIB_PATH]).decode()
+    per = bench.EXEC_MULTS_PER_CLASS
+
+    def hot(kernel, min_atoms):
+        return [l for l in sass_innermost_loops(sass, kernel) if l["atoms"] >= min_atoms]
+
+    zi = hot("ks_persistent_kernelILi0ELi0ELb0EEE", 4)                 # no-clamp and clamp noise loops
+    assert len(zi) == 2 and {l["mults"] / 4 for l in zi} == {per["noise"]} == {bench.EXEC_MULTS_PER_EVENT["zi"]}
+    assert all(l["atoms"] == 4 for l in zi)
+    mix = hot("ks_persistent_kernelILi1ELi0ELb0EEE", 4)                # noise / maker / momentum x no-clamp / clamp
+    assert len(mix) == 6
+    assert {l["mults"] / 4 for l in mix} == {per["noise"], per["maker"], per["momentum"]}
+    assert min(l["mults"] for l in mix if l["atoms"] == 8) / 4 == per["maker"]          # the no-clamp maker loop
+    pk = hot("ks_persistent_kernelILi0ELi0ELb1EEE", 8)                 # 2 blocks x 4 agents per iteration
+    assert len(pk) == 2 and {l["mults"] / 8 for l in pk} == {bench.EXEC_MULTS_PER_EVENT["zi_packed4"]}
+    assert bench.EXEC_MULTS_PER_EVENT["zi_packed4"] == per["packed_block"] / 4 + 2
+    pm = hot("ks_persistent_kernelILi1ELi0ELb1EEE", 8)                 # three block classes x no-clamp / clamp
+    assert len(pm) == 6 and sum(l["mults"] for l in pm) / (6 * 8) == pytest.approx(bench.EXEC_MULTS_PER_EVENT["mix3_packed4"])
+    pa = hot("ks_persistent_kernelILi2ELi0ELb0EEE", 4)                 # model 4: three classes x no-clamp / clamp
+    assert len(pa) == 6
+    assert {l["mults"] / 4 for l in pa} == {per["paper_noise"], per["paper_momentum"], per["paper_maker"]}
 
 
 def test_state_bytes(lib):
