@@ -242,14 +242,18 @@ typedef enum {
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
   KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
   KS_OPT_PIPELINE = 4,      /* the decoupled kernel (generating warps fill a price-independent relative order
-                               histogram up to two steps ahead; one clearing warp per market, holding no
+                               histogram up to KS_OPT_RING_DEPTH steps ahead; one clearing warp per market, holding no
                                agents, merges it at the step's price and clears): 0 = automatic (when the
                                grid underfills the GPU, i.e. step latency is what counts), 1 = never,
                                2 = whenever legal (KS_MODEL_ZI / KS_MODEL_ZI_PACKED4, plain atomics,
-                               >= 64 threads, L <= 16384, book + two histograms fit shared memory)          */
+                               >= 64 threads, L <= 16384, book + the histogram ring fit shared memory)          */
   KS_OPT_REL_COLUMNS = 5,   /* decoupled kernel only: 0 = one int32 per histogram bin, 1 = 32 lane columns per
                                bin (column = lane = bank: a warp's atomics never conflict) -- the
                                aggregation ablation of north_star (3)                                       */
+  KS_OPT_RING_DEPTH = 6,    /* decoupled kernel only: how many steps the generating warps may run ahead of the
+                               clearing warp = number of relative histograms in the ring: 0 = automatic (4; 2 with
+                               KS_OPT_REL_COLUMNS), 2 or 4 (ablation: the two-deep ring leaves both sides waiting
+                               for each other's hand-over)                                                    */
   KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
                                i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
                                book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and

@@ -46,7 +46,7 @@ struct ks_sim {
   int64_t steps_done;
   int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books / found by ks_attach
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe, opt_cols;
+  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe, opt_cols, opt_ring;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
   unsigned long long* h_words;   // pinned, mapped host memory: [0] depth bound of ks_write_books (copied),
@@ -154,7 +154,7 @@ ks_status create_common(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_
   if (!s) { set_err("%s: out of host memory", who); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
   s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = attach ? 0 : 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0; s->opt_cols = 0;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0; s->opt_cols = 0; s->opt_ring = 0;
   s->dev_smem_optin = optin; s->num_sms = sms; s->device = dev;
   s->bound_pending = 0; s->h_words = nullptr; s->d_flags = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_PAPER) {
@@ -274,6 +274,9 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_REL_COLUMNS:
       if (value != 0 && value != 1) break;
       s->opt_cols = value; return KS_OK;
+    case KS_OPT_RING_DEPTH:
+      if (value != 0 && value != 2 && value != 4) break;
+      s->opt_ring = value; return KS_OK;
     case KS_OPT_CLUSTER_SIZE:
       if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break;
       if (value > 1 && (s->L / value < 32 || s->opt_atomic || s->p.model == KS_MODEL_PAPER)) break;
@@ -296,7 +299,7 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 // T = 32 beats 64/128 on C4).  A book so large that 32-thread CTAs would leave the SM short of
 // warps -> widen until ~1024 threads are resident; few markets -> widen so the whole GPU is used,
 // but never beyond the agents.
-struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; };
+struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
 
@@ -310,7 +313,7 @@ static uint32_t rel_side_for(const ks_sim* s) {
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
   pl.smem = (size_t)8 * (size_t)s->L;
-  pl.decoupled = false; pl.rel_side = 0;
+  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0;
   int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
   if (k < 1) k = 1;
   if (k > 32) k = 32;
@@ -334,14 +337,17 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   if (zi && !s->opt_atomic && s->opt_pipe != 1) {
     const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
     const uint32_t side = rel_side_for(s);
-    const bool fits = pl.smem + 4 * (size_t)side + 2048 <= (size_t)s->dev_smem_optin;
+    // ring depth: 4 histograms (the lane-columned ablation layout keeps the two-deep ring)
+    const int ring = s->opt_ring ? s->opt_ring : (s->opt_cols ? 2 : 4);
+    const bool fits = pl.smem + 2 * (size_t)ring * side + 2048 <= (size_t)s->dev_smem_optin && !(s->opt_cols && ring != 2);
     if (fits && (s->opt_pipe == 2 || underfilled)) {
       int Td = pl.T;
       if (!s->opt_threads) {
-        Td = 64;
-        while (Td < 1024 && (long long)(Td - 32) * 3 < s->A) Td *= 2;
+        // 4k generating warps (one, two, four per scheduler) + the clearing warp; <= 3 events per thread
+        Td = 160;
+        while (Td < 544 && (long long)(Td - 32) * 3 < s->A) Td = 2 * (Td - 32) + 32;
       }
-      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.smem += 4 * (size_t)side; }
+      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem += 2 * (size_t)ring * side; }
     }
   }
   return pl;
@@ -358,15 +364,26 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
   return cudaGetLastError();
 }
 
-template <bool PACKED, int COLS>
-static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_decoupled_kernel<PACKED, COLS>;
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB>
+static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
+  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   if (e != cudaSuccess) return e;
   kern<<<P.M, T, smem, st>>>(P);
   return cudaGetLastError();
+}
+
+// The decoupled kernel's instantiations: ring of 4 histograms (default) -- with the register budget
+// of 7 resident CTAs of <= 160 threads when the block is that small (C2: 6.9 markets per SM must all
+// be resident) -- or the two-deep ring (ablation; the only one with lane-columned bins).
+template <bool PACKED>
+static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, cudaStream_t st) {
+  if (cols) return launch_decoupled_as<PACKED, 32, 2, 1024, 1>(P, T, smem, st);
+  if (ring == 2) return launch_decoupled_as<PACKED, 1, 2, 1024, 1>(P, T, smem, st);
+  if (T <= 160) return launch_decoupled_as<PACKED, 1, 4, 160, 7>(P, T, smem, st);
+  return launch_decoupled_as<PACKED, 1, 4, 1024, 1>(P, T, smem, st);
 }
 
 // Cluster launch: grid = M*C CTAs in clusters of C (cluster <-> market), 8*L/C bytes of shared
@@ -471,8 +488,8 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     const LaunchPlan pl = plan_launch(s);
     P.rel_side = pl.rel_side; P.rel_stride = 2 * pl.rel_side;
     if (pl.decoupled) {
-      if (s->opt_cols) e = packed ? launch_decoupled<true, 32>(P, pl.T, pl.smem, st) : launch_decoupled<false, 32>(P, pl.T, pl.smem, st);
-      else             e = packed ? launch_decoupled<true, 1>(P, pl.T, pl.smem, st) : launch_decoupled<false, 1>(P, pl.T, pl.smem, st);
+      e = packed ? launch_decoupled<true>(P, pl.T, pl.smem, s->opt_cols, pl.ring, st)
+                 : launch_decoupled<false>(P, pl.T, pl.smem, s->opt_cols, pl.ring, st);
     } else if (paper)
       e = launch_persistent<2, 0, false>(P, pl.T, pl.smem, st);
     else if (packed)

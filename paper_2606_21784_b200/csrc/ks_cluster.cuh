@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(1024, 1) ks_cluster_kernel(const __grid_consta
       LaneBounds lbnd;
       int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
       if (P.force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, lbnd); }
-      else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, lbnd); }
+      else if (hi - lo < 32)               { base = lo; wend = min(L, base + 32); clear_rows<1>(io, L, base, lane, vmax, pstar, lbnd); }
       else if (width4 <= 128)              { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, lbnd); }
       else                                 { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, lbnd); }
       reduce_bounds(lbnd, base, wend, nb, na);

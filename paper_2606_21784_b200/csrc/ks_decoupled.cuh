@@ -1,22 +1,25 @@
-// ks_decoupled.cuh -- the latency kernel: order generation DECOUPLED from the clearing price.
+// ks_decoupled.cuh -- order generation DECOUPLED from the clearing price.
 //
 // In ks_persistent_kernel a step is a chain: generate (needs the price) | barrier | clear (gives
-// the next price) | barrier.  When many markets share an SM they hide each other's chains (C4);
-// when the grid underfills the GPU (C3: 32 markets, C1: one) the chain IS the run time.  But for a
+// the next price) | barrier.  When many markets share an SM and every market brings many agents
+// (C4), the markets hide each other's chains; with few markets per SM (C2: 7) or one (C3, C1) the
+// chain IS the run time: while one warp clears, the market's other warps idle at the barrier
+// (ncu on C2, profiles/r2a_c2_persistent.md: 42 % of all warp samples).  But for a
 // zero-intelligence agent only the TICK depends on the price, not the order: offset draw o, side
 // and quantity are pure functions of (seed, market, step, agent).  So here the generating warps
 // never see a price.  They add their orders to a relative histogram (sell[o], buy[n-1-o]: bin i of
-// either side means tick last - delta + i; ATOM 4 / 5 of ks_device.cuh), double-buffered by step
-// parity, and run up to two steps ahead; ONE clearing warp per market (which holds no agents) takes
-// buffer (s & 1) at the current price -- exactly the rule's ticks, clamped to the grid -- zeroes it,
-// hands it back, and clears (a3-a6).  In the common case (no order clamped, window <= 128 ticks)
-// the histogram is not even merged into the book first: each lane adds its ticks' bins to the
-// depth it loads for the scan.  The per-step critical path is max(generate, clear) with no price
-// round trip between the two, and the SM's other warps never idle at a barrier.
+// either side means tick last - delta + i; ATOM 4 / 5 of ks_device.cuh) taken from a RING of NB
+// histograms, and run up to NB steps ahead; ONE clearing warp per market (which holds no agents)
+// takes histogram s mod NB at the current price -- exactly the rule's ticks, clamped to the grid --
+// zeroes it, hands it back, and clears (a3-a6).  In the common case (no order clamped, window <=
+// 128 ticks) the histogram is not even merged into the book first: each lane adds its ticks' bins
+// to the depth it loads for the scan.  With a ring deep enough to absorb the hand-over latency
+// (measured: a two-deep ring leaves BOTH sides waiting for each other a third of the time) the
+// step time is max(generate, clear), and the SM's warps never idle at a barrier.
 //
-// Synchronisation: four named barriers, full[b] (generating warps arrive, clearing warp waits)
-// and free[b] (clearing warp arrives, generating warps wait), b = step parity.  A generating warp
-// can be at most two steps ahead of the clearing warp, so phases of one barrier never overlap.
+// Synchronisation: 2*NB named barriers, full[b] (generating warps arrive, clearing warp waits)
+// and free[b] (clearing warp arrives, generating warps wait), b = step mod NB.  A generating warp
+// can be at most NB steps ahead of the clearing warp, so phases of one barrier never overlap.
 // Same orders, same integer sums, same bytes as ks_persistent_kernel (tests).
 //
 // COLS = 1: one int32 per bin.  COLS = 32: the lane-columned layout -- 32 columns per bin, column =
@@ -28,43 +31,69 @@
 
 namespace ks {
 
-enum { kBarFull0 = 1, kBarFree0 = 3 };     // full[b] = 1 + b, free[b] = 3 + b; barrier 0 = __syncthreads()
-
-// barrier base + b with an immediate id in either branch (b is CTA-uniform)
-template <int BASE> __device__ __forceinline__ void bar_sync_b(int b, int n) { if (b) bar_sync<BASE + 1>(n); else bar_sync<BASE>(n); }
-template <int BASE> __device__ __forceinline__ void bar_arrive_b(int b, int n) { if (b) bar_arrive<BASE + 1>(n); else bar_arrive<BASE>(n); }
+// barrier ids: full[b] = 1 + b, free[b] = 1 + NB + b; barrier 0 = __syncthreads().  The id must be
+// an immediate (ks_kernel.cuh), hence the switch over the CTA-uniform b.
+template <int BASE, int NB> __device__ __forceinline__ void bar_sync_b(int b, int n) {
+  static_assert(NB == 2 || NB == 4, "ring depth");
+  if (NB == 2) { if (b) bar_sync<BASE + 1>(n); else bar_sync<BASE>(n); }
+  else {
+    switch (b) {
+      case 0: bar_sync<BASE>(n); break;
+      case 1: bar_sync<BASE + 1>(n); break;
+      case 2: bar_sync<BASE + (NB > 2 ? 2 : 0)>(n); break;
+      default: bar_sync<BASE + (NB > 2 ? 3 : 1)>(n); break;
+    }
+  }
+}
+template <int BASE, int NB> __device__ __forceinline__ void bar_arrive_b(int b, int n) {
+  if (NB == 2) { if (b) bar_arrive<BASE + 1>(n); else bar_arrive<BASE>(n); }
+  else {
+    switch (b) {
+      case 0: bar_arrive<BASE>(n); break;
+      case 1: bar_arrive<BASE + 1>(n); break;
+      case 2: bar_arrive<BASE + (NB > 2 ? 2 : 0)>(n); break;
+      default: bar_arrive<BASE + (NB > 2 ? 3 : 1)>(n); break;
+    }
+  }
+}
 
 __device__ __forceinline__ int lds32(uint32_t saddr) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory"); return v; }
 __device__ __forceinline__ void sts32(uint32_t saddr, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory"); }
 __device__ __forceinline__ void red32(uint32_t saddr, int v) { asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory"); }
 
-// grid = M CTAs (one per market), block = T >= 64 threads, dynamic shared memory =
-// 8*L + 2 * P.rel_stride bytes: the book, then the two relative histograms.  One histogram =
-// sell bins then buy bins (P.rel_side bytes each), bin i of either side <-> tick (last - delta) + i
-// (ks_device.cuh, rel_bin_addr).
+// grid = M CTAs (one per market), block = T >= 64 threads (<= MAXT), dynamic shared memory =
+// 8*L + NB * P.rel_stride bytes: the book, then the ring of NB relative histograms.  One histogram
+// = sell bins then buy bins (P.rel_side bytes each), bin i of either side <-> tick (last - delta) + i
+// (ks_device.cuh, rel_bin_addr).  MAXT / MINB: launch bounds (the register budget that lets MINB
+// CTAs of MAXT threads share an SM -- C2 needs 7 markets of 160 threads resident per SM).
 //
 // Roles.  The CLEARING warp's loop is the serial chain of the whole run (a single warp issues a
-// dependent instruction every ~5 cycles, so its length in instructions is the step time): it
+// dependent instruction every ~5-10 cycles, so its length in instructions is the step time): it
 // holds only what the next step needs -- take the histogram, scan, price, residual, bounds -- and
-// posts (Vmax, p*, price before) in a two-slot mailbox.  The record (a6) and the trace are kept by
-// the FIRST GENERATING warp, which picks the mail of step s-2 up when it passes the free[] barrier
-// it waits at anyway; the last two mails are taken after the loop.
-template <bool PACKED, int COLS>
-__global__ void __launch_bounds__(1024, 1) ks_decoupled_kernel(const __grid_constant__ KernelParams P) {
-  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then rel[2][P.rel_stride / 4]
+// posts (Vmax, p*, price before) in an NB-slot mailbox.  The record (a6) and the trace are kept by
+// the FIRST GENERATING warp, which picks the mail of step s-NB up when it passes the free[]
+// barrier it waits at anyway; the last NB mails are taken after the loop.
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_constant__ KernelParams P) {
+  extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then rel[NB][P.rel_stride / 4]
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
   __shared__ int s_red32[64];
   __shared__ int2 s_trace[32];
-  __shared__ __align__(16) int s_mail[2][4];          // per step parity: Vmax, p*, price before the step
+  __shared__ __align__(16) int s_mail[NB][4];         // per ring slot: Vmax, p*, price before the step
   __shared__ int s_abort;
   __shared__ int s_ovf;
   __shared__ long long s_keep[3];
   constexpr int ATOM = COLS == 1 ? 4 : 5;
+  constexpr int kBarFull0 = 1, kBarFree0 = 1 + NB;
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
   const int L = P.L;
-  const int cw = (int)(blockIdx.x % (unsigned)nwarps);     // the clearing warp (spread over the SM's schedulers)
+  // The clearing warp is the LAST warp and the block has 4k+1 warps (ks_api.cu): warps map to the
+  // SM's four schedulers by index, so the 4k generating warps load the schedulers evenly and the
+  // clearing warp shares scheduler 0 (measured on C2: with the clearing warp rotating over the
+  // warp indices, scheduler 0 carried two generating warps of most markets: 4.1 ms vs 3.6 ms).
+  const int cw = nwarps - 1;
   const bool clearing = warp == cw;
   const uint32_t market = P.market_base + blockIdx.x;
   int32_t* gbook = P.books + (size_t)blockIdx.x * 2 * (size_t)L;
@@ -79,7 +108,7 @@ __global__ void __launch_bounds__(1024, 1) ks_decoupled_kernel(const __grid_cons
   long long sb0, sa0;
   int bmax, amin;
   load_book(P, book, gbook, L, sb0, sa0, bmax, amin);
-  for (int i = tid; i < (int)(P.rel_stride / 2); i += T) rel[i] = 0;      // both buffers
+  for (int i = tid; i < (int)(NB * (P.rel_stride / 4)); i += T) rel[i] = 0;      // the whole ring
   if (tid < 16) s_rec[tid] = grec[tid];
   if (tid == 0) s_ovf = 0;
   BookTotals tot0 = block_reduce_totals(sb0, sa0, bmax, amin, s_red64, s_red32);   // has barriers
@@ -90,68 +119,58 @@ __global__ void __launch_bounds__(1024, 1) ks_decoupled_kernel(const __grid_cons
   const uint32_t S = (uint32_t)P.S;
   if (tid == 0) { s_keep[0] = tot0.sum_bid; s_keep[1] = tot0.sum_ask; s_keep[2] = s_rec[F_SUMVOL]; }
   __syncthreads();
-  const int gtid = tid - (warp > cw ? 32 : 0);             // generating threads: 0 .. T-33, the clearing warp left out
-  const bool bookkeeper = !clearing && gtid < 32;          // the first generating warp keeps the record and the trace
-  auto take_mail = [&](uint32_t s_of_mail) {               // a6 (+ trace) of one cleared step, in step order
-    const int4 m = *reinterpret_cast<const int4*>(s_mail[s_of_mail & 1u]);
-    update_record_lanes(s_rec, &s_ovf, lane, m.z, m.x, m.y, m.z);
+  const bool bookkeeper = warp == 0;                       // the first generating warp keeps the record and the trace
+  long long rec_reg = s_rec[lane & 15];                    // ... lane f (and f + 16) holding field f in a register
+  int ovf_reg = 0;
+  auto take_mail = [&](uint32_t s_of_mail, int slot) {     // a6 (+ trace) of one cleared step, in step order
+    const int4 m = *reinterpret_cast<const int4*>(s_mail[slot]);
+    update_record_reg(rec_reg, ovf_reg, lane, m.z, m.x, m.y, m.z);
     if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)s_of_mail, (long long)S, lane,
                             m.x > 0 ? m.y : m.z, m.x);
-    __syncwarp();
   };
 
   if (clearing) {
     const LocalBook io{book, L};
     const unsigned FULL = 0xffffffffu;
-    // lane masks of the 5-step scans (all-ones where the shuffled value is in range)
-    int mdn[5], mup[5];
+    for (uint32_t s0 = 0; s0 < S; s0 += NB) {
 #pragma unroll
-    for (int k = 0; k < 5; ++k) { mdn[k] = lane + (1 << k) < 32 ? -1 : 0; mup[k] = lane >= (1 << k) ? -1 : 0; }
-    for (uint32_t s = 0; s < S; ++s) {
-      const int buf = (int)(s & 1u);
-      const uint32_t rs = rel_saddr + (uint32_t)buf * P.rel_stride;   // sell bins of this step's histogram
-      const uint32_t rb = rs + P.rel_side;                           // buy bins
-      const int t_lo = last - delta;                       // tick of bin 0
-      const int lo = max(0, min(amin, t_lo));
-      const int hi = min(L - 1, max(bmax, last + delta));
-      const bool inside = t_lo >= 0 && last + delta <= L - 1;   // no order of this step is clamped
-      int vmax, pstar, nb, na;
-      bar_sync_b<kBarFull0>(buf, T);                       // every order of step s is in the histogram
-      if (COLS == 1 && inside && !P.force_generic && hi - lo < 32) {
-        // ---- a2 (second half) fused into a3-a5, one tick per lane, raw shared addresses:
-        // a lane adds its tick's two bins to the depth it scans (clear_window1's definitions)
-        const int tick = lo + lane, i = tick - t_lo;       // this lane's tick and bin
-        const bool in = tick < L, has = (unsigned)i < (unsigned)n;
-        const uint32_t pb = book_saddr + 4u * (uint32_t)tick, pa = pb + 4u * (uint32_t)L;
-        const int b0 = in ? lds32(pb) : 0, a0 = in ? lds32(pa) : 0;
-        const int inc_a = has ? lds32(rs + 4u * (uint32_t)i) : 0, inc_b = has ? lds32(rb + 4u * (uint32_t)i) : 0;
-        if (inc_a != 0) sts32(rs + 4u * (uint32_t)i, 0);
-        if (inc_b != 0) sts32(rb + 4u * (uint32_t)i, 0);
-        int b = b0 + inc_b, a = a0 + inc_a;
-        int D = b, Sc = a;                                 // inclusive suffix of bids / prefix of asks over lanes
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-          const int vb = __shfl_down_sync(FULL, D, 1 << k), va = __shfl_up_sync(FULL, Sc, 1 << k);
-          D += vb & mdn[k];
-          Sc += va & mup[k];
-        }
-        const int V = min(D, Sc);
-        vmax = __reduce_max_sync(FULL, V);
-        pstar = __reduce_min_sync(FULL, (V == vmax && vmax > 0) ? tick : 0x7fffffff);
-        if (vmax > 0) { b = min(b, max(0, D - vmax)); a = min(a, max(0, Sc - vmax)); }
-        if (in && b != b0) sts32(pb, b);
-        if (in && a != a0) sts32(pa, a);
-        if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
-        __syncwarp();
-        if (s + 2 < S) bar_arrive_b<kBarFree0>(buf, T);    // histogram empty again, mail posted: step s+2 may start
-        nb = __reduce_max_sync(FULL, b > 0 ? tick : -1);
-        na = __reduce_min_sync(FULL, a > 0 ? tick : 0x7fffffff);
-        if (nb < 0) nb = lo - 1;
-        if (na == 0x7fffffff) na = min(L, lo + 32);
-      } else {
-        int base, wend;
+      for (int buf = 0; buf < NB; ++buf) {                 // ring slot = step mod NB, a compile-time constant here
+        const uint32_t s = s0 + (uint32_t)buf;
+        if (s >= S) break;
+        const uint32_t rs = rel_saddr + (uint32_t)buf * P.rel_stride;   // sell bins of this step's histogram
+        const uint32_t rb = rs + P.rel_side;                           // buy bins
+        const int t_lo = last - delta;                     // tick of bin 0
+        const int lo = max(0, min(amin, t_lo));
+        const int hi = min(L - 1, max(bmax, last + delta));
+        const bool inside = t_lo >= 0 && last + delta <= L - 1;   // no order of this step is clamped
+        const bool fuse = COLS == 1 && inside && !P.force_generic;
+        int vmax, pstar, base, wend;
         LaneBounds lbnd;
-        if (COLS == 1 && inside && !P.force_generic && hi - (lo & ~3) + 1 <= 128) {
+        bar_sync_b<kBarFull0, NB>(buf, T);                 // every order of step s is in the histogram
+        if (fuse && hi - lo < 32) {
+          // this lane's bins of tick lo + lane (a2, second half): read and zeroed here, added to the
+          // depth inside the scan
+          int ib[1], ia[1];
+          base = lo; wend = min(L, lo + 32);
+          const int i = lo + lane - t_lo;
+          const bool has = (unsigned)i < (unsigned)n;
+          ia[0] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[0] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
+          if (ia[0] != 0) sts32(rs + 4u * (uint32_t)i, 0);
+          if (ib[0] != 0) sts32(rb + 4u * (uint32_t)i, 0);
+          clear_rows<1, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
+        } else if (fuse && hi - lo < 64) {
+          int ib[2], ia[2];
+          base = lo; wend = min(L, lo + 64);
+#pragma unroll
+          for (int r = 0; r < 2; ++r) {
+            const int i = lo + 32 * r + lane - t_lo;
+            const bool has = (unsigned)i < (unsigned)n;
+            ia[r] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[r] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
+            if (ia[r] != 0) sts32(rs + 4u * (uint32_t)i, 0);
+            if (ib[r] != 0) sts32(rb + 4u * (uint32_t)i, 0);
+          }
+          clear_rows<2, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
+        } else if (fuse && hi - (lo & ~3) + 1 <= 128) {
           base = lo & ~3; wend = min(L, base + 128);
           int ib[4], ia[4];
 #pragma unroll
@@ -200,16 +219,17 @@ __global__ void __launch_bounds__(1024, 1) ks_decoupled_kernel(const __grid_cons
         }
         if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
         __syncwarp();
-        if (s + 2 < S) bar_arrive_b<kBarFree0>(buf, T);
+        if (s + NB < S) bar_arrive_b<kBarFree0, NB>(buf, T);   // histogram empty again, mail posted: step s+NB may start
+        int nb, na;
         reduce_bounds(lbnd, base, wend, nb, na);
+        bmax = nb; amin = na;
+        last = vmax > 0 ? pstar : last;
       }
-      bmax = nb; amin = na;
-      last = vmax > 0 ? pstar : last;
     }
   } else {
-    // ---- a1 + a2 (first half) by the generating threads
+    // ---- a1 + a2 (first half) by the generating threads tid 0 .. T-33
     const MarketUniform mu = market_uniform(P, market);
-    const GenPlan<0> gplan = gen_plan<0>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, gtid, T - 32);
+    const GenPlan<0> gplan = gen_plan<0>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, tid, T - 32);
     // the most agents any generating thread holds (CTA-uniform); <= 4 takes the latency path
     const uint32_t nmax = PACKED ? 99u : gplan.cls[0].n_uniform + ((uint32_t)P.A % (uint32_t)(T - 32) != 0u ? 1u : 0u);
     BookRef bref; bref.ptr = book; bref.saddr = 0;
@@ -219,27 +239,39 @@ __global__ void __launch_bounds__(1024, 1) ks_decoupled_kernel(const __grid_cons
     const uint32_t col = COLS == 32 ? 4u * (uint32_t)lane : 0u;
     const uint32_t bin_bytes = COLS == 32 ? 128u : 4u;
     int sink = 0;
-    for (uint32_t s = 0; s < S; ++s) {
-      const int buf = (int)(s & 1u);
-      const StepUniform u = step_uniform(P, mu, t0 + s);
-      rc.rel_s = rel_saddr + (uint32_t)buf * P.rel_stride + col;
-      rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * bin_bytes;
-      if (s >= 2) {
-        bar_sync_b<kBarFree0>(buf, T);                     // the clearing warp has drained this histogram (step s-2)
-        if (bookkeeper) take_mail(s - 2);
+    // the whole step loop, instantiated per N = events a thread holds (0 = the general loop), so that
+    // nothing about N is decided inside it
+    auto gen_loop = [&](auto Ntag) {
+      constexpr int N = decltype(Ntag)::value;
+      for (uint32_t s0 = 0; s0 < S; s0 += NB) {
+#pragma unroll
+        for (int buf = 0; buf < NB; ++buf) {
+          const uint32_t s = s0 + (uint32_t)buf;
+          if (s >= S) break;
+          const StepUniform u = step_uniform(P, mu, t0 + s);
+          rc.rel_s = rel_saddr + (uint32_t)buf * P.rel_stride + col;
+          rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * bin_bytes;
+          if (s0 != 0u) {
+            bar_sync_b<kBarFree0, NB>(buf, T);             // the clearing warp has drained this histogram (step s-NB)
+            if (bookkeeper) take_mail(s - (uint32_t)NB, buf);
+          }
+          if constexpr (N > 0) generate_class_rel_few<ATOM, N>(P, bref, mu, u, rc, gplan.cls[0], gplan.p0_inc, sink);
+          else                 generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+          bar_arrive_b<kBarFull0, NB>(buf, T);
+        }
       }
-      if (nmax == 1u)      generate_class_rel_few<ATOM, 1>(P, bref, mu, u, rc, gplan.cls[0], gplan.p0_inc, sink);
-      else if (nmax == 2u) generate_class_rel_few<ATOM, 2>(P, bref, mu, u, rc, gplan.cls[0], gplan.p0_inc, sink);
-      else if (nmax == 3u) generate_class_rel_few<ATOM, 3>(P, bref, mu, u, rc, gplan.cls[0], gplan.p0_inc, sink);
-      else if (nmax == 4u) generate_class_rel_few<ATOM, 4>(P, bref, mu, u, rc, gplan.cls[0], gplan.p0_inc, sink);
-      else                 generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, gtid == 0, sink);
-      bar_arrive_b<kBarFull0>(buf, T);
-    }
+    };
+    if (nmax == 1u)      gen_loop(std::integral_constant<int, 1>{});
+    else if (nmax == 2u) gen_loop(std::integral_constant<int, 2>{});
+    else if (nmax == 3u) gen_loop(std::integral_constant<int, 3>{});
+    else if (nmax == 4u) gen_loop(std::integral_constant<int, 4>{});
+    else                 gen_loop(std::integral_constant<int, 0>{});
   }
   __syncthreads();                                         // the last clearing is done
-  if (bookkeeper) {                                        // the mails of the last two steps
-    if (S >= 2) take_mail(S - 2);
-    if (S >= 1) take_mail(S - 1);
+  if (bookkeeper) {                                        // the mails of the last NB steps, then the record goes back
+    for (uint32_t s = S > (uint32_t)NB ? S - (uint32_t)NB : 0u; s < S; ++s) take_mail(s, (int)(s & (uint32_t)(NB - 1)));
+    if (lane < 16) s_rec[lane] = rec_reg;
+    if (ovf_reg) s_ovf = 1;
   }
 
   // ---- a7 (its first block barrier publishes the bookkeeper's record)

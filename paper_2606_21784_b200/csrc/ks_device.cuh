@@ -869,36 +869,86 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
   lbnd.lb = lb; lbnd.la = la;
 }
 
-// a3-a5 for a window of at most 32 ticks starting at `base` (any alignment): one tick per lane, no
-// inner loops -- the short path for small offset ranges (C1, C3: delta = 8), where the clearing
-// chain is what bounds the step.  Same definitions as clear_window.
-template <class IO>
-__device__ __forceinline__ void clear_window1(const IO& io, int L, int base, int lane,
-                                              int& vmax, int& pstar, LaneBounds& lbnd, int inc_b = 0, int inc_a = 0) {
+// One step of an inclusive warp scan with the shuffle's own range predicate: x += value of the
+// lane d below (scan_up) / d above (scan_down) when that lane exists -- SHFL + one predicated add
+// (the CUDA intrinsics hide the predicate and need a compare or a mask besides).
+__device__ __forceinline__ int scan_up_add(int x, int d) {
+  int r;
+  asm volatile("{\n\t.reg .pred p;\n\t.reg .s32 t;\n\tshfl.sync.up.b32 t|p, %1, %2, 0, 0xffffffff;\n\tmov.s32 %0, %1;\n\t@p add.s32 %0, %1, t;\n\t}"
+               : "=r"(r) : "r"(x), "r"(d));
+  return r;
+}
+__device__ __forceinline__ int scan_down_add(int x, int d) {
+  int r;
+  asm volatile("{\n\t.reg .pred p;\n\t.reg .s32 t;\n\tshfl.sync.down.b32 t|p, %1, %2, 31, 0xffffffff;\n\tmov.s32 %0, %1;\n\t@p add.s32 %0, %1, t;\n\t}"
+               : "=r"(r) : "r"(x), "r"(d));
+  return r;
+}
+
+// a3-a5 for a window of at most 32*R ticks starting at `base` (ANY alignment), as R rows of 32
+// ticks: lane i owns ticks base + i, base + 32 + i, ... -- one tick per lane and row, so there is
+// no per-lane inner loop, every shared-memory access is a conflict-free 32-bit row, and the 2R
+// scans (suffix of bids, prefix of asks, per row) are independent chains that the warp overlaps;
+// the rows are then chained through their totals.  R = 1 is the short path of C1 / C3 (delta = 8),
+// R = 2 covers C2 (delta = 16: 33 ticks).  Same definitions as clear_window.  INC: ib[r] / ia[r]
+// are added to the loaded depth of the lane's tick in row r before the clearing (the decoupled
+// kernel's incoming orders, fused into the scan).
+template <int R, class IO, bool INC = false>
+__device__ __forceinline__ void clear_rows(const IO& io, int L, int base, int lane,
+                                           int& vmax, int& pstar, LaneBounds& lbnd,
+                                           const int* ib = nullptr, const int* ia = nullptr) {
   const unsigned FULL = 0xffffffffu;
-  const int tick = base + lane;
-  const bool in = tick < L;
-  const int b0 = in ? io.ld1(0, tick) : 0, a0 = in ? io.ld1(1, tick) : 0;
-  int b = b0 + inc_b, a = a0 + inc_a;   // inc: incoming orders fused into the scan (decoupled kernel), else 0
-  int D = b, S = a;                     // inclusive suffix of bids / prefix of asks over lanes
+  int tick[R], b0[R], a0[R], b[R], a[R], D[R], S[R];
+  bool in[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    tick[r] = base + 32 * r + lane;
+    in[r] = tick[r] < L;
+    b0[r] = in[r] ? io.ld1(0, tick[r]) : 0;
+    a0[r] = in[r] ? io.ld1(1, tick[r]) : 0;
+  }
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    b[r] = b0[r] + (INC ? ib[r] : 0);
+    a[r] = a0[r] + (INC ? ia[r] : 0);
+    D[r] = b[r]; S[r] = a[r];
+  }
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
-    int vb = __shfl_down_sync(FULL, D, d);
-    int va = __shfl_up_sync(FULL, S, d);
-    if (lane + d < 32) D += vb;
-    if (lane >= d) S += va;
+#pragma unroll
+    for (int r = 0; r < R; ++r) { D[r] = scan_down_add(D[r], d); S[r] = scan_up_add(S[r], d); }
   }
-  const int V = min(D, S);
-  vmax = __reduce_max_sync(FULL, V);
-  pstar = __reduce_min_sync(FULL, (V == vmax && vmax > 0) ? tick : 0x7fffffff);
+  if (R > 1) {                          // chain the rows: asks of the lower rows, bids of the higher rows
+    int rowA[R], rowB[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { rowA[r] = __shfl_sync(FULL, S[r], 31); rowB[r] = __shfl_sync(FULL, D[r], 0); }
+    int carryA = 0, carryB = 0;
+#pragma unroll
+    for (int r = 1; r < R; ++r) { carryA += rowA[r - 1]; S[r] += carryA; }
+#pragma unroll
+    for (int r = R - 2; r >= 0; --r) { carryB += rowB[r + 1]; D[r] += carryB; }
+  }
+  int V[R], bestV = 0;
+#pragma unroll
+  for (int r = 0; r < R; ++r) { V[r] = min(D[r], S[r]); bestV = max(bestV, V[r]); }
+  vmax = __reduce_max_sync(FULL, bestV);
+  int cand = 0x7fffffff;
+#pragma unroll
+  for (int r = R - 1; r >= 0; --r) if (V[r] == vmax) cand = tick[r];      // descending: the lowest row wins
+  pstar = __reduce_min_sync(FULL, vmax > 0 ? cand : 0x7fffffff);
   if (vmax > 0) {
-    b = min(b, max(0, D - vmax));
-    a = min(a, max(0, S - vmax));
+#pragma unroll
+    for (int r = 0; r < R; ++r) { b[r] = min(b[r], max(0, D[r] - vmax)); a[r] = min(a[r], max(0, S[r] - vmax)); }
   }
-  if (in && b != b0) io.st1(0, tick, b);
-  if (in && a != a0) io.st1(1, tick, a);
-  lbnd.lb = b > 0 ? tick : -1;
-  lbnd.la = a > 0 ? tick : 0x7fffffff;
+  int lb = -1, la = 0x7fffffff;
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    if (in[r] && b[r] != b0[r]) io.st1(0, tick[r], b[r]);
+    if (in[r] && a[r] != a0[r]) io.st1(1, tick[r], a[r]);
+    if (b[r] > 0) lb = tick[r];                                            // ascending: the highest wins
+    if (a[R - 1 - r] > 0) la = tick[R - 1 - r];                            // descending: the lowest wins
+  }
+  lbnd.lb = lb; lbnd.la = la;
 }
 
 // General window of any width: chunks of 128 ticks, three passes (total bid depth; profiles and

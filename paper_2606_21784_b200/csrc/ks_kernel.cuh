@@ -77,6 +77,27 @@ __device__ __forceinline__ void update_record_lanes(long long* rec, int* ovf_fla
   }
 }
 
+// The same update with the lane's field held in a REGISTER (ks_decoupled_kernel's bookkeeping warp:
+// no shared-memory round trip per step); ovf is a per-lane sticky flag.
+__device__ __forceinline__ void update_record_reg(long long& rec, int& ovf, int lane, int last, int vmax, int pstar,
+                                                  int prev_value) {
+  const unsigned long long XC = 0x0000006551441111ull;
+  const unsigned long long YC = 0x0000006655344321ull;
+  const int f = lane & 15;
+  const int xc = (int)((XC >> (4 * f)) & 7ull), yc = (int)((YC >> (4 * f)) & 7ull);
+  const int tr = vmax > 0 ? 1 : 0;
+  const int new_last = tr ? pstar : last;
+  const int pt = tr ? pstar : 0;
+  const int r = new_last - last, r2 = r * r;
+  const long long old = rec;
+  const long long inc = (long long)rec_pick(xc, tr, vmax, pt, r, r2) * (long long)rec_pick(yc, tr, vmax, pt, r, r2);
+  const long long sum = (long long)((unsigned long long)old + (unsigned long long)inc);
+  const unsigned long long x = tr ? (((unsigned long long)(unsigned)vmax << 16) | (unsigned long long)(unsigned)pstar) : 0xFFFFull;
+  const long long hash = (long long)(((unsigned long long)old ^ x) * kHashPrime);
+  rec = f == F_HASH ? hash : (f == F_LAST ? (long long)new_last : (f == F_PREV ? (long long)prev_value : sum));
+  if (((old ^ sum) & (inc ^ sum)) < 0) ovf = 1;          // inc = 0 for the fields that are set, not added
+}
+
 // The per-thread generation plan of a launch (MODEL 2 = the paper's agent model has its own).
 template <int MODEL>
 __device__ __forceinline__ GenPlan<MODEL> make_gen_plan(const KernelParams& P, bool packed, int tid, int T) {
@@ -183,7 +204,8 @@ __device__ __forceinline__ void clear_active_window(const LocalBook& io, int L, 
                                                     int& vmax, int& pstar, LaneBounds& lbnd, int& base, int& wend) {
   const int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
   if (force_generic || width8 > 256) { base = lo & ~3; wend = min(L, hi + 1); clear_generic(io, L, base, hi, lane, vmax, pstar, lbnd); }
-  else if (hi - lo < 32)             { base = lo; wend = min(L, base + 32); clear_window1(io, L, base, lane, vmax, pstar, lbnd); }
+  else if (hi - lo < 32)             { base = lo; wend = min(L, base + 32); clear_rows<1>(io, L, base, lane, vmax, pstar, lbnd); }
+  else if (hi - lo < 64)             { base = lo; wend = min(L, base + 64); clear_rows<2>(io, L, base, lane, vmax, pstar, lbnd); }
   else if (width4 <= 128)            { base = lo & ~3; wend = min(L, base + 128); clear_window<4>(io, L, base, lane, vmax, pstar, lbnd); }
   else                               { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, lbnd); }
 }

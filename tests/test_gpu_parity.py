@@ -97,11 +97,11 @@ def test_block_sizes_atomic_modes_and_clear_paths_give_identical_bytes(ks, oracl
 
 def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
     """KS_OPT_PIPELINE: ks_decoupled_kernel -- generating warps fill a price-independent relative
-    order histogram (double-buffered, up to two steps ahead), one clearing warp per market merges
+    order histogram (a ring of 4, or 2, histograms: up to that many steps ahead), one clearing warp per market merges
     it at the step's price.  Forced on (2) and off (1) for several block sizes and ragged agent
     counts, plain bins and the 32-lane-column layout, literal and PACKED4 draws, prices pinned to the
-    grid edges (the clamp happens at the merge), split and launch-per-step runs, S = 1, 2, 3 (the
-    double buffer's corner cases), the trace: always the oracle's bytes."""
+    grid edges (the clamp happens at the merge), split and launch-per-step runs, S = 1 .. 5 (the
+    ring's corner cases), the trace: always the oracle's bytes."""
     import torch
     L, seed, S = 128, 2, 150
     p = zi_params(8, 10)
@@ -110,10 +110,18 @@ def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
                     (7, 1024, 160), (6, 1024, 128), (9, 1000, 96), (5, 3000, 224), (11, 4096, 1024), (3, 4096, 288)]:
         ids = np.arange(M)
         eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
-        for pipe, cols in ((2, 0), (2, 1), (1, 0)):
+        for pipe, cols, ring in ((2, 0, 0), (2, 0, 2), (2, 1, 0), (1, 0, 0)):
             b, r = _gpu(ks, M, L, A, p, seed, S, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, pipe),
-                                                        (ks.KS_OPT_REL_COLUMNS, cols)])
-            assert_rows_equal(b, r, ids, eb, er, "decoupled=%d cols=%d A=%d T=%d" % (pipe, cols, A, T))
+                                                        (ks.KS_OPT_REL_COLUMNS, cols), (ks.KS_OPT_RING_DEPTH, ring)])
+            assert_rows_equal(b, r, ids, eb, er, "decoupled=%d cols=%d ring=%d A=%d T=%d" % (pipe, cols, ring, A, T))
+    # the C2 shape's window (delta = 16: 33 ticks, the two-row fused scan), 7 markets of 160 threads
+    p2 = zi_params(16, 100)
+    for M, A, T in [(9, 1024, 160), (5, 777, 128), (3, 2000, 544)]:
+        eb, er = oracle_rows(oracle, p2, 256, A, 1, np.arange(M), 90)
+        for ring in (0, 2):
+            b, r = _gpu(ks, M, 256, A, p2, 1, 90, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, 2),
+                                                        (ks.KS_OPT_RING_DEPTH, ring)])
+            assert_rows_equal(b, r, np.arange(M), eb, er, "decoupled C2 shape ring=%d A=%d T=%d" % (ring, A, T))
     pk = packed4(zi_params(16, 100))
     for M, A, T in [(6, 1001, 128), (5, 3, 64), (7, 4096, 288)]:
         eb, er = oracle_rows(oracle, pk, 256, A, 9, np.arange(M), 70)
@@ -126,7 +134,7 @@ def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
     for init in (0, L - 1, 4):
         q = dict(p, init_price=init)
         eb, er, et = oracle.run_markets_traced(q, L, A, seed, ids, 60)
-        for kw in (dict(), dict(split=[1, 29, 30]), dict(split=[2, 3, 55]), dict(stepwise=True)):
+        for kw in (dict(), dict(split=[1, 29, 30]), dict(split=[2, 3, 55]), dict(split=[4, 5, 51]), dict(stepwise=True)):
             for cols in (0, 1):
                 b, r = _gpu(ks, M, L, A, q, seed, 60, opts=[(ks.KS_OPT_BLOCK_THREADS, T), (ks.KS_OPT_PIPELINE, 2),
                                                             (ks.KS_OPT_REL_COLUMNS, cols)], **kw)
