@@ -330,24 +330,42 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   }
   pl.T = T;
   // ks_decoupled_kernel: legal for the zero-intelligence rules (literal or PACKED4) with plain
-  // atomics when book + two relative histograms fit the CTA's shared memory; automatic when the
-  // grid leaves the GPU underfilled, i.e. the step latency is what counts (C1, C3).  Block size for
-  // it: one clearing warp + the smallest power-of-two-minus... generating threads holding <= 3 events.
+  // atomics when book + the ring of relative histograms fit the CTA's shared memory.  Automatic
+  //  (a) when the grid leaves the GPU underfilled, i.e. the step latency is what counts (C1, C3):
+  //      4k generating warps holding <= 3 events per thread + the clearing warp (T = 160/288/544),
+  //      ring of 4;
+  //  (b) when the SM holds only a few markets (C2: 6.9 per SM): there the persistent kernel's
+  //      markets cannot hide each other's clearing, and 7 resident CTAs of 4 generating warps + 1
+  //      clearing warp (T = 160) win.  Measured on B200, L = 256, delta = 16, A = 256..4096:
+  //      the decoupled kernel is faster up to M = 2048 (13.8 markets per SM: +4 % .. +37 %) and
+  //      slower at M = 4096 (-2 % .. -10 %), where the persistent kernel runs one warp per market.
   const bool zi = s->p.model == KS_MODEL_ZI || s->p.model == KS_MODEL_ZI_PACKED4;
   if (zi && !s->opt_atomic && s->opt_pipe != 1) {
     const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
+    const bool few_per_sm = (long long)s->M <= 16LL * s->num_sms;
     const uint32_t side = rel_side_for(s);
-    // ring depth: 4 histograms (the lane-columned ablation layout keeps the two-deep ring)
-    const int ring = s->opt_ring ? s->opt_ring : (s->opt_cols ? 2 : 4);
-    const bool fits = pl.smem + 2 * (size_t)ring * side + 2048 <= (size_t)s->dev_smem_optin && !(s->opt_cols && ring != 2);
-    if (fits && (s->opt_pipe == 2 || underfilled)) {
+    // ring depth: 4 histograms when the step latency counts, 2 when throughput does (half the code
+    // in the instruction cache: C2 3.30 vs 3.38 ms); the lane-columned ablation layout has 2
+    const int ring = s->opt_ring ? s->opt_ring : ((s->opt_cols || (long long)s->M > 2LL * s->num_sms) ? 2 : 4);
+    const size_t dsmem = pl.smem + 2 * (size_t)ring * side;
+    const bool fits = dsmem + 2048 <= (size_t)s->dev_smem_optin && !(s->opt_cols && ring != 2);
+    const bool seven_fit = 7 * ((long long)dsmem + kSmemCtaOverhead) <= kSmemPerSM;
+    if (fits && (s->opt_pipe == 2 || underfilled || (few_per_sm && seven_fit))) {
       int Td = pl.T;
       if (!s->opt_threads) {
-        // 4k generating warps (one, two, four per scheduler) + the clearing warp; <= 3 events per thread
-        Td = 160;
-        while (Td < 544 && (long long)(Td - 32) * 3 < s->A) Td = 2 * (Td - 32) + 32;
+        if (s->A < 128) {
+          Td = 32 + 32 * ((s->A + 31) / 32 > 0 ? (s->A + 31) / 32 : 1);     // a handful of agents: no idle generating warps
+        } else {
+          // 4k generating warps (one, two, four per scheduler) + the clearing warp; <= 3 events per
+          // thread when the step latency counts, one generating warp per scheduler otherwise
+          Td = 160;
+          if ((long long)s->M <= 2LL * s->num_sms) {
+            while (Td < 544 && (long long)(Td - 32) * 3 < s->A) Td = 2 * (Td - 32) + 32;
+            if (s->M > s->num_sms && Td > 288) Td = 288;
+          }
+        }
       }
-      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem += 2 * (size_t)ring * side; }
+      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem = dsmem; }
     }
   }
   return pl;
@@ -381,7 +399,8 @@ static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t 
 template <bool PACKED>
 static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, cudaStream_t st) {
   if (cols) return launch_decoupled_as<PACKED, 32, 2, 1024, 1>(P, T, smem, st);
-  if (ring == 2) return launch_decoupled_as<PACKED, 1, 2, 1024, 1>(P, T, smem, st);
+  if (ring == 2) return T <= 160 ? launch_decoupled_as<PACKED, 1, 2, 160, 7>(P, T, smem, st)
+                                 : launch_decoupled_as<PACKED, 1, 2, 1024, 1>(P, T, smem, st);
   if (T <= 160) return launch_decoupled_as<PACKED, 1, 4, 160, 7>(P, T, smem, st);
   return launch_decoupled_as<PACKED, 1, 4, 1024, 1>(P, T, smem, st);
 }
