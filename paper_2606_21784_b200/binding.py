@@ -74,10 +74,13 @@ def load():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
+    # KINETICSIM_LIB selects another build of the SAME CUDA library (the KS_DEBUG_CHECKS build); it is
+    # not a fallback: the path must exist
+    path = os.environ.get("KINETICSIM_LIB") or LIB_PATH
+    if not os.path.exists(path):
         raise RuntimeError("libkineticsim.so is not built (%s); run `python -m paper_2606_21784_b200.build` "
-                           "or __graft_entry__.build() -- there is no CPU fallback" % LIB_PATH)
-    L = C.CDLL(LIB_PATH, mode=C.RTLD_GLOBAL)
+                           "or __graft_entry__.build() -- there is no CPU fallback" % path)
+    L = C.CDLL(path, mode=C.RTLD_GLOBAL)
     vp, i32, i64, u64, u32, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_uint32, C.c_double
     pp = C.POINTER(KsAgentParams)
     L.ks_state_bytes.argtypes = [i32, i32]; L.ks_state_bytes.restype = C.c_size_t

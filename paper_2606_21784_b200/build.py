@@ -42,6 +42,34 @@ def _compile(out: str, sources, extra, verbose: bool) -> None:
     os.replace(tmp, out)
 
 
+DEBUG_LIB = os.path.join(HERE, "libkineticsim_dbg.so")
+
+
+DEBUG_INJECT_LIB = os.path.join(HERE, "libkineticsim_dbg_inject.so")
+
+
+def build_debug_checks(verbose: bool = False, inject_race: bool = False) -> str:
+    """The same library compiled with -DKS_DEBUG_CHECKS (ks_device.cuh): device-side bounds and
+    phase-structure checks that trap on failure.  Loaded instead of the product library by setting
+    KINETICSIM_LIB to its path (tests/test_gpu_parity.py::test_debug_checks_build).
+    inject_race: the negative control -- additionally drops barrier B1 of the persistent kernel
+    (-DKS_DEBUG_INJECT_RACE), which the checks must catch."""
+    out = DEBUG_INJECT_LIB if inject_race else DEBUG_LIB
+    tmp = out + ".tmp.%d" % os.getpid()
+    cmd = [_nvcc()] + NVCC_FLAGS + ["-DKS_DEBUG_CHECKS"] + (["-DKS_DEBUG_INJECT_RACE"] if inject_race else []) + \
+          (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
+    subprocess.check_call(cmd)
+    os.replace(tmp, out)
+    return out
+
+
+def debug_is_stale(path: str) -> bool:
+    if not os.path.exists(path):
+        return True
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    return any(os.path.getmtime(d) > os.path.getmtime(path) for d in deps)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
@@ -52,4 +80,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--debug-checks" in sys.argv:
+        print(build_debug_checks(verbose="-v" in sys.argv))
+        print(build_debug_checks(verbose="-v" in sys.argv, inject_race=True))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -85,6 +85,10 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   __shared__ int s_ovf;
   __shared__ long long s_keep[3];
   constexpr int ATOM = COLS == 1 ? 4 : 5;
+#ifdef KS_DEBUG_CHECKS
+  __shared__ int s_dbg_count[NB];                     // orders added to each ring slot since it was last drained
+  if (threadIdx.x < NB) s_dbg_count[threadIdx.x] = 0;
+#endif
   constexpr int kBarFull0 = 1, kBarFree0 = 1 + NB;
 
   const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
@@ -147,6 +151,10 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
         int vmax, pstar, base, wend;
         LaneBounds lbnd;
         bar_sync_b<kBarFull0, NB>(buf, T);                 // every order of step s is in the histogram
+#ifdef KS_DEBUG_CHECKS
+        if (lane == 0) { KS_CHECK(s_dbg_count[buf] == P.A, "orders in the histogram at full[] != agents"); s_dbg_count[buf] = 0; }
+        __syncwarp();
+#endif
         if (fuse && hi - lo < 32) {
           // this lane's bins of tick lo + lane (a2, second half): read and zeroed here, added to the
           // depth inside the scan
@@ -251,6 +259,10 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
           const StepUniform u = step_uniform(P, mu, t0 + s);
           rc.rel_s = rel_saddr + (uint32_t)buf * P.rel_stride + col;
           rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * bin_bytes;
+#ifdef KS_DEBUG_CHECKS
+          bref.dbg_lo = rel_saddr + (uint32_t)buf * P.rel_stride; bref.dbg_hi = bref.dbg_lo + P.rel_stride;
+          bref.dbg_count = &s_dbg_count[buf];
+#endif
           if (s0 != 0u) {
             bar_sync_b<kBarFree0, NB>(buf, T);             // the clearing warp has drained this histogram (step s-NB)
             if (bookkeeper) take_mail(s - (uint32_t)NB, buf);

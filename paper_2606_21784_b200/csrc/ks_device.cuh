@@ -15,6 +15,7 @@
 // previous clearing, so the window is ~2*dmax+1 ticks wide instead of L.
 #pragma once
 #include <cstdint>
+#include <cstdio>
 #include <cuda_runtime.h>
 
 #ifndef KS_GEN_UNROLL
@@ -241,10 +242,41 @@ struct BookRef {
   int32_t* ptr;        // generic pointer to the book
   uint32_t saddr;      // its 32-bit shared-window address
   int log2L, log2Lc;   // ATOM 3 only: L = 1 << log2L ticks, 1 << log2Lc of them per CTA
+#ifdef KS_DEBUG_CHECKS
+  uint32_t dbg_lo, dbg_hi;   // shared-window byte range an order may be added to (book, or relative histogram)
+  int* dbg_count;            // shared counter of the orders added in the current step
+#endif
 };
+
+// KS_DEBUG_CHECKS (python -m paper_2606_21784_b200.build --debug-checks -> libkineticsim_dbg.so):
+// the library's own bounds and phase checks, in place of compute-sanitizer (closed on this pool,
+// profiles/r2_sanitizer.md).  Every order's shared-memory address must lie inside the book (or the
+// relative histogram being filled); every book access of the clearing code inside [0, L); and --
+// the phase structure of Alg.1 -- when the clearing warp starts on a
+// step, EXACTLY the step's orders have been added since it last looked (a missed or early barrier
+// shows up as a wrong count).  A failed check prints its location and traps.
+#ifdef KS_DEBUG_CHECKS
+#define KS_CHECK(cond, what)                                                                                   \
+  do {                                                                                                         \
+    if (!(cond)) {                                                                                             \
+      printf("KS_DEBUG_CHECKS failed: %s (%s:%d) block %d thread %d\n", what, __FILE__, __LINE__, (int)blockIdx.x, \
+             (int)threadIdx.x);                                                                                \
+      __trap();                                                                                                \
+    }                                                                                                          \
+  } while (0)
+#else
+#define KS_CHECK(cond, what) do { } while (0)
+#endif
 
 template <int ATOM>
 __device__ __forceinline__ void book_add_at(const BookRef& book, uint32_t saddr, int q, int& sink) {
+#ifdef KS_DEBUG_CHECKS
+  if (ATOM != 2) {
+    KS_CHECK(saddr >= book.dbg_lo && saddr + 4u <= book.dbg_hi && (saddr & 3u) == 0u, "order address outside its target array");
+    KS_CHECK(q > 0, "order quantity not positive");
+    atomicAdd(book.dbg_count, 1);
+  }
+#endif
   if (ATOM == 0) {
     asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(saddr), "r"(q) : "memory");
   } else if (ATOM == 2) {
@@ -757,13 +789,22 @@ struct LocalBook {
   int32_t* book;
   int L;
   __device__ __forceinline__ int4 ld4(int side, int tick) const {
+    KS_CHECK(tick >= 0 && tick + 4 <= L && (tick & 3) == 0, "clearing: vector load outside the grid");
     return *reinterpret_cast<const int4*>((side ? book + L : book) + tick);
   }
   __device__ __forceinline__ void st4(int side, int tick, int4 v) const {
+    KS_CHECK(tick >= 0 && tick + 4 <= L && (tick & 3) == 0, "clearing: vector store outside the grid");
+    KS_CHECK(v.x >= 0 && v.y >= 0 && v.z >= 0 && v.w >= 0, "clearing: negative residual depth");
     *reinterpret_cast<int4*>((side ? book + L : book) + tick) = v;
   }
-  __device__ __forceinline__ int ld1(int side, int tick) const { return (side ? book + L : book)[tick]; }
-  __device__ __forceinline__ void st1(int side, int tick, int v) const { (side ? book + L : book)[tick] = v; }
+  __device__ __forceinline__ int ld1(int side, int tick) const {
+    KS_CHECK(tick >= 0 && tick < L, "clearing: load outside the grid");
+    return (side ? book + L : book)[tick];
+  }
+  __device__ __forceinline__ void st1(int side, int tick, int v) const {
+    KS_CHECK(tick >= 0 && tick < L && v >= 0, "clearing: store outside the grid or negative depth");
+    (side ? book + L : book)[tick] = v;
+  }
 };
 
 // ---------------------------------------------------------------------------------------------

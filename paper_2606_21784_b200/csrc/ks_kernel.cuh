@@ -248,6 +248,11 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   const MarketUniform mu = market_uniform(P, market);
   const GenPlan<MODEL> gplan = make_gen_plan<MODEL>(P, PACKED, tid, T);
   BookRef bref; bref.ptr = book; bref.saddr = (uint32_t)__cvta_generic_to_shared(book);
+#ifdef KS_DEBUG_CHECKS
+  __shared__ int s_dbg_count;
+  bref.dbg_lo = bref.saddr; bref.dbg_hi = bref.saddr + 8u * (uint32_t)L; bref.dbg_count = &s_dbg_count;
+  if (tid == 0) s_dbg_count = 0;
+#endif
 
   // ---- a0
   long long sb0, sa0;
@@ -281,6 +286,11 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   __syncthreads();
   // a3-a6: clearing by the clearing warp on the active window
   auto clear_step = [&](uint32_t s, int mid2_now) {
+#ifdef KS_DEBUG_CHECKS
+    // B1 held: exactly this step's orders are in the book, and none of the next step's yet
+    if (lane == 0) { KS_CHECK((long long)s_dbg_count == P.orders_per_step, "orders in the book at B1 != orders of the step"); s_dbg_count = 0; }
+    __syncwarp();
+#endif
     int lo, hi;
     if (MODEL == 2) {
       lo = max(0, min(amin, (mid2_now >> 1) - P.dmax));
@@ -314,6 +324,9 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
   // ---- S steps, all on-chip
   for (uint32_t s = 0; s < S; ++s) {
     const uint32_t t = t0 + s;
+#ifdef KS_DEBUG_INJECT_RACE                            // negative control: B1 dropped and the other warps made late
+    if (!clearing) __nanosleep(20000);
+#endif
     const StepUniform u = step_uniform(P, mu, t);
     const int4 ctl = *reinterpret_cast<const int4*>(s_ctl);
     last = ctl.x;
@@ -335,7 +348,9 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
       // a1 + a2: order generation and aggregation
       generate_step<MODEL, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
     }
+#ifndef KS_DEBUG_INJECT_RACE                           // (the negative control of the KS_DEBUG_CHECKS build drops B1)
     __syncthreads();                                   // B1: the combined book is complete
+#endif
     if (clearing) clear_step(s, rc.mid2);
     __syncthreads();                                   // B2: residual book and new price visible
     prev = last;

@@ -636,3 +636,31 @@ def test_run_to_run_determinism(ks):
     a = _gpu(ks, 256, c.L, c.A, c.params, c.seed, 50)
     b = _gpu(ks, 256, c.L, c.A, c.params, c.seed, 50)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_debug_checks_build(ks):
+    """compute-sanitizer is closed on this pool (profiles/r2_sanitizer.md); the library's own
+    KS_DEBUG_CHECKS build stands in for it: every order address inside its target array, every
+    clearing access inside the grid, no negative depth, and -- the phase structure of Alg.1
+     -- exactly the step's orders in the book / histogram when the
+    clearing warp starts.  All kernel families run under it (tests/sanitizer_cases.py, compared
+    with the oracle); the negative control (barrier B1 dropped) must trap."""
+    import os
+    import subprocess
+    import sys
+    from paper_2606_21784_b200 import build
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for inject in (False, True):
+        lib = build.DEBUG_INJECT_LIB if inject else build.DEBUG_LIB
+        if build.debug_is_stale(lib):
+            build.build_debug_checks(inject_race=inject)
+    env = dict(os.environ, KINETICSIM_LIB=build.DEBUG_LIB)
+    p = subprocess.run([sys.executable, os.path.join(root, "tests", "sanitizer_cases.py")], env=env, capture_output=True,
+                       text=True, timeout=900)
+    assert p.returncode == 0 and "all sanitizer cases ok" in p.stdout, p.stdout[-2000:] + p.stderr[-2000:]
+    assert "KS_DEBUG_CHECKS failed" not in p.stdout + p.stderr
+    env = dict(os.environ, KINETICSIM_LIB=build.DEBUG_INJECT_LIB)
+    p = subprocess.run([sys.executable, os.path.join(root, "tests", "sanitizer_cases.py"), "c5"], env=env, capture_output=True,
+                       text=True, timeout=900)
+    assert p.returncode != 0 and "KS_DEBUG_CHECKS failed: orders in the book at B1" in p.stdout + p.stderr, \
+        "the injected race was not caught: " + p.stdout[-1000:] + p.stderr[-1000:]
