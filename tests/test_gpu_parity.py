@@ -466,7 +466,7 @@ def _assert_stats_close(got, exp, what, K):
     assert np.all(err <= 1e-12 * scale[m]), "%s: worst err/tol %g" % (what, np.max(err / np.maximum(1e-12 * scale[m], 1e-300)))
 
 
-@pytest.mark.parametrize("case", ["zi", "mix3", "packed4", "cluster"])
+@pytest.mark.parametrize("case", ["zi", "mix3", "packed4", "cluster", "long"])
 def test_trace_and_return_statistics(ks, oracle, case):
     """the (price, Vmax) trace is bit-exact against the oracle's, tracing
     leaves the state bytes unchanged, traces of split runs concatenate, ragged step counts (not a
@@ -479,6 +479,8 @@ def test_trace_and_return_statistics(ks, oracle, case):
         M, L, A, seed, p, runs = 21, 1024, 900, 4, mix3_params(), [150]
     elif case == "packed4":
         M, L, A, seed, p, runs = 19, 512, 1001, 6, packed4(mix3_params()), [64, 37]
+    elif case == "long":             # S = 10^5, the bound include/kineticsim.h states for ks_trace_stats (decoupled kernel)
+        M, L, A, seed, p, runs = 3, 128, 64, 13, zi_params(8, 10), [100000]
     else:
         M, L, A, seed, p, runs = 9, 512, 600, 8, zi_params(32, 50), [70]
         opts = [(ks.KS_OPT_CLUSTER_SIZE, 4)]

@@ -1,4 +1,4 @@
-"""N > 1 host logic on CPU (world_size 2, gloo): contiguous market shards keyed by the GLOBAL
+"""N > 1 host logic (world_size 2, gloo) on CPU, and -- marked gpu -- the same split through the library: contiguous market shards keyed by the GLOBAL
 market id reproduce the single-process run, with no data-path collective (SURVEY.md S8(e),
 PAPER.md:105-107).  The per-shard compute stands in for one GPU's ks_create_ex(market_base) +
 ks_run; here it is the oracle, which is keyed the same way.  Only the gather of the results and
@@ -71,3 +71,47 @@ def test_shard_markets_partitions_the_range():
             for (b0, c0), (b1, _) in zip(parts, parts[1:]):
                 assert b1 == b0 + c0
             assert max(c for _, c in parts) - min(c for _, c in parts) <= 1
+
+
+# ---- the same split through the LIBRARY: each rank = ks_create_ex(market_base = shard start) + ks_run.
+# One GPU is enough: the ranks' kernels never wait on one another (there is no data-path collective),
+# so two processes sharing cuda:0 exercise exactly what two GPUs would run.
+def _gpu_worker(rank, world, port, case, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2606_21784_b200 import binding as ks
+        ks.load()
+        M, L, A, S, seed, params = case
+        base, count = shard_markets(M, rank, world)
+        sim = ks.KsSim(count, L, A, params, seed, market_base=base, device="cuda:0")
+        sim.ks_run(S)
+        books, recs = sim.books_to_host(), sim.stats_to_host()
+        sim.ks_destroy()
+        gathered = [None] * world
+        dist.all_gather_object(gathered, (base, count, books, recs))
+        if rank == 0:
+            gathered.sort(key=lambda g: g[0])
+            np.save(os.path.join(out_dir, "books.npy"), np.concatenate([g[2] for g in gathered]))
+            np.save(os.path.join(out_dir, "recs.npy"), np.concatenate([g[3] for g in gathered]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", [
+    (7, 64, 100, 30, 11, zi_params(8, 10)),            # shards of 4 and 3 markets
+    (301, 256, 1024, 40, 1, zi_params(16, 100)),       # the C2 shape cut 151 / 150: decoupled kernel on both ranks
+    (5, 512, 700, 25, 4, mix3_params()),
+])
+def test_two_rank_shards_through_the_library(oracle, tmp_path, case):
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from ks_testlib import oracle_rows
+    world = 2
+    mp.spawn(_gpu_worker, args=(world, _free_port(), case, str(tmp_path)), nprocs=world, join=True)
+    M, L, A, S, seed, params = case
+    eb, er = oracle_rows(oracle, params, L, A, seed, np.arange(M, dtype=np.uint32), S)
+    assert np.array_equal(np.load(tmp_path / "books.npy"), eb)
+    assert np.array_equal(np.load(tmp_path / "recs.npy"), er)
