@@ -616,7 +616,7 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
     # a8 ablation on C2: one launch per step, book through HBM every step
     c = CONFIGS["C2"]
     pers = allc.get("C2") or time_case(ks, torch, dev, c, reps=5)
-    sw = time_case(ks, torch, dev, c, reps=3, mode="stepwise")
+    sw = time_case(ks, torch, dev, c, reps=2, mode="stepwise")
     out["ablation_launch_per_step_C2"] = {
         "ms": sw["ms"], "events_per_s": sw["events_per_s"], "launches": c.S, "persistent_ms": pers["ms"],
         "slowdown_vs_persistent": sw["ms"] / pers["ms"],
