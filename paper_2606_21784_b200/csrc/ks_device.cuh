@@ -829,13 +829,28 @@ __device__ __forceinline__ void reduce_bounds(const LaneBounds& c, int base, int
   if (amin_new == 0x7fffffff) amin_new = wend;
 }
 
+// EXT (model 4's marketable orders): depth that rests OUTSIDE the window but counts
+// towards every profile value inside it -- ext.b = the marketable buys at tick L-1 (above the
+// window's top: part of D[p] for every p), ext.a = the marketable sells at tick 0 (below its base:
+// part of S[p] for every p) -- so that one marketable order does not widen the scan to the grid
+// edge.  The window's result is the full-grid result of Eq.1-2 iff
+//   ext.b <= S[top]                 (else the buys would reach asks resting above the window), and
+//   ext.a == 0, or ext.a <= D[base] and Vmax > ext.a   (else they would reach bids below it; and
+//                                    with Vmax == ext.a the lowest-tick tie-break picks a tick
+//                                    below the window -- tick 0 itself);
+// then both are filled completely (Vmax >= V[top] >= ext.b, Vmax > ext.a) and their ticks end empty.
+// The functions return false -- having written nothing -- when the condition fails; the caller
+// falls back to the scan that reaches the edge.
+struct ExtDepth { int b, a; };
+
 // INC: ib[j] / ia[j] are added to the loaded bid / ask depth of the lane's j-th tick before the
 // clearing (the decoupled kernel's incoming orders, fused into the scan instead of being merged
 // into the book first); the residual is then stored even when nothing traded.
-template <int K, class IO, bool INC = false>
-__device__ __forceinline__ void clear_window(const IO& io, int L, int base, int lane,
+template <int K, class IO, bool INC = false, bool EXT = false>
+__device__ __forceinline__ bool clear_window(const IO& io, int L, int base, int lane,
                                              int& vmax, int& pstar, LaneBounds& lbnd,
-                                             const int* ib = nullptr, const int* ia = nullptr) {
+                                             const int* ib = nullptr, const int* ia = nullptr,
+                                             ExtDepth ext = ExtDepth{0, 0}) {
   static_assert(K % 4 == 0, "K must be a multiple of 4 (16-byte shared-memory vectors)");
   const unsigned FULL = 0xffffffffu;
   const int tick0 = base + lane * K;
@@ -867,7 +882,7 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
     if (lane >= d) prea += va;
   }
   // profiles are recomputed in the residual pass instead of being kept: K fewer registers x 2
-  const int D0 = sufb, S0 = prea - ta;
+  const int D0 = sufb + (EXT ? ext.b : 0), S0 = prea - ta + (EXT ? ext.a : 0);
   int bestV = 0, bestp = 0x7fffffff;
   {
     int Drun = D0, Srun = S0;
@@ -881,6 +896,10 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
   }
   vmax = __reduce_max_sync(FULL, bestV);
   pstar = __reduce_min_sync(FULL, bestV == vmax ? bestp : 0x7fffffff);
+  if (EXT) {
+    const int Dbase = __shfl_sync(FULL, D0, 0), Stop = __shfl_sync(FULL, S0 + ta, 31);
+    if (ext.b > Stop || (ext.a != 0 && (ext.a > Dbase || vmax <= ext.a))) return false;
+  }
   int lb = -1, la = 0x7fffffff;
   if (vmax > 0 || INC) {
     if (vmax > 0) {
@@ -908,6 +927,7 @@ __device__ __forceinline__ void clear_window(const IO& io, int L, int base, int 
     if (a[K - 1 - j] > 0) la = tick0 + K - 1 - j;      // descending: the lowest wins
   }
   lbnd.lb = lb; lbnd.la = la;
+  return true;
 }
 
 // One step of an inclusive warp scan with the shuffle's own range predicate: x += value of the
@@ -934,10 +954,11 @@ __device__ __forceinline__ int scan_down_add(int x, int d) {
 // R = 2 covers C2 (delta = 16: 33 ticks).  Same definitions as clear_window.  INC: ib[r] / ia[r]
 // are added to the loaded depth of the lane's tick in row r before the clearing (the decoupled
 // kernel's incoming orders, fused into the scan).
-template <int R, class IO, bool INC = false>
-__device__ __forceinline__ void clear_rows(const IO& io, int L, int base, int lane,
+template <int R, class IO, bool INC = false, bool EXT = false>
+__device__ __forceinline__ bool clear_rows(const IO& io, int L, int base, int lane,
                                            int& vmax, int& pstar, LaneBounds& lbnd,
-                                           const int* ib = nullptr, const int* ia = nullptr) {
+                                           const int* ib = nullptr, const int* ia = nullptr,
+                                           ExtDepth ext = ExtDepth{0, 0}) {
   const unsigned FULL = 0xffffffffu;
   int tick[R], b0[R], a0[R], b[R], a[R], D[R], S[R];
   bool in[R];
@@ -969,6 +990,10 @@ __device__ __forceinline__ void clear_rows(const IO& io, int L, int base, int la
 #pragma unroll
     for (int r = R - 2; r >= 0; --r) { carryB += rowB[r + 1]; D[r] += carryB; }
   }
+  if (EXT) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) { D[r] += ext.b; S[r] += ext.a; }
+  }
   int V[R], bestV = 0;
 #pragma unroll
   for (int r = 0; r < R; ++r) { V[r] = min(D[r], S[r]); bestV = max(bestV, V[r]); }
@@ -977,6 +1002,10 @@ __device__ __forceinline__ void clear_rows(const IO& io, int L, int base, int la
 #pragma unroll
   for (int r = R - 1; r >= 0; --r) if (V[r] == vmax) cand = tick[r];      // descending: the lowest row wins
   pstar = __reduce_min_sync(FULL, vmax > 0 ? cand : 0x7fffffff);
+  if (EXT) {
+    const int Dbase = __shfl_sync(FULL, D[0], 0), Stop = __shfl_sync(FULL, S[R - 1], 31);
+    if (ext.b > Stop || (ext.a != 0 && (ext.a > Dbase || vmax <= ext.a))) return false;
+  }
   if (vmax > 0) {
 #pragma unroll
     for (int r = 0; r < R; ++r) { b[r] = min(b[r], max(0, D[r] - vmax)); a[r] = min(a[r], max(0, S[r] - vmax)); }
@@ -990,6 +1019,7 @@ __device__ __forceinline__ void clear_rows(const IO& io, int L, int base, int la
     if (a[R - 1 - r] > 0) la = tick[R - 1 - r];                            // descending: the lowest wins
   }
   lbnd.lb = lb; lbnd.la = la;
+  return true;
 }
 
 // General window of any width: chunks of 128 ticks, three passes (total bid depth; profiles and

@@ -210,6 +210,36 @@ __device__ __forceinline__ void clear_active_window(const LocalBook& io, int L, 
   else                               { base = lo & ~7; wend = min(L, base + 256); clear_window<8>(io, L, base, lane, vmax, pstar, lbnd); }
 }
 
+// Model 4: the same on the window the limit orders span, with the step's marketable depth at the
+// grid's edge ticks (bid[L-1], ask[0]) counted as ExtDepth when the chosen scan does not reach
+// them -- so that a marketable order does not turn the step into a full-grid scan.  Returns false,
+// having written nothing, when the exactness condition of ExtDepth fails or the window needs the
+// chunked scan; the caller then scans to the edge.  On success the edge ticks end empty.
+__device__ __forceinline__ bool clear_active_window_ext(const LocalBook& io, int L, int lo, int hi, bool mkt_buy, bool mkt_sell,
+                                                        int lane, int& vmax, int& pstar, LaneBounds& lbnd, int& base, int& wend) {
+  const int width4 = hi - (lo & ~3) + 1, width8 = hi - (lo & ~7) + 1;
+  int path;
+  if (width8 > 256)       return false;
+  else if (hi - lo < 32)  { path = 1; base = lo; wend = min(L, base + 32); }
+  else if (hi - lo < 64)  { path = 2; base = lo; wend = min(L, base + 64); }
+  else if (width4 <= 128) { path = 4; base = lo & ~3; wend = min(L, base + 128); }
+  else                    { path = 8; base = lo & ~7; wend = min(L, base + 256); }
+  ExtDepth ext;
+  ext.b = (mkt_buy && wend <= L - 1) ? io.ld1(0, L - 1) : 0;    // a scan that reaches the edge tick counts it itself
+  ext.a = (mkt_sell && base > 0) ? io.ld1(1, 0) : 0;
+  bool ok;
+  if (path == 1)      ok = clear_rows<1, LocalBook, false, true>(io, L, base, lane, vmax, pstar, lbnd, nullptr, nullptr, ext);
+  else if (path == 2) ok = clear_rows<2, LocalBook, false, true>(io, L, base, lane, vmax, pstar, lbnd, nullptr, nullptr, ext);
+  else if (path == 4) ok = clear_window<4, LocalBook, false, true>(io, L, base, lane, vmax, pstar, lbnd, nullptr, nullptr, ext);
+  else                ok = clear_window<8, LocalBook, false, true>(io, L, base, lane, vmax, pstar, lbnd, nullptr, nullptr, ext);
+  if (ok && lane == 0) {
+    if (ext.b != 0) io.st1(0, L - 1, 0);
+    if (ext.a != 0) io.st1(1, 0, 0);
+  }
+  __syncwarp();
+  return ok;
+}
+
 // ---------------------------------------------------------------------------------------------
 // The persistent kernel.  grid = M CTAs (one per market), block = T threads (any multiple of 32),
 // dynamic shared memory = 8*L bytes (the book).  MODEL: 0 = ZI, 1 = MIX3, 2 = the paper's agent
@@ -292,20 +322,26 @@ __global__ void __launch_bounds__(1024, 1) ks_persistent_kernel(const __grid_con
     __syncwarp();
 #endif
     int lo, hi;
+    int vmax, pstar, base, wend, nb, na;
+    LaneBounds lbnd;
+    const LocalBook io{book, L};
+    bool cleared = false;
     if (MODEL == 2) {
       lo = max(0, min(amin, (mid2_now >> 1) - P.dmax));
       hi = min(L - 1, max(bmax, ((mid2_now + 1) >> 1) + P.dmax));
-      if (s_mkt[0]) hi = L - 1;                      // marketable buys sit at tick L-1,
-      if (s_mkt[1]) lo = 0;                          // marketable sells at tick 0
+      const bool mkt_buy = s_mkt[0] != 0, mkt_sell = s_mkt[1] != 0;   // marketable buys sit at tick L-1, sells at tick 0
       __syncwarp();
+      if ((mkt_buy || mkt_sell) && !P.force_generic)
+        cleared = clear_active_window_ext(io, L, lo, hi, mkt_buy, mkt_sell, lane, vmax, pstar, lbnd, base, wend);
+      if (!cleared) {                                // the scan reaches the edge ticks itself
+        if (mkt_buy) hi = L - 1;
+        if (mkt_sell) lo = 0;
+      }
     } else {
       lo = max(0, min(amin, last - P.dmax));
       hi = min(L - 1, max(bmax, last + P.dmax));
     }
-    int vmax, pstar, base, wend, nb, na;
-    LaneBounds lbnd;
-    const LocalBook io{book, L};
-    clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
+    if (!cleared) clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
     reduce_bounds(lbnd, base, wend, nb, na);
     if (MODEL == 2) {
       // the mid price needs the EXACT best quotes: a side with no depth inside the window is
