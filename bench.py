@@ -56,8 +56,8 @@ EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 14.0 + 19.0) / 3.0,
 WIDE_MUL_LANES_PER_SM_PER_CLK = 4 * 8
 # dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 25261312 + 237688320,            # profiles/r1h_persistent_full.md
-                                  "C4_packed4": 23691008 + 254493952}    # profiles/r1g_packed_persistent_full.md
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 24508928 + 237626880,            # profiles/r2c_c4_full.md
+                                  "C4_packed4": 22112512 + 253766400}    # profiles/r2c_c4_packed4_full.md
 
 
 def model_key(params: dict) -> str:
