@@ -580,10 +580,12 @@ def main():
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum summed over the launches, from the ncu captures of
-# `bench.py --case C2 --M 128 --S {100,1000} --mode {persistent,stepwise}` (profiles/r2_traffic.md):
-# measured counters, not algorithmic bytes.  Filled in when the capture exists.
-PROFILED_TRAFFIC_C2_M128 = None
+# dram__bytes_read.sum + dram__bytes_write.sum and the L1 global load + store bytes, summed over the
+# launches of one run, from the ncu captures of `bench.py --case C2 --S 1000 [--mode stepwise]`
+# (profiles/r2c_traffic.md): measured counters, not algorithmic bytes.
+PROFILED_TRAFFIC_C2 = {"persistent": {"dram_bytes": 232704 + 0, "global_load_store_bytes": 131072 + 2228224},
+                       "launch_per_step": {"dram_bytes": 2312446208 + 0, "global_load_store_bytes": 2226e6 + 2228e6},
+                       "source": "profiles/r2c_traffic.md (ncu; the L2 is invalidated between launches under ncu)"}
 
 
 def extras(ks, torch, dev, peak_tmults, headline_cfg):
@@ -621,7 +623,7 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
         "ms": sw["ms"], "events_per_s": sw["events_per_s"], "launches": c.S, "persistent_ms": pers["ms"],
         "slowdown_vs_persistent": sw["ms"] / pers["ms"],
         "algorithmic_hbm_bytes": float(c.S) * c.M * 2 * (8 * c.L + 128), "persistent_algorithmic_hbm_bytes": float(c.M) * (8 * c.L + 128),
-        "measured_dram_bytes": PROFILED_TRAFFIC_C2_M128}
+        "measured_traffic": PROFILED_TRAFFIC_C2}
 
     # context runs in the paper's own shapes: Table IV's fixed workload and the
     # latency configuration with zero-intelligence agents -- NOT the paper's

@@ -241,12 +241,13 @@ typedef enum {
   KS_OPT_BLOCK_THREADS = 0, /* threads per CTA: 0 = automatic, else 32..1024, multiple of 32          */
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
   KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
-  KS_OPT_PIPELINE = 4,      /* the decoupled kernel (generating warps fill a price-independent relative order
-                               histogram up to KS_OPT_RING_DEPTH steps ahead; one clearing warp per market, holding no
-                               agents, merges it at the step's price and clears): 0 = automatic (when the
-                               grid underfills the GPU, i.e. step latency is what counts), 1 = never,
-                               2 = whenever legal (KS_MODEL_ZI / KS_MODEL_ZI_PACKED4, plain atomics,
-                               >= 64 threads, L <= 16384, book + the histogram ring fit shared memory)          */
+  KS_OPT_PIPELINE = 4,      /* the decoupled kernel (generating warps fill a ring of price-independent relative order
+                               histograms up to KS_OPT_RING_DEPTH steps ahead; one clearing warp per market, holding no
+                               agents, merges them at the step's price and clears): 0 = automatic (when the grid
+                               underfills the GPU, i.e. step latency is what counts, or when an SM holds only a few
+                               markets, M <= 16 x #SMs), 1 = never, 2 = whenever legal (KS_MODEL_ZI /
+                               KS_MODEL_ZI_PACKED4, plain atomics, >= 64 threads, L <= 16384, book + the histogram
+                               ring fit shared memory)                                                        */
   KS_OPT_REL_COLUMNS = 5,   /* decoupled kernel only: 0 = one int32 per histogram bin, 1 = 32 lane columns per
                                bin (column = lane = bank: a warp's atomics never conflict) -- the
                                aggregation ablation of north_star (3)                                       */
