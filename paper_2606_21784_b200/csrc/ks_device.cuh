@@ -2,9 +2,16 @@
 //
 // One CTA per market.  The int32 book (bid[L], ask[L]) lives in shared memory for all S steps
 // (Alg.1).  Per step: every thread generates orders for its agents with
-// Philox4x32-10 and adds them to the book with shared-memory atomics (a1, a2); warp 0 then clears
-// the ACTIVE WINDOW of the book with a register-blocked warp-shuffle scan (a3-a5) and updates the
-// price state and the int64 statistics (a6).  Two __syncthreads() per step.
+// Philox4x32-10 and adds them to the book with shared-memory atomics (a1, a2); one warp then
+// clears the ACTIVE WINDOW of the book with a warp-shuffle scan (a3-a5) and updates the price
+// state and the int64 statistics (a6).  Two __syncthreads() per step in ks_persistent_kernel
+// (ks_kernel.cuh); in ks_decoupled_kernel (ks_decoupled.cuh) generation runs ahead of the clearing
+// through a ring of price-independent histograms; ks_cluster_kernel (ks_cluster.cuh) splits a book
+// over the CTAs of a cluster.  This file holds what they share: Philox, the agent rules, the
+// aggregation and the clearing scans.
+//
+// tests/test_window_arguments.py checks the two exactness arguments used below (the window, and
+// ExtDepth) by brute force against the full-grid definition.
 //
 // Why a window is enough: let amin be the lowest tick with ask
 // depth and bmax the highest tick with bid depth in the combined book.  V[p] = min(D[p], S[p]) is
