@@ -123,7 +123,13 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   const uint32_t S = (uint32_t)P.S;
   if (tid == 0) { s_keep[0] = tot0.sum_bid; s_keep[1] = tot0.sum_ask; s_keep[2] = s_rec[F_SUMVOL]; }
   __syncthreads();
-  const bool bookkeeper = warp == 0;                       // the first generating warp keeps the record and the trace
+  // Who keeps the record (a6) and the trace.  Latency regime (C1, C3): the clearing warp's chain IS
+  // the step time, so the first generating warp does it from the mailbox.  Throughput regime (the
+  // (160, 7) two-deep-ring instantiation, C2): the SM is bound by dispatched instructions and the
+  // clearing warp has slack (it waits at full[] 40 % of its time), so it does the bookkeeping itself,
+  // straight from its registers: no mailbox round trip, and the four generating warps stay equal.
+  constexpr bool kClearingKeepsBooks = MAXT <= 160 && NB == 2;
+  const bool bookkeeper = kClearingKeepsBooks ? clearing : warp == 0;
   long long rec_reg = s_rec[lane & 15];                    // ... lane f (and f + 16) holding field f in a register
   int ovf_reg = 0;
   auto take_mail = [&](uint32_t s_of_mail, int slot) {     // a6 (+ trace) of one cleared step, in step order
@@ -225,9 +231,16 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
           __syncwarp();
           clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
         }
-        if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
+        if (!kClearingKeepsBooks) {
+          if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
+        }
         __syncwarp();
         if (s + NB < S) bar_arrive_b<kBarFree0, NB>(buf, T);   // histogram empty again, mail posted: step s+NB may start
+        if (kClearingKeepsBooks) {
+          update_record_reg(rec_reg, ovf_reg, lane, last, vmax, pstar, last);
+          if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)s, (long long)S, lane,
+                                  vmax > 0 ? pstar : last, vmax);
+        }
         int nb, na;
         reduce_bounds(lbnd, base, wend, nb, na);
         bmax = nb; amin = na;
@@ -265,7 +278,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
 #endif
           if (s0 != 0u) {
             bar_sync_b<kBarFree0, NB>(buf, T);             // the clearing warp has drained this histogram (step s-NB)
-            if (bookkeeper) take_mail(s - (uint32_t)NB, buf);
+            if (!kClearingKeepsBooks && bookkeeper) take_mail(s - (uint32_t)NB, buf);
           }
           if constexpr (N > 0) generate_class_rel_few<ATOM, N>(P, bref, mu, u, rc, gplan.cls[0], gplan.p0_inc, sink);
           else                 generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
@@ -281,7 +294,8 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   }
   __syncthreads();                                         // the last clearing is done
   if (bookkeeper) {                                        // the mails of the last NB steps, then the record goes back
-    for (uint32_t s = S > (uint32_t)NB ? S - (uint32_t)NB : 0u; s < S; ++s) take_mail(s, (int)(s & (uint32_t)(NB - 1)));
+    if (!kClearingKeepsBooks)
+      for (uint32_t s = S > (uint32_t)NB ? S - (uint32_t)NB : 0u; s < S; ++s) take_mail(s, (int)(s & (uint32_t)(NB - 1)));
     if (lane < 16) s_rec[lane] = rec_reg;
     if (ovf_reg) s_ovf = 1;
   }
