@@ -79,6 +79,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_all(force: bool = True) -> None:
+    """Product + bench libraries and the two KS_DEBUG_CHECKS builds, the three independent nvcc runs
+    side by side (each is one translation unit of ~75 s)."""
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(3) as ex:
+        jobs = [ex.submit(build, force), ex.submit(build_debug_checks), ex.submit(build_debug_checks, False, True)]
+        for j in jobs:
+            j.result()
+
+
 if __name__ == "__main__":
     if "--debug-checks" in sys.argv:
         print(build_debug_checks(verbose="-v" in sys.argv))
