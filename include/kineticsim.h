@@ -255,6 +255,10 @@ typedef enum {
                                clearing warp = number of relative histograms in the ring: 0 = automatic (4; 2 with
                                KS_OPT_REL_COLUMNS), 2 or 4 (ablation: the two-deep ring leaves both sides waiting
                                for each other's hand-over)                                                    */
+  KS_OPT_STEP_PAIRS = 7,    /* decoupled kernel, KS_MODEL_ZI, <= 160 threads: the generating warps make TWO steps per
+                               pass over their agents (the step-independent Philox rounds and the counter add are
+                               shared: 18 multiplies per event instead of 19) and hand them over together:
+                               0 = automatic, 1 = never, 2 = whenever legal                                     */
   KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
                                i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
                                book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libkineticsim.so")
 BENCH_LIB_PATH = os.path.join(_HERE, "libkineticsim_bench.so")
 
 KS_OK, KS_ERR_INVALID_ARG, KS_ERR_UNSUPPORTED, KS_ERR_OVERFLOW, KS_ERR_CUDA, KS_ERR_NOMEM = 0, -1, -2, -3, -4, -5
-KS_OPT_BLOCK_THREADS, KS_OPT_ATOMIC_MODE, KS_OPT_CLEAR_PATH, KS_OPT_CLUSTER_SIZE, KS_OPT_PIPELINE, KS_OPT_REL_COLUMNS, KS_OPT_RING_DEPTH = 0, 1, 2, 3, 4, 5, 6
+KS_OPT_BLOCK_THREADS, KS_OPT_ATOMIC_MODE, KS_OPT_CLEAR_PATH, KS_OPT_CLUSTER_SIZE, KS_OPT_PIPELINE, KS_OPT_REL_COLUMNS, KS_OPT_RING_DEPTH, KS_OPT_STEP_PAIRS = 0, 1, 2, 3, 4, 5, 6, 7
 
 PARAM_FIELDS = ("model", "noise_delta", "noise_qmax", "maker_spread_max", "maker_qty", "mom_delta",
                 "mom_qmax", "init_price", "paper_n_mom", "paper_n_maker", "paper_pmkt_q16")

@@ -46,7 +46,7 @@ struct ks_sim {
   int64_t steps_done;
   int64_t resting_bound;      // bound on the per-side depth total injected by ks_write_books / found by ks_attach
   int32_t fresh;              // books known all-zero (no run, no ks_write_books yet)
-  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe, opt_cols, opt_ring;
+  int32_t opt_threads, opt_atomic, opt_clear, opt_cluster, opt_pipe, opt_cols, opt_ring, opt_pair;
   int32_t n_noise, n_maker, n_mom;
   int64_t inflow_per_step;    // per-side bound on the quantity one step can add
   unsigned long long* h_words;   // pinned, mapped host memory: [0] depth bound of ks_write_books (copied),
@@ -154,7 +154,7 @@ ks_status create_common(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_
   if (!s) { set_err("%s: out of host memory", who); return KS_ERR_NOMEM; }
   s->M = M; s->L = L; s->A = A; s->p = *p; s->seed = seed; s->market_base = market_base;
   s->d_state = d_state; s->steps_done = 0; s->resting_bound = 0; s->fresh = attach ? 0 : 1;
-  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0; s->opt_cols = 0; s->opt_ring = 0;
+  s->opt_threads = 0; s->opt_atomic = 0; s->opt_clear = 0; s->opt_cluster = 0; s->opt_pipe = 0; s->opt_cols = 0; s->opt_ring = 0; s->opt_pair = 0;
   s->dev_smem_optin = optin; s->num_sms = sms; s->device = dev;
   s->bound_pending = 0; s->h_words = nullptr; s->d_flags = nullptr; s->bound_event = nullptr;
   if (p->model == KS_MODEL_PAPER) {
@@ -274,6 +274,9 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
     case KS_OPT_REL_COLUMNS:
       if (value != 0 && value != 1) break;
       s->opt_cols = value; return KS_OK;
+    case KS_OPT_STEP_PAIRS:
+      if (value != 0 && value != 1 && value != 2) break;
+      s->opt_pair = value; return KS_OK;
     case KS_OPT_RING_DEPTH:
       if (value != 0 && value != 2 && value != 4) break;
       s->opt_ring = value; return KS_OK;
@@ -299,7 +302,7 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 // T = 32 beats 64/128 on C4).  A book so large that 32-thread CTAs would leave the SM short of
 // warps -> widen until ~1024 threads are resident; few markets -> widen so the whole GPU is used,
 // but never beyond the agents.
-struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; };
+struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; bool pair; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
 
@@ -313,7 +316,7 @@ static uint32_t rel_side_for(const ks_sim* s) {
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
   pl.smem = (size_t)8 * (size_t)s->L;
-  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0;
+  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0; pl.pair = false;
   int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
   if (k < 1) k = 1;
   if (k > 32) k = 32;
@@ -365,7 +368,15 @@ static LaunchPlan plan_launch(const ks_sim* s) {
           }
         }
       }
-      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem = dsmem; }
+      if (Td >= 64) {
+        pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem = dsmem;
+        // two steps per hand-over (literal contract, plain bins, the (160, 7) instantiation): ring of 4
+        const bool can_pair = s->p.model == KS_MODEL_ZI && !s->opt_cols && Td <= 160 && (s->opt_ring == 0 || s->opt_ring == 4) &&
+                              pl.smem - 2 * (size_t)ring * side + 8 * (size_t)side + 2048 <= (size_t)s->dev_smem_optin;
+        if (can_pair && s->opt_pair == 2) {
+          pl.pair = true; pl.smem += 2 * (size_t)(4 - ring) * side; pl.ring = 4;
+        }
+      }
     }
   }
   return pl;
@@ -382,9 +393,9 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
   return cudaGetLastError();
 }
 
-template <bool PACKED, int COLS, int NB, int MAXT, int MINB>
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB, bool PAIR = false>
 static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB>;
+  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB, PAIR>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -397,8 +408,11 @@ static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t 
 // of 7 resident CTAs of <= 160 threads when the block is that small (C2: 6.9 markets per SM must all
 // be resident) -- or the two-deep ring (ablation; the only one with lane-columned bins).
 template <bool PACKED>
-static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, cudaStream_t st) {
+static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, bool pair, cudaStream_t st) {
   if (cols) return launch_decoupled_as<PACKED, 32, 2, 1024, 1>(P, T, smem, st);
+  if constexpr (!PACKED) {
+    if (pair && ring == 4 && T <= 160) return launch_decoupled_as<false, 1, 4, 160, 7, true>(P, T, smem, st);
+  }
   if (ring == 2) return T <= 160 ? launch_decoupled_as<PACKED, 1, 2, 160, 7>(P, T, smem, st)
                                  : launch_decoupled_as<PACKED, 1, 2, 1024, 1>(P, T, smem, st);
   if (T <= 160) return launch_decoupled_as<PACKED, 1, 4, 160, 7>(P, T, smem, st);
@@ -507,8 +521,8 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     const LaunchPlan pl = plan_launch(s);
     P.rel_side = pl.rel_side; P.rel_stride = 2 * pl.rel_side;
     if (pl.decoupled) {
-      e = packed ? launch_decoupled<true>(P, pl.T, pl.smem, s->opt_cols, pl.ring, st)
-                 : launch_decoupled<false>(P, pl.T, pl.smem, s->opt_cols, pl.ring, st);
+      e = packed ? launch_decoupled<true>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.pair, st)
+                 : launch_decoupled<false>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.pair, st);
     } else if (paper)
       e = launch_persistent<2, 0, false>(P, pl.T, pl.smem, st);
     else if (packed)

@@ -73,8 +73,9 @@ __device__ __forceinline__ void red32(uint32_t saddr, int v) { asm volatile("red
 // posts (Vmax, p*, price before) in an NB-slot mailbox.  The record (a6) and the trace are kept by
 // the FIRST GENERATING warp, which picks the mail of step s-NB up when it passes the free[]
 // barrier it waits at anyway; the last NB mails are taken after the loop.
-template <bool PACKED, int COLS, int NB, int MAXT, int MINB>
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB, bool PAIR = false>
 __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_constant__ KernelParams P) {
+  static_assert(!PAIR || (NB == 4 && COLS == 1 && !PACKED), "PAIR: two steps per hand-over, ring of 4, literal contract");
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then rel[NB][P.rel_stride / 4]
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
@@ -128,7 +129,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   // (160, 7) two-deep-ring instantiation, C2): the SM is bound by dispatched instructions and the
   // clearing warp has slack (it waits at full[] 40 % of its time), so it does the bookkeeping itself,
   // straight from its registers: no mailbox round trip, and the four generating warps stay equal.
-  constexpr bool kClearingKeepsBooks = MAXT <= 160 && NB == 2;
+  constexpr bool kClearingKeepsBooks = (MAXT <= 160 && NB == 2) || PAIR;
   const bool bookkeeper = kClearingKeepsBooks ? clearing : warp == 0;
   long long rec_reg = s_rec[lane & 15];                    // ... lane f (and f + 16) holding field f in a register
   int ovf_reg = 0;
@@ -142,109 +143,143 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   if (clearing) {
     const LocalBook io{book, L};
     const unsigned FULL = 0xffffffffu;
+    int vmax, pstar, base, wend;
+    LaneBounds lbnd;
+    // a2 (second half) + a3-a5 of one step on the histogram whose sell bins start at rs (ring slot
+    // `slot`); wait() is called where the histogram is first needed
+    auto clear_core = [&](uint32_t rs, int slot, auto wait) {
+      (void)slot;
+      const uint32_t rb = rs + P.rel_side;                           // buy bins
+      const int t_lo = last - delta;                     // tick of bin 0
+      const int lo = max(0, min(amin, t_lo));
+      const int hi = min(L - 1, max(bmax, last + delta));
+      const bool inside = t_lo >= 0 && last + delta <= L - 1;   // no order of this step is clamped
+      const bool fuse = COLS == 1 && inside && !P.force_generic;
+      wait();                                            // every order of this step is in the histogram
+#ifdef KS_DEBUG_CHECKS
+      if (lane == 0) { KS_CHECK(s_dbg_count[slot] == P.A, "orders in the histogram at full[] != agents"); s_dbg_count[slot] = 0; }
+      __syncwarp();
+#endif
+      if (fuse && hi - lo < 32) {
+        // this lane's bins of tick lo + lane (a2, second half): read and zeroed here, added to the
+        // depth inside the scan
+        int ib[1], ia[1];
+        base = lo; wend = min(L, lo + 32);
+        const int i = lo + lane - t_lo;
+        const bool has = (unsigned)i < (unsigned)n;
+        ia[0] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[0] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
+        if (ia[0] != 0) sts32(rs + 4u * (uint32_t)i, 0);
+        if (ib[0] != 0) sts32(rb + 4u * (uint32_t)i, 0);
+        clear_rows<1, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
+      } else if (fuse && hi - lo < 64) {
+        int ib[2], ia[2];
+        base = lo; wend = min(L, lo + 64);
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+          const int i = lo + 32 * r + lane - t_lo;
+          const bool has = (unsigned)i < (unsigned)n;
+          ia[r] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[r] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
+          if (ia[r] != 0) sts32(rs + 4u * (uint32_t)i, 0);
+          if (ib[r] != 0) sts32(rb + 4u * (uint32_t)i, 0);
+        }
+        clear_rows<2, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
+      } else if (fuse && hi - (lo & ~3) + 1 <= 128) {
+        base = lo & ~3; wend = min(L, base + 128);
+        int ib[4], ia[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int i = base + 4 * lane + j - t_lo;
+          const bool has = (unsigned)i < (unsigned)n;
+          ia[j] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[j] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
+          if (ia[j] != 0) sts32(rs + 4u * (uint32_t)i, 0);
+          if (ib[j] != 0) sts32(rb + 4u * (uint32_t)i, 0);
+        }
+        clear_window<4, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
+      } else {
+        // ---- general merge: bins -> clamped ticks, into the combined book; then the usual clearing
+        if (COLS == 1) {
+          for (int i = lane; i < n; i += 32) {
+            const int va = lds32(rs + 4u * (uint32_t)i), vb = lds32(rb + 4u * (uint32_t)i);
+            const int tick = clamp_tick(t_lo + i, L);
+            if (va != 0) { sts32(rs + 4u * (uint32_t)i, 0); red32(book_saddr + 4u * (uint32_t)(tick + L), va); }
+            if (vb != 0) { sts32(rb + 4u * (uint32_t)i, 0); red32(book_saddr + 4u * (uint32_t)tick, vb); }
+          }
+        } else {
+          // lane-columned bins: 8 bins at a time (independent loads), one REDUX per bin and side
+          for (int i0 = 0; i0 < n; i0 += 8) {
+            int va[8], vb[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const bool has = i0 + j < n;
+              va[j] = has ? lds32(rs + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane) : 0;
+              vb[j] = has ? lds32(rb + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane) : 0;
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              if (i0 + j < n) {
+                if (va[j] != 0) sts32(rs + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane, 0);
+                if (vb[j] != 0) sts32(rb + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane, 0);
+                const int ta = __reduce_add_sync(FULL, va[j]), tb = __reduce_add_sync(FULL, vb[j]);
+                const int tick = clamp_tick(t_lo + i0 + j, L);
+                if (lane == 0 && ta != 0) red32(book_saddr + 4u * (uint32_t)(tick + L), ta);
+                if (lane == 1 && tb != 0) red32(book_saddr + 4u * (uint32_t)tick, tb);
+              }
+            }
+          }
+        }
+        __syncwarp();
+        clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
+      }
+    };
+    if (!PAIR) {
     for (uint32_t s0 = 0; s0 < S; s0 += NB) {
 #pragma unroll
-      for (int buf = 0; buf < NB; ++buf) {                 // ring slot = step mod NB, a compile-time constant here
-        const uint32_t s = s0 + (uint32_t)buf;
-        if (s >= S) break;
-        const uint32_t rs = rel_saddr + (uint32_t)buf * P.rel_stride;   // sell bins of this step's histogram
-        const uint32_t rb = rs + P.rel_side;                           // buy bins
-        const int t_lo = last - delta;                     // tick of bin 0
-        const int lo = max(0, min(amin, t_lo));
-        const int hi = min(L - 1, max(bmax, last + delta));
-        const bool inside = t_lo >= 0 && last + delta <= L - 1;   // no order of this step is clamped
-        const bool fuse = COLS == 1 && inside && !P.force_generic;
-        int vmax, pstar, base, wend;
-        LaneBounds lbnd;
-        bar_sync_b<kBarFull0, NB>(buf, T);                 // every order of step s is in the histogram
-#ifdef KS_DEBUG_CHECKS
-        if (lane == 0) { KS_CHECK(s_dbg_count[buf] == P.A, "orders in the histogram at full[] != agents"); s_dbg_count[buf] = 0; }
-        __syncwarp();
-#endif
-        if (fuse && hi - lo < 32) {
-          // this lane's bins of tick lo + lane (a2, second half): read and zeroed here, added to the
-          // depth inside the scan
-          int ib[1], ia[1];
-          base = lo; wend = min(L, lo + 32);
-          const int i = lo + lane - t_lo;
-          const bool has = (unsigned)i < (unsigned)n;
-          ia[0] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[0] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
-          if (ia[0] != 0) sts32(rs + 4u * (uint32_t)i, 0);
-          if (ib[0] != 0) sts32(rb + 4u * (uint32_t)i, 0);
-          clear_rows<1, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
-        } else if (fuse && hi - lo < 64) {
-          int ib[2], ia[2];
-          base = lo; wend = min(L, lo + 64);
-#pragma unroll
-          for (int r = 0; r < 2; ++r) {
-            const int i = lo + 32 * r + lane - t_lo;
-            const bool has = (unsigned)i < (unsigned)n;
-            ia[r] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[r] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
-            if (ia[r] != 0) sts32(rs + 4u * (uint32_t)i, 0);
-            if (ib[r] != 0) sts32(rb + 4u * (uint32_t)i, 0);
-          }
-          clear_rows<2, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
-        } else if (fuse && hi - (lo & ~3) + 1 <= 128) {
-          base = lo & ~3; wend = min(L, base + 128);
-          int ib[4], ia[4];
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int i = base + 4 * lane + j - t_lo;
-            const bool has = (unsigned)i < (unsigned)n;
-            ia[j] = has ? lds32(rs + 4u * (uint32_t)i) : 0; ib[j] = has ? lds32(rb + 4u * (uint32_t)i) : 0;
-            if (ia[j] != 0) sts32(rs + 4u * (uint32_t)i, 0);
-            if (ib[j] != 0) sts32(rb + 4u * (uint32_t)i, 0);
-          }
-          clear_window<4, LocalBook, true>(io, L, base, lane, vmax, pstar, lbnd, ib, ia);
-        } else {
-          // ---- general merge: bins -> clamped ticks, into the combined book; then the usual clearing
-          if (COLS == 1) {
-            for (int i = lane; i < n; i += 32) {
-              const int va = lds32(rs + 4u * (uint32_t)i), vb = lds32(rb + 4u * (uint32_t)i);
-              const int tick = clamp_tick(t_lo + i, L);
-              if (va != 0) { sts32(rs + 4u * (uint32_t)i, 0); red32(book_saddr + 4u * (uint32_t)(tick + L), va); }
-              if (vb != 0) { sts32(rb + 4u * (uint32_t)i, 0); red32(book_saddr + 4u * (uint32_t)tick, vb); }
-            }
-          } else {
-            // lane-columned bins: 8 bins at a time (independent loads), one REDUX per bin and side
-            for (int i0 = 0; i0 < n; i0 += 8) {
-              int va[8], vb[8];
-#pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                const bool has = i0 + j < n;
-                va[j] = has ? lds32(rs + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane) : 0;
-                vb[j] = has ? lds32(rb + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane) : 0;
-              }
-#pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                if (i0 + j < n) {
-                  if (va[j] != 0) sts32(rs + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane, 0);
-                  if (vb[j] != 0) sts32(rb + 128u * (uint32_t)(i0 + j) + 4u * (uint32_t)lane, 0);
-                  const int ta = __reduce_add_sync(FULL, va[j]), tb = __reduce_add_sync(FULL, vb[j]);
-                  const int tick = clamp_tick(t_lo + i0 + j, L);
-                  if (lane == 0 && ta != 0) red32(book_saddr + 4u * (uint32_t)(tick + L), ta);
-                  if (lane == 1 && tb != 0) red32(book_saddr + 4u * (uint32_t)tick, tb);
-                }
-              }
-            }
+        for (int buf = 0; buf < NB; ++buf) {                 // ring slot = step mod NB, a compile-time constant here
+          const uint32_t s = s0 + (uint32_t)buf;
+          if (s >= S) break;
+          clear_core(rel_saddr + (uint32_t)buf * P.rel_stride, buf, [&] { bar_sync_b<kBarFull0, NB>(buf, T); });
+          if (!kClearingKeepsBooks) {
+            if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
           }
           __syncwarp();
-          clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
+          if (s + NB < S) bar_arrive_b<kBarFree0, NB>(buf, T);   // histogram empty again, mail posted: step s+NB may start
+          if (kClearingKeepsBooks) {
+            update_record_reg(rec_reg, ovf_reg, lane, last, vmax, pstar, last);
+            if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)s, (long long)S, lane,
+                                    vmax > 0 ? pstar : last, vmax);
+          }
+          int nb, na;
+          reduce_bounds(lbnd, base, wend, nb, na);
+          bmax = nb; amin = na;
+          last = vmax > 0 ? pstar : last;
         }
-        if (!kClearingKeepsBooks) {
-          if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
+      }
+    }
+    if (PAIR) {
+      // two steps per hand-over: ring slots 2p, 2p+1 belong to pair p = (s / 2) mod 2; one full[p] /
+      // free[p] barrier per pair (ids: full 1 + p, free 3 + p); the two steps are cleared by a rolled loop
+      for (uint32_t s0 = 0; s0 < S; s0 += 4) {
+#pragma unroll
+        for (int pr = 0; pr < 2; ++pr) {
+          const uint32_t s = s0 + 2u * (uint32_t)pr;
+          if (s >= S) break;
+          const uint32_t ns = min(2u, S - s);
+          for (uint32_t g = 0; g < ns; ++g) {
+            const int slot = 2 * pr + (int)g;
+            clear_core(rel_saddr + (uint32_t)slot * P.rel_stride, slot, [&] { if (g == 0) bar_sync_b<1, 2>(pr, T); });
+            if (g + 1 == ns) {
+              __syncwarp();
+              if (s + 4 < S) bar_arrive_b<3, 2>(pr, T);    // both histograms empty again: steps s+4, s+5 may start
+            }
+            update_record_reg(rec_reg, ovf_reg, lane, last, vmax, pstar, last);
+            if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)(s + g), (long long)S, lane,
+                                    vmax > 0 ? pstar : last, vmax);
+            int nb, na;
+            reduce_bounds(lbnd, base, wend, nb, na);
+            bmax = nb; amin = na;
+            last = vmax > 0 ? pstar : last;
+          }
         }
-        __syncwarp();
-        if (s + NB < S) bar_arrive_b<kBarFree0, NB>(buf, T);   // histogram empty again, mail posted: step s+NB may start
-        if (kClearingKeepsBooks) {
-          update_record_reg(rec_reg, ovf_reg, lane, last, vmax, pstar, last);
-          if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)s, (long long)S, lane,
-                                  vmax > 0 ? pstar : last, vmax);
-        }
-        int nb, na;
-        reduce_bounds(lbnd, base, wend, nb, na);
-        bmax = nb; amin = na;
-        last = vmax > 0 ? pstar : last;
       }
     }
   } else {
@@ -260,6 +295,33 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
     const uint32_t col = COLS == 32 ? 4u * (uint32_t)lane : 0u;
     const uint32_t bin_bytes = COLS == 32 ? 128u : 4u;
     int sink = 0;
+    if (PAIR) {
+      // two steps per pass over the agents: for one agent the Philox rounds that do not depend on the
+      // step (M0*a, M1*n2, M0*c0: two multiplies and two xors of round 0-2) and the counter add are
+      // shared by the two steps, and the per-step prologue of the loop is paid once per pair
+      RuleCtx rc1 = rc;
+      BookRef bref1 = bref;
+      for (uint32_t s0 = 0; s0 < S; s0 += 4) {
+#pragma unroll
+        for (int pr = 0; pr < 2; ++pr) {
+          const uint32_t s = s0 + 2u * (uint32_t)pr;
+          if (s >= S) break;
+          const bool two = s + 1 < S;
+          const StepUniform u0 = step_uniform(P, mu, t0 + s), u1 = step_uniform(P, mu, t0 + s + 1);
+          rc.rel_s = rel_saddr + (uint32_t)(2 * pr) * P.rel_stride;
+          rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * 4u;
+          rc1.rel_s = rc.rel_s + P.rel_stride; rc1.rel_b = rc.rel_b + P.rel_stride;
+#ifdef KS_DEBUG_CHECKS
+          bref.dbg_lo = rc.rel_s; bref.dbg_hi = bref.dbg_lo + P.rel_stride; bref.dbg_count = &s_dbg_count[2 * pr];
+          bref1.dbg_lo = rc1.rel_s; bref1.dbg_hi = bref1.dbg_lo + P.rel_stride; bref1.dbg_count = &s_dbg_count[2 * pr + 1];
+#endif
+          if (s0 != 0u) bar_sync_b<3, 2>(pr, T);           // free[pr]: the clearing warp has drained both histograms
+          if (two) generate_class_rel_pair<ATOM>(P, bref, bref1, mu, u0, u1, rc, rc1, gplan.cls[0], gplan.p0_inc, sink);
+          else     generate_step<0, ATOM, PACKED>(P, bref, mu, u0, rc, gplan, tid == 0, sink);
+          bar_arrive_b<1, 2>(pr, T);                       // full[pr]
+        }
+      }
+    }
     // the whole step loop, instantiated per N = events a thread holds (0 = the general loop), so that
     // nothing about N is decided inside it
     auto gen_loop = [&](auto Ntag) {
@@ -286,7 +348,8 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
         }
       }
     };
-    if (nmax == 1u)      gen_loop(std::integral_constant<int, 1>{});
+    if (PAIR)            { }
+    else if (nmax == 1u) gen_loop(std::integral_constant<int, 1>{});
     else if (nmax == 2u) gen_loop(std::integral_constant<int, 2>{});
     else if (nmax == 3u) gen_loop(std::integral_constant<int, 3>{});
     else if (nmax == 4u) gen_loop(std::integral_constant<int, 4>{});

@@ -588,6 +588,29 @@ __device__ __forceinline__ void generate_class_rel_few(const KernelParams& P, co
     if (e < n_mine) book_add_at<0>(book, addr[e], q[e], sink);
 }
 
+// Two steps of the noise class in one pass over a thread's agents (ks_decoupled_kernel, PAIR): the
+// same agent's orders of steps t (-> rc0's histogram) and t+1 (-> rc1's).  Written as two plain
+// Philox evaluations on the same p0: everything that does not depend on the step -- n2, M1*n2, c0,
+// c1, M0*c0 -- is common to both and is computed once (18 multiplies per event instead of 19, two
+// xors and the 64-bit counter add shared).  Two agents per unrolled trip = four chains.
+template <int ATOM>
+__device__ __forceinline__ void generate_class_rel_pair(const KernelParams& P, const BookRef& book0, const BookRef& book1,
+                                                        const MarketUniform& mu, const StepUniform& u0, const StepUniform& u1,
+                                                        const RuleCtx& rc0, const RuleCtx& rc1, const ClassPlan& pl,
+                                                        const P0Step& p0_inc, int& sink) {
+  auto one = [&](uint64_t p0) {
+    uint32_t a0, a1, a2, b0, b1, b2;
+    philox_from_p0<true>(P, mu, u0, p0, a0, a1, a2);
+    philox_from_p0<true>(P, mu, u1, p0, b0, b1, b2);
+    noise_order<ATOM, false>(P, book0, rc0, a0, a1, a2, sink);
+    noise_order<ATOM, false>(P, book1, rc1, b0, b1, b2, sink);
+  };
+  uint64_t p0 = pl.p0;
+#pragma unroll 2
+  for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, p0_inc.inc, p0_inc.a_step); }
+  if (pl.extra) one(p0);
+}
+
 // PACKED4: one class of BLOCKS of four agents.  MIX = false: all noise.  MIX = true: the blocks of
 // class CLS are b = 3i + CLS, so agent 4b + j has type (4b + j) mod 3 = (CLS + j) mod 3 -- uniform
 // over the warp for every j.

@@ -157,6 +157,42 @@ def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
         assert_rows_equal(b, r, np.arange(M), eb, er, "decoupled injected cols=%d" % cols)
 
 
+def test_step_pairs_give_identical_bytes(ks, oracle):
+    """KS_OPT_STEP_PAIRS: the decoupled kernel's generating warps make two steps per pass over
+    their agents (shared step-independent Philox rounds) and hand them over together; the clearing
+    warp keeps the record.  Odd and tiny step counts (the last pair holds one step), split and
+    launch-per-step runs (a pair never spans two ks_run calls), ragged agent counts, grid-edge
+    prices (clamped at the merge), the trace, the C2 and C4 shapes' windows: the oracle's bytes."""
+    import torch
+    opts = [(ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_STEP_PAIRS, 2)]
+    for (M, L, A, delta, qmax, T, S) in [(9, 256, 1024, 16, 100, 160, 91), (5, 512, 4096, 32, 100, 160, 40), (7, 128, 300, 8, 10, 160, 75),
+                                         (3, 256, 1000, 16, 100, 96, 33), (4, 128, 33, 8, 10, 64, 50), (2, 64, 0, 8, 10, 160, 9)]:
+        p = zi_params(delta, qmax)
+        ids = np.arange(M)
+        eb, er = oracle_rows(oracle, p, L, A, 3, ids, S)
+        for kw in (dict(), dict(split=[1, 2, S - 3]), dict(split=[3, S - 8, 5]), dict(stepwise=True)):
+            b, r = _gpu(ks, M, L, A, p, 3, S, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, T)], **kw)
+            assert_rows_equal(b, r, ids, eb, er, "pairs M=%d A=%d T=%d S=%d %r" % (M, A, T, S, kw))
+    for S in (1, 2, 3, 4, 5, 6, 7):
+        p = zi_params(16, 100)
+        eb, er = oracle_rows(oracle, p, 256, 700, 8, np.arange(4), S)
+        b, r = _gpu(ks, 4, 256, 700, p, 8, S, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, 160)])
+        assert_rows_equal(b, r, np.arange(4), eb, er, "pairs S=%d" % S)
+    M, L, A = 4, 128, 480
+    for init in (0, L - 1, 5):
+        q = dict(zi_params(8, 10), init_price=init)
+        eb, er, et = oracle.run_markets_traced(q, L, A, 2, np.arange(M), 61)
+        sim = ks.KsSim(M, L, A, q, 2)
+        for o, v in opts + [(ks.KS_OPT_BLOCK_THREADS, 160)]:
+            sim.ks_set_option(o, v)
+        tr = torch.empty((M, 61, 2), dtype=torch.int32, device="cuda")
+        sim.ks_run_traced(61, tr)
+        b, r = sim.books_to_host(), sim.stats_to_host()
+        sim.ks_destroy()
+        assert_rows_equal(b, r, np.arange(M), eb, er, "pairs traced init=%d" % init)
+        assert np.array_equal(tr.cpu().numpy(), et)
+
+
 def test_split_run_and_stepwise_ablation_are_bit_identical(ks, oracle):
     """ks_run(S1); ks_run(S2) == ks_run(S1+S2); the launch-per-step ablation (a8) == persistent."""
     c = CONFIGS["C3"]
