@@ -46,6 +46,7 @@ ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0,
 # hot loops).  tests/test_library_host.py counts them in the SASS of the built library, so these
 # constants cannot go stale silently.
 EXEC_MULTS_PER_CLASS = {"noise": 19.0, "maker": 14.0, "momentum": 19.0,                 # literal contract (a%3 classes)
+                        "noise_pair": 18.0,      # decoupled kernel, two steps per pass: rounds 0-2's step-independent products shared
                         "paper_noise": 19.0, "paper_momentum": 18.0, "paper_maker": 16.0,   # model 4 (all four words)
                         "packed_block": 17.0}                                               # one Philox block of 4 agents
 EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 14.0 + 19.0) / 3.0,
@@ -58,6 +59,14 @@ WIDE_MUL_LANES_PER_SM_PER_CLK = 4 * 8
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
 PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 24508928 + 237626880,            # profiles/r2c_c4_full.md
                                   "C4_packed4": 22112512 + 253766400}    # profiles/r2c_c4_packed4_full.md
+
+
+def exec_mults(params: dict, plan: str) -> float:
+    """Executed multiplies per event of the kernel the library's plan names (ks_plan_string)."""
+    mk = model_key(params)
+    if mk == "zi" and "steps_per_pass=2" in plan:
+        return EXEC_MULTS_PER_CLASS["noise_pair"]
+    return EXEC_MULTS_PER_EVENT[mk]
 
 
 def model_key(params: dict) -> str:
@@ -261,6 +270,7 @@ def time_case(ks, torch, dev, c, *, reps=3, mode="persistent", S=None, M=None, o
         try:
             for o, v in opts:
                 sim.ks_set_option(o, v)
+            plan = sim.ks_plan_string()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record()
             if mode == "stepwise":
@@ -276,7 +286,8 @@ def time_case(ks, torch, dev, c, *, reps=3, mode="persistent", S=None, M=None, o
         finally:
             sim.ks_destroy()
     ms = float(np.median(ts[warm:]))
-    return {"ms": ms, "events_per_s": float(M) * c.A * S / (ms * 1e-3), "M": M, "L": c.L, "A": c.A, "S": S, "reps": reps}
+    return {"ms": ms, "events_per_s": float(M) * c.A * S / (ms * 1e-3), "M": M, "L": c.L, "A": c.A, "S": S, "reps": reps,
+            "plan": plan}
 
 
 def run_case(args):
@@ -386,12 +397,17 @@ def main():
     base, M, M_job = rank_markets(cfg.M, rank, world, args.scaling)
     state = torch.empty(ks.ks_state_bytes(M, L), dtype=torch.uint8, device=dev)
 
+    plans = []
+
     def one_step(ev_pairs=None):
         sim = ks.KsSim(M, L, A, cfg.params, cfg.seed, market_base=base, state=state)
         if args.threads:
             sim.ks_set_option(ks.KS_OPT_BLOCK_THREADS, args.threads)
         if args.atomic_mode:
             sim.ks_set_option(ks.KS_OPT_ATOMIC_MODE, args.atomic_mode)
+        if args.pipeline:
+            sim.ks_set_option(ks.KS_OPT_PIPELINE, args.pipeline)
+        plans.append(sim.ks_plan_string())
         if ev_pairs is not None:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
@@ -524,8 +540,9 @@ def main():
     # ---- roofline of the dominant kernel (ks_persistent_kernel): bound by the 32x32->64 multiply pipe
     peak = mulwide_peak if mulwide_peak else peak_derived
     achieved = ALG_MULTS_PER_EVENT[model] * kev / 1e12
-    executed = EXEC_MULTS_PER_EVENT[model] * kev / 1e12
-    roofline = {"bound": "alu", "kernel": "ks_persistent_kernel", "achieved": achieved, "peak": peak,
+    exec_per_event = exec_mults(cfg.params, plans[-1])
+    executed = exec_per_event * kev / 1e12
+    roofline = {"bound": "alu", "kernel": plans[-1], "achieved": achieved, "peak": peak,
                 "unit": "T 32x32->64-bit integer multiplies/s", "frac": achieved / peak,
                 "frac_executed": executed / peak,
                 "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name if args.rng == "literal" else cfg.name + "_packed4"),
@@ -536,11 +553,12 @@ def main():
                 "frac_executed_of_derived_peak": executed / peak_derived,
                 "peak_derived_source": "%d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
                                        % (sms, sm_max_mhz, "MEASURED_PEAKS.json sm_max_mhz" if peaks else "NVML max clock"),
-                "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "executed_mults_per_event": EXEC_MULTS_PER_EVENT[model],
+                "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "executed_mults_per_event": exec_per_event,
                 "avg_launch_ms": avg_kern_s * 1e3,
                 "frac_note": "achieved/frac count the ALGORITHMIC multiplies (SURVEY.md S8(d): 22 per event); the kernel executes "
-                             "fewer (19: hoisted / strength-reduced rounds, w3 skipped; counted in the SASS by "
-                             "tests/test_library_host.py), so frac can pass 1.0 -- the pipe's own utilisation is frac_executed "
+                             "fewer (19, or 18 when two steps share a pass over the agents: hoisted / strength-reduced / shared "
+                             "rounds, w3 skipped; counted in the SASS by tests/test_library_host.py), so frac can pass 1.0 -- "
+                             "the pipe's own utilisation is frac_executed "
                              "(ncu: sm__pipe_fmaheavy_cycles_active, profiles/)",
                 "hbm": {"algorithmic_bytes": M * (8 * L + 128), "achieved_GBps": M * (8 * L + 128) / avg_kern_s / 1e9,
                         "peak_GBps": peaks.get("hbm_gbs", 6650.0),
@@ -596,8 +614,8 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
     out = {}
 
     def with_frac(r, c):
-        mk = model_key(c.params)
-        r["frac_executed"] = EXEC_MULTS_PER_EVENT[mk] * r["events_per_s"] / 1e12 / peak_tmults
+        r["executed_mults_per_event"] = exec_mults(c.params, r["plan"])
+        r["frac_executed"] = r["executed_mults_per_event"] * r["events_per_s"] / 1e12 / peak_tmults
         r["us_per_step"] = r["ms"] * 1e3 / r["S"]
         return r
 

@@ -257,14 +257,21 @@ typedef enum {
                                for each other's hand-over)                                                    */
   KS_OPT_STEP_PAIRS = 7,    /* decoupled kernel, KS_MODEL_ZI, <= 160 threads: the generating warps make TWO steps per
                                pass over their agents (the step-independent Philox rounds and the counter add are
-                               shared: 18 multiplies per event instead of 19) and hand them over together:
-                               0 = automatic, 1 = never, 2 = whenever legal                                     */
+                               shared: 18 multiplies per event instead of 19) and hand them over together (ring
+                               of 4, the clearing warp keeps the record): 0 = automatic (>= 4 events per
+                               generating thread and the grid not underfilled), 1 = never, 2 = whenever legal   */
   KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
                                i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
                                book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and
                                KS_OPT_ATOMIC_MODE 0                                                          */
 } ks_option;
 KS_API ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value);
+
+/* HOST-only: which kernel and launch shape the next ks_run on this handle will use under its current
+ * options, as text ("ks_persistent_kernel T=32", "ks_decoupled_kernel T=96 ring=4 steps_per_pass=2",
+ * "ks_cluster_kernel C=2") -- for logs and for bench.py, which must know how many multiplies per
+ * event the chosen kernel executes.  buf: HOST, n bytes, always NUL-terminated. */
+KS_API ks_status ks_plan_string(ks_sim* s, char* buf, size_t n);
 
 /* HOST-only helper: derive the fp64 statistics of n records. */
 KS_API void ks_derive_stats(const ks_market_stats* rec, ks_derived_stats* out, int64_t n);

@@ -28,7 +28,7 @@ DERIVED_FIELDS = ("mean_px", "vwap", "vol_per_step", "ret_mean", "ret_var", "exc
 # every symbol the two headers declare (tests check that each library exports exactly these)
 EXPORTS = ("ks_state_bytes", "ks_create", "ks_create_ex", "ks_attach", "ks_run", "ks_read_books", "ks_read_stats",
            "ks_write_books", "ks_run_traced", "ks_trace_stats", "ks_set_option", "ks_derive_stats", "ks_destroy", "ks_last_error",
-           "ks_launch_count", "ks_error_state")
+           "ks_launch_count", "ks_error_state", "ks_plan_string")
 BENCH_EXPORTS = ("ks_run_stepwise", "ks_bench_smem_atomic", "ks_bench_generate_only", "ks_bench_int_pipe")
 
 
@@ -96,6 +96,7 @@ def load():
     L.ks_set_option.argtypes = [vp, i32, i32]; L.ks_set_option.restype = i32
     L.ks_derive_stats.argtypes = [vp, vp, i64]; L.ks_derive_stats.restype = None
     L.ks_error_state.argtypes = [vp]; L.ks_error_state.restype = i32
+    L.ks_plan_string.argtypes = [vp, C.c_char_p, C.c_size_t]; L.ks_plan_string.restype = i32
     L.ks_destroy.argtypes = [vp]; L.ks_destroy.restype = None
     L.ks_last_error.argtypes = []; L.ks_last_error.restype = C.c_char_p
     L.ks_launch_count.argtypes = []; L.ks_launch_count.restype = i64
@@ -201,6 +202,11 @@ class KsSim:
 
     def ks_error_state(self):
         _check(load().ks_error_state(self._h))
+
+    def ks_plan_string(self) -> str:
+        buf = C.create_string_buffer(128)
+        _check(load().ks_plan_string(self._h, buf, 128))
+        return buf.value.decode()
 
     def ks_destroy(self):
         if self._h:

@@ -302,7 +302,7 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 // T = 32 beats 64/128 on C4).  A book so large that 32-thread CTAs would leave the SM short of
 // warps -> widen until ~1024 threads are resident; few markets -> widen so the whole GPU is used,
 // but never beyond the agents.
-struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; bool pair; };
+struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; int group; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
 
@@ -316,7 +316,7 @@ static uint32_t rel_side_for(const ks_sim* s) {
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
   pl.smem = (size_t)8 * (size_t)s->L;
-  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0; pl.pair = false;
+  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0; pl.group = 1;
   int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
   if (k < 1) k = 1;
   if (k > 32) k = 32;
@@ -353,6 +353,24 @@ static LaunchPlan plan_launch(const ks_sim* s) {
     const size_t dsmem = pl.smem + 2 * (size_t)ring * side;
     const bool fits = dsmem + 2048 <= (size_t)s->dev_smem_optin && !(s->opt_cols && ring != 2);
     const bool seven_fit = 7 * ((long long)dsmem + kSmemCtaOverhead) <= kSmemPerSM;
+    // (c) two steps per pass (GROUP = 2, ring of 4, the clearing warp keeps the record): the literal
+    //     contract with plain bins, >= 4 events per generating thread, seven CTAs fitting an SM, and
+    //     the grid not underfilled.  Measured on B200 (L = 256 / 512): faster than every other plan
+    //     for A >= 512 when an SM holds few markets (C2: 3.21 -> 2.99 ms) and for A >= 1024 at any M
+    //     (C4: 640 ms persistent -> 608 ms with T = 96); slower for 2 events per thread (A = 256).
+    const size_t gsmem = pl.smem + 8 * (size_t)side;
+    const bool group_legal = s->p.model == KS_MODEL_ZI && !s->opt_cols && s->opt_ring == 0 && s->opt_pair != 1 &&
+                             gsmem + 2048 <= (size_t)s->dev_smem_optin;
+    const bool group_fit7 = 7 * ((long long)gsmem + kSmemCtaOverhead) <= kSmemPerSM;
+    const bool group_auto = group_legal && group_fit7 && !underfilled && !s->opt_threads &&
+                            ((few_per_sm && s->A >= 512) || s->A >= 1024);
+    if (group_legal && (s->opt_pair == 2 || (s->opt_pair == 0 && group_auto))) {
+      int Td = s->opt_threads ? s->opt_threads : (few_per_sm ? 160 : 96);
+      if (Td >= 64 && Td <= 160) {
+        pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = 4; pl.group = 2; pl.smem = gsmem;
+        return pl;
+      }
+    }
     if (fits && (s->opt_pipe == 2 || underfilled || (few_per_sm && seven_fit))) {
       int Td = pl.T;
       if (!s->opt_threads) {
@@ -368,15 +386,7 @@ static LaunchPlan plan_launch(const ks_sim* s) {
           }
         }
       }
-      if (Td >= 64) {
-        pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem = dsmem;
-        // two steps per hand-over (literal contract, plain bins, the (160, 7) instantiation): ring of 4
-        const bool can_pair = s->p.model == KS_MODEL_ZI && !s->opt_cols && Td <= 160 && (s->opt_ring == 0 || s->opt_ring == 4) &&
-                              pl.smem - 2 * (size_t)ring * side + 8 * (size_t)side + 2048 <= (size_t)s->dev_smem_optin;
-        if (can_pair && s->opt_pair == 2) {
-          pl.pair = true; pl.smem += 2 * (size_t)(4 - ring) * side; pl.ring = 4;
-        }
-      }
+      if (Td >= 64) { pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = ring; pl.smem = dsmem; }
     }
   }
   return pl;
@@ -393,9 +403,9 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
   return cudaGetLastError();
 }
 
-template <bool PACKED, int COLS, int NB, int MAXT, int MINB, bool PAIR = false>
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1>
 static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB, PAIR>;
+  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB, GROUP>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -408,10 +418,10 @@ static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t 
 // of 7 resident CTAs of <= 160 threads when the block is that small (C2: 6.9 markets per SM must all
 // be resident) -- or the two-deep ring (ablation; the only one with lane-columned bins).
 template <bool PACKED>
-static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, bool pair, cudaStream_t st) {
+static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, int group, cudaStream_t st) {
   if (cols) return launch_decoupled_as<PACKED, 32, 2, 1024, 1>(P, T, smem, st);
   if constexpr (!PACKED) {
-    if (pair && ring == 4 && T <= 160) return launch_decoupled_as<false, 1, 4, 160, 7, true>(P, T, smem, st);
+    if (group == 2 && T <= 160) return launch_decoupled_as<false, 1, 4, 160, 7, 2>(P, T, smem, st);
   }
   if (ring == 2) return T <= 160 ? launch_decoupled_as<PACKED, 1, 2, 160, 7>(P, T, smem, st)
                                  : launch_decoupled_as<PACKED, 1, 2, 1024, 1>(P, T, smem, st);
@@ -521,8 +531,8 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     const LaunchPlan pl = plan_launch(s);
     P.rel_side = pl.rel_side; P.rel_stride = 2 * pl.rel_side;
     if (pl.decoupled) {
-      e = packed ? launch_decoupled<true>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.pair, st)
-                 : launch_decoupled<false>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.pair, st);
+      e = packed ? launch_decoupled<true>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.group, st)
+                 : launch_decoupled<false>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.group, st);
     } else if (paper)
       e = launch_persistent<2, 0, false>(P, pl.T, pl.smem, st);
     else if (packed)
@@ -556,6 +566,22 @@ ks_status ks_trace_stats(const int32_t* d_trace, int32_t M, int64_t S, int32_t K
       reinterpret_cast<const int2*>(d_trace), M, (long long)S, K, d_out);
   KS_CUDA(cudaGetLastError());
   g_launches++;
+  return KS_OK;
+}
+
+ks_status ks_plan_string(ks_sim* s, char* buf, size_t n) {
+  if (!s || !buf || n == 0) { set_err("ks_plan_string: bad argument"); return KS_ERR_INVALID_ARG; }
+  int C = s->opt_cluster;
+  if (C == 0) C = s->L > kMaxLPerCta ? s->L / kMaxLPerCta : 1;
+  if (C > 1) {
+    snprintf(buf, n, "ks_cluster_kernel C=%d", C);
+    return KS_OK;
+  }
+  const LaunchPlan pl = plan_launch(s);
+  if (pl.decoupled)
+    snprintf(buf, n, "ks_decoupled_kernel T=%d ring=%d steps_per_pass=%d%s", pl.T, pl.ring, pl.group, s->opt_cols ? " lane_columns" : "");
+  else
+    snprintf(buf, n, "ks_persistent_kernel T=%d", pl.T);
   return KS_OK;
 }
 

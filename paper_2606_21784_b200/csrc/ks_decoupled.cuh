@@ -73,9 +73,10 @@ __device__ __forceinline__ void red32(uint32_t saddr, int v) { asm volatile("red
 // posts (Vmax, p*, price before) in an NB-slot mailbox.  The record (a6) and the trace are kept by
 // the FIRST GENERATING warp, which picks the mail of step s-NB up when it passes the free[]
 // barrier it waits at anyway; the last NB mails are taken after the loop.
-template <bool PACKED, int COLS, int NB, int MAXT, int MINB, bool PAIR = false>
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1>
 __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_constant__ KernelParams P) {
-  static_assert(!PAIR || (NB == 4 && COLS == 1 && !PACKED), "PAIR: two steps per hand-over, ring of 4, literal contract");
+  constexpr bool PAIR = GROUP > 1;      // GROUP = 2 or 4 steps per pass over the agents and per hand-over
+  static_assert(!PAIR || (NB == 2 * GROUP && COLS == 1 && !PACKED), "GROUP steps per hand-over: ring of 2*GROUP, literal contract");
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then rel[NB][P.rel_stride / 4]
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
@@ -231,7 +232,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
         clear_active_window(io, L, lo, hi, P.force_generic != 0, lane, vmax, pstar, lbnd, base, wend);
       }
     };
-    if (!PAIR) {
+    if constexpr (!PAIR) {
     for (uint32_t s0 = 0; s0 < S; s0 += NB) {
 #pragma unroll
         for (int buf = 0; buf < NB; ++buf) {                 // ring slot = step mod NB, a compile-time constant here
@@ -255,21 +256,22 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
         }
       }
     }
-    if (PAIR) {
-      // two steps per hand-over: ring slots 2p, 2p+1 belong to pair p = (s / 2) mod 2; one full[p] /
-      // free[p] barrier per pair (ids: full 1 + p, free 3 + p); the two steps are cleared by a rolled loop
-      for (uint32_t s0 = 0; s0 < S; s0 += 4) {
+    if constexpr (PAIR) {
+      // GROUP steps per hand-over: ring slots GROUP*p .. GROUP*p + GROUP-1 belong to group p = (s / GROUP) mod 2;
+      // one full[p] / free[p] barrier per group (ids: full 1 + p, free 3 + p); the steps of a group are
+      // cleared by a rolled loop
+      for (uint32_t s0 = 0; s0 < S; s0 += 2 * GROUP) {
 #pragma unroll
         for (int pr = 0; pr < 2; ++pr) {
-          const uint32_t s = s0 + 2u * (uint32_t)pr;
+          const uint32_t s = s0 + (uint32_t)(GROUP * pr);
           if (s >= S) break;
-          const uint32_t ns = min(2u, S - s);
+          const uint32_t ns = min((uint32_t)GROUP, S - s);
           for (uint32_t g = 0; g < ns; ++g) {
-            const int slot = 2 * pr + (int)g;
+            const int slot = GROUP * pr + (int)g;
             clear_core(rel_saddr + (uint32_t)slot * P.rel_stride, slot, [&] { if (g == 0) bar_sync_b<1, 2>(pr, T); });
             if (g + 1 == ns) {
               __syncwarp();
-              if (s + 4 < S) bar_arrive_b<3, 2>(pr, T);    // both histograms empty again: steps s+4, s+5 may start
+              if (s + 2 * GROUP < S) bar_arrive_b<3, 2>(pr, T);   // the group's histograms are empty again
             }
             update_record_reg(rec_reg, ovf_reg, lane, last, vmax, pstar, last);
             if (P.trace) trace_step(s_trace, P.trace + (size_t)blockIdx.x * (size_t)S, (long long)(s + g), (long long)S, lane,
@@ -295,29 +297,37 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
     const uint32_t col = COLS == 32 ? 4u * (uint32_t)lane : 0u;
     const uint32_t bin_bytes = COLS == 32 ? 128u : 4u;
     int sink = 0;
-    if (PAIR) {
-      // two steps per pass over the agents: for one agent the Philox rounds that do not depend on the
-      // step (M0*a, M1*n2, M0*c0: two multiplies and two xors of round 0-2) and the counter add are
-      // shared by the two steps, and the per-step prologue of the loop is paid once per pair
-      RuleCtx rc1 = rc;
-      BookRef bref1 = bref;
-      for (uint32_t s0 = 0; s0 < S; s0 += 4) {
+    if constexpr (PAIR) {
+      // GROUP steps per pass over the agents: for one agent the Philox rounds that do not depend on
+      // the step (M0*a, M1*n2, M0*c0: two multiplies and two xors of rounds 0-2) and the counter add
+      // are shared by the GROUP steps, and the per-step prologue of the loop is paid once per group
+      for (uint32_t s0 = 0; s0 < S; s0 += 2 * GROUP) {
 #pragma unroll
         for (int pr = 0; pr < 2; ++pr) {
-          const uint32_t s = s0 + 2u * (uint32_t)pr;
+          const uint32_t s = s0 + (uint32_t)(GROUP * pr);
           if (s >= S) break;
-          const bool two = s + 1 < S;
-          const StepUniform u0 = step_uniform(P, mu, t0 + s), u1 = step_uniform(P, mu, t0 + s + 1);
-          rc.rel_s = rel_saddr + (uint32_t)(2 * pr) * P.rel_stride;
-          rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * 4u;
-          rc1.rel_s = rc.rel_s + P.rel_stride; rc1.rel_b = rc.rel_b + P.rel_stride;
+          const uint32_t slot0 = rel_saddr + (uint32_t)(GROUP * pr) * P.rel_stride;
+          if (s0 != 0u) bar_sync_b<3, 2>(pr, T);           // free[pr]: the clearing warp has drained the group's histograms
+          if (s + GROUP <= S) {
+            StepUniform ug[GROUP];
+#pragma unroll
+            for (int g = 0; g < GROUP; ++g) ug[g] = step_uniform(P, mu, t0 + s + (uint32_t)g);
 #ifdef KS_DEBUG_CHECKS
-          bref.dbg_lo = rc.rel_s; bref.dbg_hi = bref.dbg_lo + P.rel_stride; bref.dbg_count = &s_dbg_count[2 * pr];
-          bref1.dbg_lo = rc1.rel_s; bref1.dbg_hi = bref1.dbg_lo + P.rel_stride; bref1.dbg_count = &s_dbg_count[2 * pr + 1];
+            bref.dbg_lo = slot0; bref.dbg_hi = slot0 + GROUP * P.rel_stride; bref.dbg_count = &s_dbg_count[GROUP * pr];
 #endif
-          if (s0 != 0u) bar_sync_b<3, 2>(pr, T);           // free[pr]: the clearing warp has drained both histograms
-          if (two) generate_class_rel_pair<ATOM>(P, bref, bref1, mu, u0, u1, rc, rc1, gplan.cls[0], gplan.p0_inc, sink);
-          else     generate_step<0, ATOM, PACKED>(P, bref, mu, u0, rc, gplan, tid == 0, sink);
+            generate_class_rel_group<ATOM, GROUP>(P, bref, mu, ug, slot0, P.rel_stride, P.rel_side + (uint32_t)(n - 1) * 4u,
+                                                  gplan.cls[0], gplan.p0_inc, sink);
+          } else {                                         // the run's last, partial group: step by step
+            for (uint32_t g = 0; s + g < S; ++g) {
+              const StepUniform u = step_uniform(P, mu, t0 + s + g);
+              rc.rel_s = slot0 + g * P.rel_stride;
+              rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * 4u;
+#ifdef KS_DEBUG_CHECKS
+              bref.dbg_lo = rc.rel_s; bref.dbg_hi = bref.dbg_lo + P.rel_stride; bref.dbg_count = &s_dbg_count[GROUP * pr + (int)g];
+#endif
+              generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+            }
+          }
           bar_arrive_b<1, 2>(pr, T);                       // full[pr]
         }
       }
@@ -348,12 +358,13 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
         }
       }
     };
-    if (PAIR)            { }
-    else if (nmax == 1u) gen_loop(std::integral_constant<int, 1>{});
-    else if (nmax == 2u) gen_loop(std::integral_constant<int, 2>{});
-    else if (nmax == 3u) gen_loop(std::integral_constant<int, 3>{});
-    else if (nmax == 4u) gen_loop(std::integral_constant<int, 4>{});
-    else                 gen_loop(std::integral_constant<int, 0>{});
+    if constexpr (!PAIR) {
+      if (nmax == 1u)      gen_loop(std::integral_constant<int, 1>{});
+      else if (nmax == 2u) gen_loop(std::integral_constant<int, 2>{});
+      else if (nmax == 3u) gen_loop(std::integral_constant<int, 3>{});
+      else if (nmax == 4u) gen_loop(std::integral_constant<int, 4>{});
+      else                 gen_loop(std::integral_constant<int, 0>{});
+    }
   }
   __syncthreads();                                         // the last clearing is done
   if (bookkeeper) {                                        // the mails of the last NB steps, then the record goes back

@@ -588,25 +588,31 @@ __device__ __forceinline__ void generate_class_rel_few(const KernelParams& P, co
     if (e < n_mine) book_add_at<0>(book, addr[e], q[e], sink);
 }
 
-// Two steps of the noise class in one pass over a thread's agents (ks_decoupled_kernel, PAIR): the
-// same agent's orders of steps t (-> rc0's histogram) and t+1 (-> rc1's).  Written as two plain
-// Philox evaluations on the same p0: everything that does not depend on the step -- n2, M1*n2, c0,
-// c1, M0*c0 -- is common to both and is computed once (18 multiplies per event instead of 19, two
-// xors and the 64-bit counter add shared).  Two agents per unrolled trip = four chains.
-template <int ATOM>
-__device__ __forceinline__ void generate_class_rel_pair(const KernelParams& P, const BookRef& book0, const BookRef& book1,
-                                                        const MarketUniform& mu, const StepUniform& u0, const StepUniform& u1,
-                                                        const RuleCtx& rc0, const RuleCtx& rc1, const ClassPlan& pl,
-                                                        const P0Step& p0_inc, int& sink) {
+// G steps of the noise class in one pass over a thread's agents (ks_decoupled_kernel, GROUP): the
+// same agent's orders of steps t .. t+G-1, step g into the relative histogram at slot0 + g*stride.
+// Written as G plain Philox evaluations on the same p0: everything that does not depend on the
+// step -- n2, M1*n2, c0, c1, M0*c0 -- is common to all and is computed once (G = 2: 18 multiplies
+// per event instead of 19, G = 4: 17.5; two xors and the 64-bit counter add shared as well).
+// Four chains per unrolled trip (4 / G agents).
+template <int ATOM, int G>
+__device__ __forceinline__ void generate_class_rel_group(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                                         const StepUniform (&u)[G], uint32_t slot0, uint32_t stride,
+                                                         uint32_t buy_off, const ClassPlan& pl, const P0Step& p0_inc, int& sink) {
+  static_assert(ATOM == 4, "plain bins");
   auto one = [&](uint64_t p0) {
-    uint32_t a0, a1, a2, b0, b1, b2;
-    philox_from_p0<true>(P, mu, u0, p0, a0, a1, a2);
-    philox_from_p0<true>(P, mu, u1, p0, b0, b1, b2);
-    noise_order<ATOM, false>(P, book0, rc0, a0, a1, a2, sink);
-    noise_order<ATOM, false>(P, book1, rc1, b0, b1, b2, sink);
+    uint32_t w0[G], w1[G], w2[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) philox_from_p0<true>(P, mu, u[g], p0, w0[g], w1[g], w2[g]);
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      RuleCtx rc;
+      rc.rel_s = slot0 + (uint32_t)g * stride;
+      rc.rel_b = rc.rel_s + buy_off;
+      noise_order<ATOM, false>(P, book, rc, w0[g], w1[g], w2[g], sink);
+    }
   };
   uint64_t p0 = pl.p0;
-#pragma unroll 2
+#pragma unroll(4 / G)
   for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, p0_inc.inc, p0_inc.a_step); }
   if (pl.extra) one(p0);
 }

@@ -157,14 +157,15 @@ def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
         assert_rows_equal(b, r, np.arange(M), eb, er, "decoupled injected cols=%d" % cols)
 
 
-def test_step_pairs_give_identical_bytes(ks, oracle):
-    """KS_OPT_STEP_PAIRS: the decoupled kernel's generating warps make two steps per pass over
-    their agents (shared step-independent Philox rounds) and hand them over together; the clearing
-    warp keeps the record.  Odd and tiny step counts (the last pair holds one step), split and
-    launch-per-step runs (a pair never spans two ks_run calls), ragged agent counts, grid-edge
+@pytest.mark.parametrize("group", [2])
+def test_step_pairs_give_identical_bytes(ks, oracle, group):
+    """KS_OPT_STEP_PAIRS: the decoupled kernel's generating warps make two steps per pass
+    over their agents (shared step-independent Philox rounds) and hand them over together; the
+    clearing warp keeps the record.  Step counts that leave a partial last group, split and
+    launch-per-step runs (a group never spans two ks_run calls), ragged agent counts, grid-edge
     prices (clamped at the merge), the trace, the C2 and C4 shapes' windows: the oracle's bytes."""
     import torch
-    opts = [(ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_STEP_PAIRS, 2)]
+    opts = [(ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_STEP_PAIRS, group)]
     for (M, L, A, delta, qmax, T, S) in [(9, 256, 1024, 16, 100, 160, 91), (5, 512, 4096, 32, 100, 160, 40), (7, 128, 300, 8, 10, 160, 75),
                                          (3, 256, 1000, 16, 100, 96, 33), (4, 128, 33, 8, 10, 64, 50), (2, 64, 0, 8, 10, 160, 9)]:
         p = zi_params(delta, qmax)
@@ -173,7 +174,7 @@ def test_step_pairs_give_identical_bytes(ks, oracle):
         for kw in (dict(), dict(split=[1, 2, S - 3]), dict(split=[3, S - 8, 5]), dict(stepwise=True)):
             b, r = _gpu(ks, M, L, A, p, 3, S, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, T)], **kw)
             assert_rows_equal(b, r, ids, eb, er, "pairs M=%d A=%d T=%d S=%d %r" % (M, A, T, S, kw))
-    for S in (1, 2, 3, 4, 5, 6, 7):
+    for S in (1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13):
         p = zi_params(16, 100)
         eb, er = oracle_rows(oracle, p, 256, 700, 8, np.arange(4), S)
         b, r = _gpu(ks, 4, 256, 700, p, 8, S, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, 160)])
