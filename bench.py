@@ -34,7 +34,7 @@ if ROOT not in sys.path:
 from paper_2606_21784_b200.workloads import (CONFIGS, KS_MODEL_PAPER, KS_MODEL_ZI, packed4, paper_params,  # noqa: E402
                                              sampled_markets, shard_markets, zi_params)
 
-# Roofline of ks_persistent_kernel: the fmaheavy pipe that executes the 32x32->64
+# Roofline of the headline kernel: the fmaheavy pipe that executes the 32x32->64
 # multiplies.  Algorithmic multiplies per agent event: 20 of Philox4x32-10 + the
 # mulhi draws of the rule (noise/momentum: offset and quantity; maker: spread only).
 ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0,

@@ -414,6 +414,10 @@ static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t 
   return cudaGetLastError();
 }
 
+#ifndef KS_GROUP_MAXT
+#define KS_GROUP_MAXT 160      // launch bounds of the two-steps-per-pass instantiation: 7 CTAs of 160 threads per SM
+#define KS_GROUP_MINB 7        // (56 registers)
+#endif
 // The decoupled kernel's instantiations: ring of 4 histograms (default) -- with the register budget
 // of 7 resident CTAs of <= 160 threads when the block is that small (C2: 6.9 markets per SM must all
 // be resident) -- or the two-deep ring (ablation; the only one with lane-columned bins).
@@ -421,7 +425,7 @@ template <bool PACKED>
 static cudaError_t launch_decoupled(const ks::KernelParams& P, int T, size_t smem, int cols, int ring, int group, cudaStream_t st) {
   if (cols) return launch_decoupled_as<PACKED, 32, 2, 1024, 1>(P, T, smem, st);
   if constexpr (!PACKED) {
-    if (group == 2 && T <= 160) return launch_decoupled_as<false, 1, 4, 160, 7, 2>(P, T, smem, st);
+    if (group == 2 && T <= 160) return launch_decoupled_as<false, 1, 4, KS_GROUP_MAXT, KS_GROUP_MINB, 2>(P, T, smem, st);
   }
   if (ring == 2) return T <= 160 ? launch_decoupled_as<PACKED, 1, 2, 160, 7>(P, T, smem, st)
                                  : launch_decoupled_as<PACKED, 1, 2, 1024, 1>(P, T, smem, st);
