@@ -55,9 +55,9 @@ EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 14.0 + 19.0) / 3.0,
                         "paper": 0.70 * 19.0 + 0.15 * 18.0 + 0.15 * 16.0}
 # derived peak: a 32-lane IMAD.WIDE/IMAD.HI occupies an SMSP's fmaheavy pipe for 4 cycles -> 8 lanes/clk/SMSP
 WIDE_MUL_LANES_PER_SM_PER_CLK = 4 * 8
-# dram__bytes_read.sum + dram__bytes_write.sum of one ks_persistent_kernel launch from the
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the headline kernel from the
 # `ncu --set full` capture summarised under profiles/ (None until measured for that config).
-PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 24508928 + 237626880,            # profiles/r2c_c4_full.md
+PROFILED_DRAM_BYTES_PER_LAUNCH = {"C4": 26893824 + 238403072,            # profiles/r2d_c4_full.md
                                   "C4_packed4": 22112512 + 253766400}    # profiles/r2c_c4_packed4_full.md
 
 
