@@ -600,10 +600,10 @@ def main():
 
 # dram__bytes_read.sum + dram__bytes_write.sum and the L1 global load + store bytes, summed over the
 # launches of one run, from the ncu captures of `bench.py --case C2 --S 1000 [--mode stepwise]`
-# (profiles/r2c_traffic.md): measured counters, not algorithmic bytes.
-PROFILED_TRAFFIC_C2 = {"persistent": {"dram_bytes": 232704 + 0, "global_load_store_bytes": 131072 + 2228224},
-                       "launch_per_step": {"dram_bytes": 2312446208 + 0, "global_load_store_bytes": 2226e6 + 2228e6},
-                       "source": "profiles/r2c_traffic.md (ncu; the L2 is invalidated between launches under ncu)"}
+# (profiles/r2d_traffic.md): measured counters, not algorithmic bytes.
+PROFILED_TRAFFIC_C2 = {"persistent": {"dram_bytes": 215040 + 0, "global_load_store_bytes": 131072 + 2228224},
+                       "launch_per_step": {"dram_bytes": 2301881088 + 0, "global_load_store_bytes": 2226e6 + 2228e6},
+                       "source": "profiles/r2d_traffic.md (ncu; the L2 is invalidated between launches under ncu)"}
 
 
 def extras(ks, torch, dev, peak_tmults, headline_cfg):
