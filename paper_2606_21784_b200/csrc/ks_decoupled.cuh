@@ -144,11 +144,9 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   if (clearing) {
     const LocalBook io{book, L};
     const unsigned FULL = 0xffffffffu;
-    int vmax, pstar, base, wend;
-    LaneBounds lbnd;
     // a2 (second half) + a3-a5 of one step on the histogram whose sell bins start at rs (ring slot
     // `slot`); wait() is called where the histogram is first needed
-    auto clear_core = [&](uint32_t rs, int slot, auto wait) {
+    auto clear_core = [&](uint32_t rs, int slot, auto wait, int& vmax, int& pstar, int& base, int& wend, LaneBounds& lbnd) {
       (void)slot;
       const uint32_t rb = rs + P.rel_side;                           // buy bins
       const int t_lo = last - delta;                     // tick of bin 0
@@ -238,7 +236,9 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
         for (int buf = 0; buf < NB; ++buf) {                 // ring slot = step mod NB, a compile-time constant here
           const uint32_t s = s0 + (uint32_t)buf;
           if (s >= S) break;
-          clear_core(rel_saddr + (uint32_t)buf * P.rel_stride, buf, [&] { bar_sync_b<kBarFull0, NB>(buf, T); });
+          int vmax, pstar, base, wend;
+          LaneBounds lbnd;
+          clear_core(rel_saddr + (uint32_t)buf * P.rel_stride, buf, [&] { bar_sync_b<kBarFull0, NB>(buf, T); }, vmax, pstar, base, wend, lbnd);
           if (!kClearingKeepsBooks) {
             if (lane == 0) *reinterpret_cast<int4*>(s_mail[buf]) = make_int4(vmax, pstar, last, 0);
           }
@@ -268,7 +268,9 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
           const uint32_t ns = min((uint32_t)GROUP, S - s);
           for (uint32_t g = 0; g < ns; ++g) {
             const int slot = GROUP * pr + (int)g;
-            clear_core(rel_saddr + (uint32_t)slot * P.rel_stride, slot, [&] { if (g == 0) bar_sync_b<1, 2>(pr, T); });
+            int vmax, pstar, base, wend;
+            LaneBounds lbnd;
+            clear_core(rel_saddr + (uint32_t)slot * P.rel_stride, slot, [&] { if (g == 0) bar_sync_b<1, 2>(pr, T); }, vmax, pstar, base, wend, lbnd);
             if (g + 1 == ns) {
               __syncwarp();
               if (s + 2 * GROUP < S) bar_arrive_b<3, 2>(pr, T);   // the group's histograms are empty again
