@@ -144,6 +144,9 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   if (clearing) {
     const LocalBook io{book, L};
     const unsigned FULL = 0xffffffffu;
+#ifdef KS_DEBUG_CHECKS
+    int dbg_steps = 1;                                   // steps handed over with the group being cleared
+#endif
     // a2 (second half) + a3-a5 of one step on the histogram whose sell bins start at rs (ring slot
     // `slot`); wait() is called where the histogram is first needed
     auto clear_core = [&](uint32_t rs, int slot, auto wait, int& vmax, int& pstar, int& base, int& wend, LaneBounds& lbnd) {
@@ -156,7 +159,13 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
       const bool fuse = COLS == 1 && inside && !P.force_generic;
       wait();                                            // every order of this step is in the histogram
 #ifdef KS_DEBUG_CHECKS
-      if (lane == 0) { KS_CHECK(s_dbg_count[slot] == P.A, "orders in the histogram at full[] != agents"); s_dbg_count[slot] = 0; }
+      // (GROUP steps per hand-over: the whole group's orders are counted in its first slot's counter and
+      // checked when its first step is cleared)
+      if (lane == 0 && (!PAIR || slot % GROUP == 0)) {
+        const int steps_here = PAIR ? dbg_steps : 1;
+        KS_CHECK(s_dbg_count[slot] == steps_here * P.A, "orders in the histogram(s) at full[] != agents x steps handed over");
+        s_dbg_count[slot] = 0;
+      }
       __syncwarp();
 #endif
       if (fuse && hi - lo < 32) {
@@ -266,6 +275,9 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
           const uint32_t s = s0 + (uint32_t)(GROUP * pr);
           if (s >= S) break;
           const uint32_t ns = min((uint32_t)GROUP, S - s);
+#ifdef KS_DEBUG_CHECKS
+          dbg_steps = (int)ns;
+#endif
           for (uint32_t g = 0; g < ns; ++g) {
             const int slot = GROUP * pr + (int)g;
             int vmax, pstar, base, wend;
@@ -325,7 +337,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
               rc.rel_s = slot0 + g * P.rel_stride;
               rc.rel_b = rc.rel_s + P.rel_side + (uint32_t)(n - 1) * 4u;
 #ifdef KS_DEBUG_CHECKS
-              bref.dbg_lo = rc.rel_s; bref.dbg_hi = bref.dbg_lo + P.rel_stride; bref.dbg_count = &s_dbg_count[GROUP * pr + (int)g];
+              bref.dbg_lo = rc.rel_s; bref.dbg_hi = bref.dbg_lo + P.rel_stride; bref.dbg_count = &s_dbg_count[GROUP * pr];
 #endif
               generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
             }

@@ -6,6 +6,7 @@ Each case goes through the C ABI and is compared with the oracle, so a hazard th
 fails here too.  Sizes are tiny because the sanitizer serialises the GPU.  Cases (SURVEY.md S4(4),
 Alg.1's phase structure PAPER.md:143-176, 200-212):
   c1          C1 in the automatic plan (ks_decoupled_kernel: named barriers, two-step look-ahead)
+  pairs       the two-steps-per-pass decoupled kernel (groups of ring slots handed over together), odd and split S
   c5          a shrunk C5 (M=4, L=4096, A=1500, S=20, MIX3): ks_persistent_kernel, several warps, two barriers
   t32         one warp per market (T = 32): the barrier-light path C4 runs
   cluster     C = 4 CTAs per market, L = 1024: DSMEM reductions, barrier.cluster
@@ -51,6 +52,12 @@ def c1():
     c = CONFIGS["C1"]
     check("c1", c.M, c.L, c.A, c.params, c.seed, c.S)
     check("c1 decoupled 3 markets", 3, 128, 512, zi_params(8, 10), 2, 40, opts=[(ks.KS_OPT_PIPELINE, 2)])
+
+
+def pairs():
+    opts = [(ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_STEP_PAIRS, 2)]
+    check("pairs C2 shape, odd S", 9, 256, 1024, zi_params(16, 100), 1, 41, opts=opts)
+    check("pairs T=96 split", 5, 512, 1500, zi_params(32, 100), 3, 30, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, 96)], split=[1, 4, 25])
 
 
 def c5():
@@ -112,7 +119,7 @@ def attach():
     print("attach ok", flush=True)
 
 
-CASES = dict(c1=c1, c5=c5, t32=t32, cluster=cluster, paper=paper, traced=traced, packed=packed, generic=generic, attach=attach)
+CASES = dict(c1=c1, pairs=pairs, c5=c5, t32=t32, cluster=cluster, paper=paper, traced=traced, packed=packed, generic=generic, attach=attach)
 
 if __name__ == "__main__":
     ks.load()
