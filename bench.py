@@ -47,6 +47,7 @@ ALG_MULTS_PER_EVENT = {"zi": 22.0, "mix3": (22.0 + 21.0 + 22.0) / 3.0,
 # constants cannot go stale silently.
 EXEC_MULTS_PER_CLASS = {"noise": 19.0, "maker": 14.0, "momentum": 19.0,                 # literal contract (a%3 classes)
                         "noise_pair": 18.0,      # decoupled kernel, two steps per pass: rounds 0-2's step-independent products shared
+                        "maker_pair": 13.0, "momentum_pair": 18.0,
                         "paper_noise": 19.0, "paper_momentum": 18.0, "paper_maker": 16.0,   # model 4 (all four words)
                         "packed_block": 17.0}                                               # one Philox block of 4 agents
 EXEC_MULTS_PER_EVENT = {"zi": 19.0, "mix3": (19.0 + 14.0 + 19.0) / 3.0,
@@ -66,6 +67,8 @@ def exec_mults(params: dict, plan: str) -> float:
     mk = model_key(params)
     if mk == "zi" and "steps_per_pass=2" in plan:
         return EXEC_MULTS_PER_CLASS["noise_pair"]
+    if mk == "mix3" and "steps_per_pass=2" in plan:
+        return (EXEC_MULTS_PER_CLASS["noise_pair"] + EXEC_MULTS_PER_CLASS["maker_pair"] + EXEC_MULTS_PER_CLASS["momentum_pair"]) / 3.0
     return EXEC_MULTS_PER_EVENT[mk]
 
 

@@ -302,7 +302,7 @@ ks_status ks_set_option(ks_sim* s, int32_t option, int32_t value) {
 // T = 32 beats 64/128 on C4).  A book so large that 32-thread CTAs would leave the SM short of
 // warps -> widen until ~1024 threads are resident; few markets -> widen so the whole GPU is used,
 // but never beyond the agents.
-struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; int group; };
+struct LaunchPlan { int T; size_t smem; bool decoupled; uint32_t rel_side; int ring; int group; bool mix; uint32_t rel_stride, mk_off, mom_off, mom_side; };
 
 static const long long kSmemPerSM = 228LL * 1024, kSmemCtaOverhead = 1024 + 1024;   // reserve + static
 
@@ -316,7 +316,7 @@ static uint32_t rel_side_for(const ks_sim* s) {
 static LaunchPlan plan_launch(const ks_sim* s) {
   LaunchPlan pl;
   pl.smem = (size_t)8 * (size_t)s->L;
-  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0; pl.group = 1;
+  pl.decoupled = false; pl.rel_side = 0; pl.ring = 0; pl.group = 1; pl.mix = false; pl.rel_stride = 0; pl.mk_off = pl.mom_off = pl.mom_side = 0;
   int k = (int)(kSmemPerSM / ((long long)pl.smem + kSmemCtaOverhead));
   if (k < 1) k = 1;
   if (k > 32) k = 32;
@@ -342,6 +342,29 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   //      clearing warp (T = 160) win.  Measured on B200, L = 256, delta = 16, A = 256..4096:
   //      the decoupled kernel is faster up to M = 2048 (13.8 markets per SM: +4 % .. +37 %) and
   //      slower at M = 4096 (-2 % .. -10 %), where the persistent kernel runs one warp per market.
+  //  (d) the three-type population (KS_MODEL_MIX3, literal draws): two steps per pass with every rule
+  //      relative to the step's opening price (generate_mix3_rel_group); needs >= 4 events per
+  //      generating thread and class, small maker / momentum ranges (<= 64 bins) and four CTAs per SM.
+  if (s->p.model == KS_MODEL_MIX3 && !s->opt_atomic && s->opt_pipe != 1 && s->opt_pair != 1 && !s->opt_cols && s->opt_ring == 0 &&
+      s->p.maker_spread_max <= 64 && s->p.mom_delta + 1 <= 64) {
+    const uint32_t side = rel_side_for(s);
+    const uint32_t mk = (((uint32_t)s->p.maker_spread_max * 4u + 127u) / 128u) * 128u;
+    const uint32_t ms = (((uint32_t)(s->p.mom_delta + 1) * 4u + 127u) / 128u) * 128u;
+    const uint32_t stride = 2 * side + mk + 2 * ms;
+    const size_t gsmem = pl.smem + 4 * (size_t)stride;
+    const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
+    const bool legal = gsmem + 2048 <= (size_t)s->dev_smem_optin;
+    const bool fit4 = 4 * ((long long)gsmem + kSmemCtaOverhead) <= kSmemPerSM;
+    const bool autom = legal && fit4 && !underfilled && !s->opt_threads && s->A >= 3 * 128 * 4 && s->opt_pipe != 2;
+    if (legal && (s->opt_pair == 2 || s->opt_pipe == 2 || (s->opt_pair == 0 && autom))) {
+      const int Td = s->opt_threads ? s->opt_threads : 160;
+      if (Td >= 64 && Td <= 160) {
+        pl.T = Td; pl.decoupled = true; pl.rel_side = side; pl.ring = 4; pl.group = 2; pl.mix = true; pl.smem = gsmem;
+        pl.rel_stride = stride; pl.mk_off = 2 * side; pl.mom_off = 2 * side + mk; pl.mom_side = ms;
+        return pl;
+      }
+    }
+  }
   const bool zi = s->p.model == KS_MODEL_ZI || s->p.model == KS_MODEL_ZI_PACKED4;
   if (zi && !s->opt_atomic && s->opt_pipe != 1) {
     const bool underfilled = (long long)s->M * pl.T < (long long)s->num_sms * 512;
@@ -403,9 +426,9 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
   return cudaGetLastError();
 }
 
-template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1>
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1, bool MIX = false>
 static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
-  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB, GROUP>;
+  auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB, GROUP, MIX>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -533,8 +556,11 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
     else         e = mix ? launch_cluster<1, true>(P, C, T, st) : launch_cluster<0, true>(P, C, T, st);
   } else {
     const LaunchPlan pl = plan_launch(s);
-    P.rel_side = pl.rel_side; P.rel_stride = 2 * pl.rel_side;
-    if (pl.decoupled) {
+    P.rel_side = pl.rel_side; P.rel_stride = pl.mix ? pl.rel_stride : 2 * pl.rel_side;
+    P.rel_mk_off = pl.mk_off; P.rel_mom_off = pl.mom_off; P.rel_mom_side = pl.mom_side;
+    if (pl.decoupled && pl.mix) {
+      e = launch_decoupled_as<false, 1, 4, KS_GROUP_MAXT, KS_GROUP_MINB, 2, true>(P, pl.T, pl.smem, st);
+    } else if (pl.decoupled) {
       e = packed ? launch_decoupled<true>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.group, st)
                  : launch_decoupled<false>(P, pl.T, pl.smem, s->opt_cols, pl.ring, pl.group, st);
     } else if (paper)
@@ -583,7 +609,8 @@ ks_status ks_plan_string(ks_sim* s, char* buf, size_t n) {
   }
   const LaunchPlan pl = plan_launch(s);
   if (pl.decoupled)
-    snprintf(buf, n, "ks_decoupled_kernel T=%d ring=%d steps_per_pass=%d%s", pl.T, pl.ring, pl.group, s->opt_cols ? " lane_columns" : "");
+    snprintf(buf, n, "ks_decoupled_kernel T=%d ring=%d steps_per_pass=%d%s%s", pl.T, pl.ring, pl.group, s->opt_cols ? " lane_columns" : "",
+             pl.mix ? " mix3" : "");
   else
     snprintf(buf, n, "ks_persistent_kernel T=%d", pl.T);
   return KS_OK;

@@ -73,10 +73,14 @@ __device__ __forceinline__ void red32(uint32_t saddr, int v) { asm volatile("red
 // posts (Vmax, p*, price before) in an NB-slot mailbox.  The record (a6) and the trace are kept by
 // the FIRST GENERATING warp, which picks the mail of step s-NB up when it passes the free[]
 // barrier it waits at anyway; the last NB mails are taken after the loop.
-template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1>
+// MIX: the three-type population (KS_MODEL_MIX3) -- every rule expressed relative to the price the
+// step starts from (generate_mix3_rel_group); the clearing warp merges the bins at the step's price
+// and price change.  Only with GROUP steps per hand-over.
+template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1, bool MIX = false>
 __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_constant__ KernelParams P) {
   constexpr bool PAIR = GROUP > 1;      // GROUP = 2 or 4 steps per pass over the agents and per hand-over
   static_assert(!PAIR || (NB == 2 * GROUP && COLS == 1 && !PACKED), "GROUP steps per hand-over: ring of 2*GROUP, literal contract");
+  static_assert(!MIX || PAIR, "MIX3 runs with GROUP steps per hand-over only");
   extern __shared__ __align__(16) int32_t book[];     // [2][L]: bid then ask; then rel[NB][P.rel_stride / 4]
   __shared__ long long s_rec[16];
   __shared__ long long s_red64[64];
@@ -144,6 +148,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
   if (clearing) {
     const LocalBook io{book, L};
     const unsigned FULL = 0xffffffffu;
+    int prevp = (int)s_rec[F_PREV];                      // MIX3: the price before `last` (momentum's side)
 #ifdef KS_DEBUG_CHECKS
     int dbg_steps = 1;                                   // steps handed over with the group being cleared
 #endif
@@ -161,14 +166,47 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
 #ifdef KS_DEBUG_CHECKS
       // (GROUP steps per hand-over: the whole group's orders are counted in its first slot's counter and
       // checked when its first step is cleared)
-      if (lane == 0 && (!PAIR || slot % GROUP == 0)) {
+      if (lane == 0 && !MIX && (!PAIR || slot % GROUP == 0)) {
         const int steps_here = PAIR ? dbg_steps : 1;
         KS_CHECK(s_dbg_count[slot] == steps_here * P.A, "orders in the histogram(s) at full[] != agents x steps handed over");
         s_dbg_count[slot] = 0;
       }
       __syncwarp();
 #endif
-      if (fuse && hi - lo < 32) {
+      if constexpr (MIX) {
+        // ---- MIX3 merge: every bin -> its clamped tick(s) in the combined book, then the usual clearing.
+        // noise: bin i of either side <-> tick last - delta + i
+        for (int i = lane; i < n; i += 32) {
+          const int va = lds32(rs + 4u * (uint32_t)i), vb = lds32(rb + 4u * (uint32_t)i);
+          const int tick = clamp_tick(t_lo + i, L);
+          if (va != 0) { sts32(rs + 4u * (uint32_t)i, 0); red32(book_saddr + 4u * (uint32_t)(tick + L), va); }
+          if (vb != 0) { sts32(rb + 4u * (uint32_t)i, 0); red32(book_saddr + 4u * (uint32_t)tick, vb); }
+        }
+        // makers: bin s0 -> bid at last - 1 - s0 AND ask at last + 1 + s0
+        for (int i = lane; i < P.maker_spread_max; i += 32) {
+          const uint32_t a = rs + P.rel_mk_off + 4u * (uint32_t)i;
+          const int v = lds32(a);
+          if (v != 0) {
+            sts32(a, 0);
+            red32(book_saddr + 4u * (uint32_t)clamp_tick(last - 1 - i, L), v);
+            red32(book_saddr + 4u * (uint32_t)(clamp_tick(last + 1 + i, L) + L), v);
+          }
+        }
+        // momentum: side = sgn(last - prev) of the step being cleared; the coin bins decide a flat price
+        const int dp = last - prevp;
+        for (int i = lane; i < P.mom_n; i += 32) {
+          const uint32_t a = rs + P.rel_mom_off + 4u * (uint32_t)i;
+          const int vall = lds32(a), vcoin = lds32(a + P.rel_mom_side);
+          if (vall != 0) sts32(a, 0);
+          if (vcoin != 0) sts32(a + P.rel_mom_side, 0);
+          const int vbuy = dp > 0 ? vall : (dp < 0 ? 0 : vcoin), vsell = vall - vbuy;
+          if (vbuy != 0) red32(book_saddr + 4u * (uint32_t)clamp_tick(last + i, L), vbuy);
+          if (vsell != 0) red32(book_saddr + 4u * (uint32_t)(clamp_tick(last - i, L) + L), vsell);
+        }
+        __syncwarp();
+        clear_active_window(io, L, max(0, min(amin, last - P.dmax)), min(L - 1, max(bmax, last + P.dmax)), P.force_generic != 0,
+                            lane, vmax, pstar, lbnd, base, wend);
+      } else if (fuse && hi - lo < 32) {
         // this lane's bins of tick lo + lane (a2, second half): read and zeroed here, added to the
         // depth inside the scan
         int ib[1], ia[1];
@@ -293,6 +331,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
             int nb, na;
             reduce_bounds(lbnd, base, wend, nb, na);
             bmax = nb; amin = na;
+            prevp = last;
             last = vmax > 0 ? pstar : last;
           }
         }
@@ -302,6 +341,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
     // ---- a1 + a2 (first half) by the generating threads tid 0 .. T-33
     const MarketUniform mu = market_uniform(P, market);
     const GenPlan<0> gplan = gen_plan<0>(PACKED ? (uint32_t)P.A >> 2 : (uint32_t)P.A, tid, T - 32);
+    const GenPlan<1> gplan3 = gen_plan<1>((uint32_t)P.A, tid, T - 32);     // MIX3: agent 3j + c has type c
     // the most agents any generating thread holds (CTA-uniform); <= 4 takes the latency path
     const uint32_t nmax = PACKED ? 99u : gplan.cls[0].n_uniform + ((uint32_t)P.A % (uint32_t)(T - 32) != 0u ? 1u : 0u);
     BookRef bref; bref.ptr = book; bref.saddr = 0;
@@ -329,8 +369,11 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
 #ifdef KS_DEBUG_CHECKS
             bref.dbg_lo = slot0; bref.dbg_hi = slot0 + GROUP * P.rel_stride; bref.dbg_count = &s_dbg_count[GROUP * pr];
 #endif
-            generate_class_rel_group<ATOM, GROUP>(P, bref, mu, ug, slot0, P.rel_stride, P.rel_side + (uint32_t)(n - 1) * 4u,
-                                                  gplan.cls[0], gplan.p0_inc, sink);
+            if constexpr (MIX)
+              generate_mix3_rel_group<GROUP>(P, bref, mu, ug, slot0, P.rel_stride, P.rel_side + (uint32_t)(n - 1) * 4u, gplan3, sink);
+            else
+              generate_class_rel_group<ATOM, GROUP>(P, bref, mu, ug, slot0, P.rel_stride, P.rel_side + (uint32_t)(n - 1) * 4u,
+                                                    gplan.cls[0], gplan.p0_inc, sink);
           } else {                                         // the run's last, partial group: step by step
             for (uint32_t g = 0; s + g < S; ++g) {
               const StepUniform u = step_uniform(P, mu, t0 + s + g);
@@ -339,7 +382,12 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
 #ifdef KS_DEBUG_CHECKS
               bref.dbg_lo = rc.rel_s; bref.dbg_hi = bref.dbg_lo + P.rel_stride; bref.dbg_count = &s_dbg_count[GROUP * pr];
 #endif
-              generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+              if constexpr (MIX) {
+                const StepUniform u1[1] = {u};
+                generate_mix3_rel_group<1>(P, bref, mu, u1, rc.rel_s, P.rel_stride, P.rel_side + (uint32_t)(n - 1) * 4u, gplan3, sink);
+              } else {
+                generate_step<0, ATOM, PACKED>(P, bref, mu, u, rc, gplan, tid == 0, sink);
+              }
             }
           }
           bar_arrive_b<1, 2>(pr, T);                       // full[pr]

@@ -84,6 +84,9 @@ struct KernelParams {
   unsigned long long* host_flags;
   uint32_t rel_stride, rel_side;                  // ks_decoupled_kernel: bytes of ONE relative histogram buffer
                                                   // (sell bins then buy bins) and of one side of it
+  uint32_t rel_mk_off, rel_mom_off, rel_mom_side; // ... MIX3: byte offsets, inside a buffer, of the maker bins (one per
+                                                  // spread) and of the momentum bins (all quantities per offset, then,
+                                                  // rel_mom_side bytes on, the quantities of the agents whose coin says buy)
 };
 
 // sticky error flags raised by the kernels (host_flags)
@@ -684,6 +687,64 @@ __device__ __forceinline__ GenPlan<MODEL> gen_plan(uint32_t count, int tid, int 
   // hide that p0_inc is a product: otherwise p0 += p0_inc is turned back into IMAD.WIDE(M0, a_step, p0)
   asm volatile("" : "+l"(g.p0_inc.inc));
   return g;
+}
+
+// The three-type population (MIX3) for the decoupled kernel, G steps per pass: every rule's order
+// is price-independent once it is expressed RELATIVE to the price the step will start from --
+//   noise     sell[o] / buy[n-1-o] as above;
+//   maker     one spread draw s0: bid at last-1-s0 AND ask at last+1+s0 with the same quantity ->
+//             ONE bin mk[s0] (the clearing warp adds it to both sides);
+//   momentum  offset o and quantity q; the side is sgn(last - prev), known only when the step is
+//             cleared -> all[o] += q, and coin[o] += q for the agents whose coin (w0's top bit)
+//             says buy, which decides only when last == prev.
+// Same draws, same integer sums as momentum_order / maker_order / noise_order (the clearing warp's
+// merge applies the clamp).  Classes as in generate_step<1>: agent 3j + c has type c.
+template <int G>
+__device__ __forceinline__ void generate_mix3_rel_group(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
+                                                        const StepUniform (&u)[G], uint32_t slot0, uint32_t stride,
+                                                        uint32_t buy_off, const GenPlan<1>& g3, int& sink) {
+  auto noise = [&](uint64_t p0) {
+    uint32_t w0[G], w1[G], w2[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) philox_from_p0<true>(P, mu, u[g], p0, w0[g], w1[g], w2[g]);
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      RuleCtx rc;
+      rc.rel_s = slot0 + (uint32_t)g * stride;
+      rc.rel_b = rc.rel_s + buy_off;
+      noise_order<4, false>(P, book, rc, w0[g], w1[g], w2[g], sink);
+    }
+  };
+  auto maker = [&](uint64_t p0) {
+    uint32_t w0, w1[G], w2;
+#pragma unroll
+    for (int g = 0; g < G; ++g) philox_from_p0<false>(P, mu, u[g], p0, w0, w1[g], w2);
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+      book_add_at<0>(book, slot0 + (uint32_t)g * stride + P.rel_mk_off + (__umulhi(w1[g], (uint32_t)P.maker_spread_max) << 2),
+                     P.maker_qty, sink);
+  };
+  auto momentum = [&](uint64_t p0) {
+    uint32_t w0[G], w1[G], w2[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) philox_from_p0<true>(P, mu, u[g], p0, w0[g], w1[g], w2[g]);
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      const int q = (int)hi32((uint64_t)w2[g] * (uint32_t)P.mom_qmax + P.q_addend);
+      const uint32_t a = slot0 + (uint32_t)g * stride + P.rel_mom_off + (__umulhi(w1[g], (uint32_t)P.mom_n) << 2);
+      book_add_at<0>(book, a, q, sink);
+      if ((int32_t)w0[g] < 0) book_add_at<0>(book, a + P.rel_mom_side, q, sink);
+    }
+  };
+  auto run = [&](const ClassPlan& pl, auto one) {
+    uint64_t p0 = pl.p0;
+#pragma unroll(4 / G)
+    for (uint32_t k = 0; k < pl.n_uniform; ++k) { one(p0); p0 = advance_p0(p0, g3.p0_inc.inc, g3.p0_inc.a_step); }
+    if (pl.extra) one(p0);
+  };
+  run(g3.cls[0], noise);
+  run(g3.cls[1], maker);
+  run(g3.cls[2], momentum);
 }
 
 template <int ATOM, int KIND, bool CLAMP>

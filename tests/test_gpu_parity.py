@@ -194,6 +194,51 @@ def test_step_pairs_give_identical_bytes(ks, oracle, group):
         assert np.array_equal(tr.cpu().numpy(), et)
 
 
+def test_mix3_decoupled_gives_identical_bytes(ks, oracle):
+    """The three-type population under the decoupled kernel (two steps per pass): noise, maker and
+    momentum orders go into histograms relative to the step's opening price -- makers one bin per
+    spread (added to both sides at the merge), momentum one bin per offset plus the coin-says-buy
+    share that decides a flat price -- and the clearing warp merges them at the step's price and
+    price change.  Forced on for several shapes, ragged agent counts (every class gets a tail),
+    odd and tiny step counts, split / launch-per-step runs, prices pinned to both grid edges (clamps
+    at the merge), flat-price starts (the coin path), other parameter values, the trace."""
+    import torch
+    opts = [(ks.KS_OPT_PIPELINE, 2)]
+    for (M, L, A, T, S, p) in [(7, 1024, 1541, 160, 45, mix3_params()), (5, 4096, 6000, 160, 31, mix3_params()),
+                               (4, 256, 100, 96, 60, mix3_params()), (3, 512, 7, 64, 20, mix3_params()),
+                               (6, 128, 900, 128, 50, dict(mix3_params(), noise_delta=20, maker_spread_max=9, mom_delta=30,
+                                                           noise_qmax=7, mom_qmax=3, maker_qty=1))]:
+        ids = np.arange(M)
+        eb, er = oracle_rows(oracle, p, L, A, 4, ids, S)
+        for kw in (dict(), dict(split=[1, 2, S - 3]), dict(split=[3, S - 8, 5]), dict(stepwise=True)):
+            b, r = _gpu(ks, M, L, A, p, 4, S, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, T)], **kw)
+            assert_rows_equal(b, r, ids, eb, er, "mix3 decoupled M=%d L=%d A=%d T=%d %r" % (M, L, A, T, kw))
+    for S in (1, 2, 3, 4, 5, 7):
+        eb, er = oracle_rows(oracle, mix3_params(), 512, 700, 8, np.arange(4), S)
+        b, r = _gpu(ks, 4, 512, 700, mix3_params(), 8, S, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, 160)])
+        assert_rows_equal(b, r, np.arange(4), eb, er, "mix3 decoupled S=%d" % S)
+    M, L, A = 4, 256, 600
+    for init in (0, L - 1, 3, L - 5):
+        q = dict(mix3_params(), init_price=init)
+        eb, er, et = oracle.run_markets_traced(q, L, A, 2, np.arange(M), 41)
+        sim = ks.KsSim(M, L, A, q, 2)
+        for o, v in opts + [(ks.KS_OPT_BLOCK_THREADS, 160)]:
+            sim.ks_set_option(o, v)
+        assert "mix3" in sim.ks_plan_string()
+        tr = torch.empty((M, 41, 2), dtype=torch.int32, device="cuda")
+        sim.ks_run_traced(41, tr)
+        b, r = sim.books_to_host(), sim.stats_to_host()
+        sim.ks_destroy()
+        assert_rows_equal(b, r, np.arange(M), eb, er, "mix3 decoupled traced init=%d" % init)
+        assert np.array_equal(tr.cpu().numpy(), et)
+    # injected crossed books (wide first window) and checkpoint attach
+    books = random_books(3, 512, seed=5, max_qty=30, fill=0.1)
+    eb0, er0 = oracle.init_state(3, 512, -1)
+    eb, er = oracle_rows(oracle, mix3_params(), 512, 800, 6, np.arange(3), 25, books=books, recs=er0)
+    b, r = _gpu(ks, 3, 512, 800, mix3_params(), 6, 25, books=books, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, 160)])
+    assert_rows_equal(b, r, np.arange(3), eb, er, "mix3 decoupled injected")
+
+
 def test_split_run_and_stepwise_ablation_are_bit_identical(ks, oracle):
     """ks_run(S1); ks_run(S2) == ks_run(S1+S2); the launch-per-step ablation (a8) == persistent."""
     c = CONFIGS["C3"]

@@ -93,8 +93,13 @@ def test_hot_loops_execute_the_multiplies_bench_reports():
     assert len(pm) == 6 and sum(l["mults"] for l in pm) / (6 * 8) == pytest.approx(bench.EXEC_MULTS_PER_EVENT["mix3_packed4"])
     # the decoupled kernel with two steps per pass: the step-independent rounds are shared (18 per event);
     # the single-step loops of the run's last, partial group keep 19
-    dp = [l for l in hot("ks_decoupled_kernelILb0ELi1ELi4ELi160ELi7ELi2EEE", 4) if l["atoms"] == 4]
+    dp = [l for l in hot("ks_decoupled_kernelILb0ELi1ELi4ELi160ELi7ELi2ELb0EEE", 4) if l["atoms"] == 4]
     assert {l["mults"] / 4 for l in dp} == {per["noise_pair"], per["noise"]}
+    # the three-type population under the decoupled kernel: noise 18, maker 13 (one bin, one atomic),
+    # momentum 18 per event in the pair loops; 19 / 14 / 19 in the single-step loops of a partial group
+    dm = hot("ks_decoupled_kernelILb0ELi1ELi4ELi160ELi7ELi2ELb1EEE", 4)
+    assert {l["mults"] / 4 for l in dm} == {per["noise_pair"], per["maker_pair"], per["momentum_pair"], per["noise"], per["maker"], per["momentum"]}
+    assert min(l["mults"] for l in dm) / 4 == per["maker_pair"]
     pa = hot("ks_persistent_kernelILi2ELi0ELb0EEE", 4)                 # model 4: three classes x no-clamp / clamp
     assert len(pa) == 6
     assert {l["mults"] / 4 for l in pa} == {per["paper_noise"], per["paper_momentum"], per["paper_maker"]}
