@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(MAXT, MINB) ks_decoupled_kernel(const __grid_c
       const int lo = max(0, min(amin, t_lo));
       const int hi = min(L - 1, max(bmax, last + delta));
       const bool inside = t_lo >= 0 && last + delta <= L - 1;   // no order of this step is clamped
-      const bool fuse = COLS == 1 && inside && !P.force_generic;
+      [[maybe_unused]] const bool fuse = COLS == 1 && inside && !P.force_generic;
       wait();                                            // every order of this step is in the histogram
 #ifdef KS_DEBUG_CHECKS
       // (GROUP steps per hand-over: the whole group's orders are counted in its first slot's counter and

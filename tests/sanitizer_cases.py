@@ -7,6 +7,7 @@ fails here too.  Sizes are tiny because the sanitizer serialises the GPU.  Cases
 Alg.1's phase structure PAPER.md:143-176, 200-212):
   c1          C1 in the automatic plan (ks_decoupled_kernel: named barriers, two-step look-ahead)
   pairs       the two-steps-per-pass decoupled kernel (groups of ring slots handed over together), odd and split S
+  mix3pairs   the three-type population under the decoupled kernel (relative maker / momentum bins)
   c5          a shrunk C5 (M=4, L=4096, A=1500, S=20, MIX3): ks_persistent_kernel, several warps, two barriers
   t32         one warp per market (T = 32): the barrier-light path C4 runs
   cluster     C = 4 CTAs per market, L = 1024: DSMEM reductions, barrier.cluster
@@ -58,6 +59,12 @@ def pairs():
     opts = [(ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_STEP_PAIRS, 2)]
     check("pairs C2 shape, odd S", 9, 256, 1024, zi_params(16, 100), 1, 41, opts=opts)
     check("pairs T=96 split", 5, 512, 1500, zi_params(32, 100), 3, 30, opts=opts + [(ks.KS_OPT_BLOCK_THREADS, 96)], split=[1, 4, 25])
+
+
+def mix3pairs():
+    opts = [(ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_BLOCK_THREADS, 160)]
+    check("mix3 decoupled, odd S", 5, 1024, 1541, mix3_params(), 4, 23, opts=opts)
+    check("mix3 decoupled at the grid edge", 3, 256, 700, dict(mix3_params(), init_price=2), 4, 20, opts=opts, split=[3, 17])
 
 
 def c5():
@@ -119,7 +126,7 @@ def attach():
     print("attach ok", flush=True)
 
 
-CASES = dict(c1=c1, pairs=pairs, c5=c5, t32=t32, cluster=cluster, paper=paper, traced=traced, packed=packed, generic=generic, attach=attach)
+CASES = dict(c1=c1, pairs=pairs, mix3pairs=mix3pairs, c5=c5, t32=t32, cluster=cluster, paper=paper, traced=traced, packed=packed, generic=generic, attach=attach)
 
 if __name__ == "__main__":
     ks.load()
