@@ -748,3 +748,45 @@ def test_debug_checks_build(ks):
                        text=True, timeout=900)
     assert p.returncode != 0 and "KS_DEBUG_CHECKS failed: orders in the book at B1" in p.stdout + p.stderr, \
         "the injected race was not caught: " + p.stdout[-1000:] + p.stderr[-1000:]
+
+
+def test_random_shapes_in_the_automatic_plan(ks, oracle):
+    """Seeded random shapes and parameters through WHATEVER plan the library picks (persistent, decoupled
+    single-step, two steps per pass, the three-type decoupled path: `ks_plan_string` is recorded in
+    the failure message), each also with the persistent kernel forced and with the decoupled kernel
+    and two steps per pass forced: always the oracle's bytes.
+    Shapes are drawn around the plan's thresholds (A = 128, 512, 1024, 1536; few or many markets; S
+    odd, tiny, split)."""
+    rng = np.random.default_rng(20261105)
+    seen = set()
+    for it in range(36):
+        mix = it % 3 == 2
+        L = int(rng.choice([64, 128, 256, 512, 1024]))
+        A = int(rng.choice([0, 1, 31, 127, 128, 300, 511, 512, 700, 1023, 1024, 1535, 1536, 2000, 4100]))
+        M = int(rng.choice([1, 2, 5, 37, 160, 700, 1300]))
+        S = int(rng.choice([1, 2, 3, 5, 8, 17, 30]))
+        if M * A * S > 6e6:
+            M = max(1, int(6e6 // max(1, A * S)))
+        if mix:
+            p = dict(mix3_params(), noise_delta=int(rng.integers(0, min(64, L // 4))), noise_qmax=int(rng.integers(1, 60)),
+                     maker_spread_max=int(rng.integers(1, 9)), maker_qty=int(rng.integers(1, 30)),
+                     mom_delta=int(rng.integers(0, 12)), mom_qmax=int(rng.integers(1, 60)))
+        else:
+            p = zi_params(int(rng.integers(0, min(40, L // 4))), int(rng.integers(1, 120)))
+        p["init_price"] = int(rng.choice([-1, 0, L - 1, L // 3]))
+        seed = int(rng.integers(0, 2**40))
+        ids = np.arange(M)
+        eb, er = oracle_rows(oracle, p, L, A, seed, ids, S)
+        split = None if S < 3 or it % 2 else [1, S - 2, 1]
+        for forced in ((), ((ks.KS_OPT_PIPELINE, 1),), ((ks.KS_OPT_PIPELINE, 2), (ks.KS_OPT_STEP_PAIRS, 2))):
+            sim = ks.KsSim(M, L, A, p, seed)
+            for o, v in forced:
+                sim.ks_set_option(o, v)
+            plan = sim.ks_plan_string()
+            seen.add(plan.split(" T=")[0] + (" pairs" if "steps_per_pass=2" in plan else "") + (" mix3" if "mix3" in plan else ""))
+            for s_ in (split or [S]):
+                sim.ks_run(s_)
+            b, r = sim.books_to_host(), sim.stats_to_host()
+            sim.ks_destroy()
+            assert_rows_equal(b, r, ids, eb, er, "random shape %d: M=%d L=%d A=%d S=%d %s plan=%s" % (it, M, L, A, S, "mix3" if mix else "zi", plan))
+    assert {"ks_decoupled_kernel", "ks_persistent_kernel", "ks_decoupled_kernel pairs", "ks_decoupled_kernel pairs mix3"} <= seen, seen
