@@ -235,6 +235,53 @@ KS_API ks_status ks_read_stats(ks_sim* s, ks_market_stats* dst, void* stream);
  * finished by then, else on the device (see ks_run, deferred errors). */
 KS_API ks_status ks_write_books(ks_sim* s, const int32_t* src, void* stream);
 
+/*
+ * Depth check of a book image for callers that have no device memory to lend and may not get any.
+ *
+ * What it computes is what the depth check behind ks_write_books / ks_attach computes: over all M
+ * markets and both sides, the largest per-side depth total sum_p book[m][side][p] -- the number the
+ * int32 overflow guard of ks_run needs (Eq.1: D and S are running sums of these entries
+ * and must stay below 2^31) -- or 0xFFFFFFFFFFFFFFFF when any entry is negative.
+ *
+ * Who needs it.  Everywhere else in this library the kernels' working memory comes from the caller:
+ * the depth check borrows a word from the 256-byte tail of d_state.  A caller who wants to vet an
+ * image BEFORE a ks_sim exists -- a checkpoint about to go to ks_attach, books about to go to
+ * ks_write_books -- has no d_state to lend, and often cannot make one: (1) a thread beside a running
+ * simulation must not call cudaMalloc / cudaFree, because both wait for the whole device, i.e. for a
+ * ks_run launch that holds the GPU for hundreds of milliseconds; (2) in a process whose framework has
+ * already claimed all of HBM for its own pool, a raw cudaMalloc simply fails; (3) code under a
+ * "no allocation after start-up" rule (a real-time loop, a plug-in whose host forbids it) may not ask.
+ * For them the working memory of this one call lives INSIDE the library: a file-scope device array of
+ * 32 + 2*KS_DEPTH_BOUND_STATIC_MAX_M 8-byte words (1 MiB + 256 B) that every GPU holds from the moment
+ * it loads the library until the process exits, whether or not this call is ever made.
+ *
+ *   d_books  DEVICE, on the CURRENT device, 4-byte aligned: int32 [M][2][L] (the layout of
+ *            ks_read_books); read only.
+ *   M, L     as ks_create (L a power of two, 32..32768); M <= KS_DEPTH_BOUND_STATIC_MAX_M.
+ *   d_out    DEVICE, on the current device, 8-byte aligned: receives the one 64-bit result.
+ * Enqueues a 8-byte clear and ONE kernel on `stream` and returns; it calls no cudaMalloc, cudaFree,
+ * cudaHostAlloc or any other allocating routine, and needs no ks_sim.
+ * Errors (nothing enqueued): KS_ERR_INVALID_ARG for a NULL / misaligned pointer or a bad M / L;
+ * KS_ERR_UNSUPPORTED, with the limit in ks_last_error(), when M > KS_DEPTH_BOUND_STATIC_MAX_M -- use
+ * ks_write_books / ks_attach on a real d_state for larger images, or check the image in slices of
+ * markets and take the maximum; KS_ERR_CUDA when a CUDA call fails.
+ *
+ * First call on each device.  The library looks up the device address of its array once per device
+ * (cudaGetSymbolAddress, with that device current) and remembers it.  That look-up makes the CUDA
+ * runtime load this library's device code on that GPU if it has not yet done so, so make the first
+ * call on every device during start-up, before any stream capture is begun.
+ *
+ * One array, shared by everybody.  All calls on a device -- from any thread, on any stream -- use the
+ * same words, and the array keeps whatever the previous call left in it.  The call clears the one word
+ * that has to start at zero (a ticket counter) itself, on `stream`, and every other word it reads has
+ * been written earlier in the same call, so back-to-back calls on ONE stream are safe.  Two calls that
+ * can overlap on the GPU (different streams with no ordering between them, or two host threads each
+ * on their own stream) race on those words and may both return garbage: order them yourself.
+ */
+#define KS_DEPTH_BOUND_STATIC_MAX_M 65536
+KS_API ks_status ks_depth_bound_static(const int32_t* d_books, int32_t M, int32_t L, uint64_t* d_out,
+                                       void* stream);
+
 /* Tuning / ablation switches; none of them changes a single output byte.  Returns
  * KS_ERR_INVALID_ARG for an unknown option or value. */
 typedef enum {

@@ -28,7 +28,8 @@ DERIVED_FIELDS = ("mean_px", "vwap", "vol_per_step", "ret_mean", "ret_var", "exc
 # every symbol the two headers declare (tests check that each library exports exactly these)
 EXPORTS = ("ks_state_bytes", "ks_create", "ks_create_ex", "ks_attach", "ks_run", "ks_read_books", "ks_read_stats",
            "ks_write_books", "ks_run_traced", "ks_trace_stats", "ks_set_option", "ks_derive_stats", "ks_destroy", "ks_last_error",
-           "ks_launch_count", "ks_error_state", "ks_plan_string")
+           "ks_launch_count", "ks_error_state", "ks_plan_string", "ks_depth_bound_static")
+KS_DEPTH_BOUND_STATIC_MAX_M = 65536
 BENCH_EXPORTS = ("ks_run_stepwise", "ks_bench_smem_atomic", "ks_bench_generate_only", "ks_bench_int_pipe")
 
 
@@ -100,6 +101,7 @@ def load():
     L.ks_destroy.argtypes = [vp]; L.ks_destroy.restype = None
     L.ks_last_error.argtypes = []; L.ks_last_error.restype = C.c_char_p
     L.ks_launch_count.argtypes = []; L.ks_launch_count.restype = i64
+    L.ks_depth_bound_static.argtypes = [vp, i32, i32, vp, vp]; L.ks_depth_bound_static.restype = i32
     _lib = L
     return L
 
@@ -243,6 +245,15 @@ def ks_trace_stats(d_trace, M: int, S: int, K: int, d_out=None, stream=None):
     assert d_trace.is_cuda and d_out.is_cuda and d_out.numel() >= M * (4 + 2 * K)
     _check(load().ks_trace_stats(d_trace.data_ptr(), M, S, K, d_out.data_ptr(), _stream_ptr(stream)))
     return d_out
+
+
+def ks_depth_bound_static(d_books, M: int, L: int, d_out, stream=None):
+    """Largest per-side depth total of the book image d_books (CUDA int32 [M][2][L]) -> d_out (CUDA
+    int64 tensor, one element, read it as uint64; all ones = a negative entry).  For callers that may
+    not allocate device memory: the kernel's working memory is an array inside the library, so both
+    tensors are the caller's and nothing is allocated here or in the library (include/kineticsim.h
+    has the limit M <= KS_DEPTH_BOUND_STATIC_MAX_M and the rule that overlapping calls race)."""
+    _check(load().ks_depth_bound_static(_ptr_of(d_books), M, L, _ptr_of(d_out), _stream_ptr(stream)))
 
 
 def ks_bench_smem_atomic(mode, delta, L, threads=256, ctas_per_sm=8, iters=2000, warmup=2, reps=5, stream=None):

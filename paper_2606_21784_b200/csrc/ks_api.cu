@@ -673,3 +673,113 @@ void ks_derive_stats(const ks_market_stats* rec, ks_derived_stats* out, int64_t 
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------
+// ks_depth_bound_static -- the depth check for callers who cannot allocate (include/kineticsim.h says
+// who they are and why).  Every other kernel of this library works in memory the caller handed over;
+// this one works in an array that is part of the library image itself, so the call needs neither a
+// ks_sim nor a d_state and never asks the driver for memory.
+//
+// Layout of the array (8-byte words): [0] ticket counter, [1..31] unused (keeps the totals on their own
+// 256-byte line), [32 + b] depth total of side b = 2*market + side.  It costs 1 MiB + 256 B of every
+// GPU that loads the library, until the process exits.
+//
+// g_static_scratch below is two different things.  Inside device code the name IS the array.  In
+// host code the same name is only a handle the runtime recognises -- it is not a device address, and a
+// kernel (or cudaMemsetAsync) handed `g_static_scratch` from the host would touch some unrelated host
+// location or fault.  The host therefore asks cudaGetSymbolAddress for the real address, once per
+// device and with that device current (each GPU has its own copy at its own address), and passes that.
+// ---------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned long long g_static_scratch[32 + 2 * KS_DEPTH_BOUND_STATIC_MAX_M];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+// device address of g_static_scratch per device ordinal; 0 = not looked up yet.  Two threads that
+// race on the first call both store the same value.
+std::atomic<unsigned long long*> g_static_addr[kStaticMaxDevices];
+
+// One block per (market, side), as ks_depth_bound_kernel; instead of an atomicMax into a word of the
+// caller's d_state, each block leaves its total in the library's array and takes a ticket, and the
+// block that draws the last ticket reduces all totals into *out.
+//   scratch[0] must be 0 at launch (the host clears it on the same stream); scratch[32 + b] is written
+//   by block b before it is read by the last block, so stale totals of an earlier, larger call are
+//   never looked at.
+__global__ void ks_depth_bound_static_kernel(const int32_t* __restrict__ books, int L, unsigned long long* scratch,
+                                             unsigned long long* out) {
+  const int32_t* side = books + (size_t)blockIdx.x * (size_t)L;      // grid = 2*M sides
+  long long sum = 0; int neg = 0;
+  for (int i = threadIdx.x; i < L; i += blockDim.x) { const int v = side[i]; sum += v; neg |= (v < 0); }
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  neg = __any_sync(0xffffffffu, neg);
+  __shared__ long long s_sum[32];
+  __shared__ int s_neg, s_last;
+  if (threadIdx.x == 0) { s_neg = 0; s_last = 0; }
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) { s_sum[threadIdx.x >> 5] = sum; if (neg) s_neg = 1; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    long long tot = 0;
+    for (int w = 0; w < (int)((blockDim.x + 31) >> 5); ++w) tot += s_sum[w];
+    volatile unsigned long long* totals = scratch + 32;
+    totals[blockIdx.x] = s_neg ? 0xffffffffffffffffull : (unsigned long long)tot;
+    __threadfence();                                                 // total visible before the ticket
+    const unsigned long long ticket = atomicAdd(&scratch[0], 1ull);
+    s_last = ticket == (unsigned long long)gridDim.x - 1ull;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();                                                   // every other block's total is visible now
+  const volatile unsigned long long* totals = scratch + 32;
+  unsigned long long best = 0;
+  for (unsigned b = threadIdx.x; b < gridDim.x; b += blockDim.x) { const unsigned long long v = totals[b]; best = v > best ? v : best; }
+  for (int d = 16; d > 0; d >>= 1) { const unsigned long long o = __shfl_xor_sync(0xffffffffu, best, d); best = o > best ? o : best; }
+  __shared__ unsigned long long s_best[32];
+  if ((threadIdx.x & 31) == 0) s_best[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)((blockDim.x + 31) >> 5); ++w) best = s_best[w] > best ? s_best[w] : best;
+    *out = best;
+  }
+}
+
+// Device address of the library's array on the CURRENT device; looked up on the first call per device.
+ks_status static_scratch_here(unsigned long long** out) {
+  int dev = -1;
+  KS_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) { set_err("ks_depth_bound_static: device ordinal beyond %s", "63"); return KS_ERR_UNSUPPORTED; }
+  unsigned long long* ptr = g_static_addr[dev].load(std::memory_order_acquire);
+  if (!ptr) {
+    KS_CUDA(cudaGetSymbolAddress((void**)&ptr, g_static_scratch));
+    if (!ptr) { set_err("ks_depth_bound_static: cudaGetSymbolAddress returned a NULL address"); return KS_ERR_CUDA; }
+    g_static_addr[dev].store(ptr, std::memory_order_release);
+  }
+  *out = ptr;
+  return KS_OK;
+}
+
+}  // namespace
+
+extern "C" ks_status ks_depth_bound_static(const int32_t* d_books, int32_t M, int32_t L, uint64_t* d_out, void* stream) {
+  if (!d_books || !d_out) { set_err("ks_depth_bound_static: NULL argument"); return KS_ERR_INVALID_ARG; }
+  if ((reinterpret_cast<uintptr_t>(d_books) & 3) != 0 || (reinterpret_cast<uintptr_t>(d_out) & 7) != 0) {
+    set_err("ks_depth_bound_static: d_books must be 4-byte and d_out 8-byte aligned"); return KS_ERR_INVALID_ARG;
+  }
+  if (!shape_ok(M, L)) { set_err("ks_depth_bound_static: need M >= 1 and L a power of two in 32..32768"); return KS_ERR_INVALID_ARG; }
+  if (M > KS_DEPTH_BOUND_STATIC_MAX_M) {
+    snprintf(g_err, sizeof(g_err),
+             "ks_depth_bound_static: M = %d exceeds KS_DEPTH_BOUND_STATIC_MAX_M = %d (the library's built-in scratch holds one "
+             "word per market side); check the image in slices of markets, or use ks_write_books / ks_attach on a d_state",
+             (int)M, (int)KS_DEPTH_BOUND_STATIC_MAX_M);
+    return KS_ERR_UNSUPPORTED;
+  }
+  unsigned long long* scratch = nullptr;
+  const ks_status r = static_scratch_here(&scratch);
+  if (r != KS_OK) return r;
+  cudaStream_t st = (cudaStream_t)stream;
+  KS_CUDA(cudaMemsetAsync(scratch, 0, sizeof(unsigned long long), st));            // the ticket counter starts at zero
+  ks_depth_bound_static_kernel<<<2 * M, 128, 0, st>>>(d_books, L, scratch, reinterpret_cast<unsigned long long*>(d_out));
+  KS_CUDA(cudaGetLastError());
+  g_launches++;
+  return KS_OK;
+}
