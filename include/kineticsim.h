@@ -168,7 +168,10 @@ KS_API ks_status ks_create_ex(ks_sim** out, int32_t M, int32_t L, int32_t A, con
  * leaves the bytes of one uninterrupted ks_run(S1+S2).  Unlike the other calls this one
  * SYNCHRONISES `stream`: it reads the step counter and the largest per-side depth back from the
  * device for the overflow guards of ks_run.  Arguments and errors as ks_create_ex, plus
- * KS_ERR_INVALID_ARG when d_state holds a negative depth or an impossible step counter.
+ * KS_ERR_INVALID_ARG when d_state holds a negative depth, or a record this library cannot have
+ * written: EVERY market's record is checked on the device (step counter f[0] >= 0, last price f[12]
+ * on the grid, f[13] on the grid -- or a valid doubled mid for KS_MODEL_PAPER); the guards of ks_run
+ * continue from the LARGEST step counter found.
  */
 KS_API ks_status ks_attach(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_agent_params* p,
                            uint64_t seed, uint32_t market_base, void* d_state, void* stream);
@@ -178,9 +181,12 @@ KS_API ks_status ks_attach(ks_sim** out, int32_t M, int32_t L, int32_t A, const 
  * continuing from the state in d_state: the Philox step index is steps_done + i, so
  * ks_run(S1); ks_run(S2) leaves the same bytes as ks_run(S1+S2).  S = 0 is a no-op.
  * KS_ERR_OVERFLOW (nothing enqueued) when (steps_done+S) x per-step per-side inflow bound, plus
- * the depth injected by ks_write_books, could reach 2^31 (int32 book), or steps_done+S >= 2^32.
+ * the depth injected by ks_write_books, could reach 2^31 (int32 book), or steps_done+S >= 2^32 - 8
+ * (the kernels count steps in 32 bits and look up to 8 steps ahead).
  * Deferred errors.  (1) If the depth check of a preceding ks_write_books has not finished yet, the
- * call does NOT wait for it: the kernel reads the check's result on the device and, when the bound
+ * host does NOT wait for it: the launch is ordered after the check on the device (an event wait on
+ * `stream`, so `stream` may differ from the one ks_write_books used), the kernel reads the check's
+ * result there and, when the bound
  * is violated (or a negative depth was stored), the whole launch returns without changing a byte
  * of d_state.  (2) The int64 sums of r^3 and r^4 (f[8], f[9]) can only overflow on wide grids
  * after very large price moves ((L-1)^4 x steps >= 2^63 at the earliest); the kernel detects the
@@ -289,24 +295,32 @@ typedef enum {
   KS_OPT_ATOMIC_MODE = 1,   /* 0 = plain shared-memory atomicAdd, 1 = warp-aggregated (__match_any_sync) */
   KS_OPT_CLEAR_PATH = 2,    /* 0 = automatic (windowed one-warp scan), 1 = force the chunked general scan */
   KS_OPT_PIPELINE = 4,      /* the decoupled kernel (generating warps fill a ring of price-independent relative order
-                               histograms up to KS_OPT_RING_DEPTH steps ahead; one clearing warp per market, holding no
-                               agents, merges them at the step's price and clears): 0 = automatic (when the grid
-                               underfills the GPU, i.e. step latency is what counts, or when an SM holds only a few
-                               markets, M <= 16 x #SMs), 1 = never, 2 = whenever legal (KS_MODEL_ZI /
-                               KS_MODEL_ZI_PACKED4, plain atomics, >= 64 threads, L <= 16384, book + the histogram
-                               ring fit shared memory)                                                        */
+                               histograms up to KS_OPT_RING_DEPTH steps ahead; the LAST warp of the CTA is the market's
+                               clearing warp, holds no agents, merges them at the step's price and clears):
+                               0 = automatic (when the grid underfills the GPU, i.e. step latency is what counts, or
+                               when an SM holds only a few markets, M <= 16 x #SMs; and always as part of the
+                               automatic two-steps-per-pass plan, see KS_OPT_STEP_PAIRS), 1 = never, 2 = whenever
+                               legal.  Legal for KS_MODEL_ZI / KS_MODEL_ZI_PACKED4 with plain atomics, >= 64 threads,
+                               L <= 16384 and book + histogram ring fitting shared memory; and for KS_MODEL_MIX3
+                               (literal draws) in its two-steps-per-pass form only: plain atomics, maker_spread_max
+                               <= 64, mom_delta < 64, 64 <= threads <= 160, KS_OPT_REL_COLUMNS 0, KS_OPT_RING_DEPTH 0 */
   KS_OPT_REL_COLUMNS = 5,   /* decoupled kernel only: 0 = one int32 per histogram bin, 1 = 32 lane columns per
                                bin (column = lane = bank: a warp's atomics never conflict) -- the
-                               aggregation ablation of north_star (3)                                       */
+                               aggregation ablation of north_star (3); two-deep ring, one step per pass         */
   KS_OPT_RING_DEPTH = 6,    /* decoupled kernel only: how many steps the generating warps may run ahead of the
-                               clearing warp = number of relative histograms in the ring: 0 = automatic (4; 2 with
-                               KS_OPT_REL_COLUMNS), 2 or 4 (ablation: the two-deep ring leaves both sides waiting
-                               for each other's hand-over)                                                    */
-  KS_OPT_STEP_PAIRS = 7,    /* decoupled kernel, KS_MODEL_ZI, <= 160 threads: the generating warps make TWO steps per
-                               pass over their agents (the step-independent Philox rounds and the counter add are
-                               shared: 18 multiplies per event instead of 19) and hand them over together (ring
-                               of 4, the clearing warp keeps the record): 0 = automatic (>= 4 events per
-                               generating thread and the grid not underfilled), 1 = never, 2 = whenever legal   */
+                               clearing warp = number of relative histograms in the ring: 0 = automatic (4 when the
+                               step latency counts, M <= 2 x #SMs; 2 when throughput does, M > 2 x #SMs, or with
+                               KS_OPT_REL_COLUMNS; always 4 under two steps per pass), 2 or 4 = forced (a forced
+                               value rules out two steps per pass)                                            */
+  KS_OPT_STEP_PAIRS = 7,    /* decoupled kernel, 64..160 threads: the generating warps make TWO steps per pass over
+                               their agents (the step-independent Philox rounds and the counter add are shared: 18
+                               multiplies per event instead of 19) and hand them over together (ring of 4, the
+                               clearing warp keeps the record).  KS_MODEL_ZI (literal draws), and KS_MODEL_MIX3 with
+                               maker_spread_max <= 64 and mom_delta < 64 (every rule binned relative to the step's
+                               opening price and price change).  0 = automatic (ZI: >= 4 events per generating
+                               thread, i.e. A >= 1024, or A >= 512 when M <= 16 x #SMs; MIX3: A >= 1536 and four CTAs
+                               fitting an SM; the grid not underfilled; no forced block size), 1 = never,
+                               2 = whenever legal                                                              */
   KS_OPT_CLUSTER_SIZE = 3   /* CTAs per market: 0 = automatic (1 while the book fits one CTA's shared memory,
                                i.e. L <= 16384; else L/16384), 1, or 2/4/8 = thread-block cluster with the
                                book split across the CTAs' shared memory (DSMEM); needs L/value >= 32 and

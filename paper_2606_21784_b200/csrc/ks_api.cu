@@ -203,13 +203,25 @@ ks_status create_common(ks_sim** out, int32_t M, int32_t L, int32_t A, const ks_
   } else {
     // adopt the checkpoint: the step counter (for the overflow guards) and the resting depth bound
     // come back from the device; this call synchronises `stream`
+    // scratch words [1] = largest step counter over the markets, [2] = 1 when some record cannot be
+    // one this library wrote (negative step counter, price off the grid)
+    unsigned long long chk[2] = {0, 0};
     long long steps0 = 0;
     ks_status r = enqueue_depth_check(s, st);
     if (r == KS_OK) {
-      e = cudaMemcpyAsync(&steps0, recs_ptr(s), sizeof(long long), cudaMemcpyDeviceToHost, st);
+      e = cudaMemsetAsync(scratch_ptr(s) + 1, 0, 2 * sizeof(unsigned long long), st);
+      if (e == cudaSuccess) {
+        ks::ks_attach_check_kernel<<<(M + 255) / 256, 256, 0, st>>>(recs_ptr(s), M, L, p->model == KS_MODEL_PAPER ? 2 * L - 1 : L,
+                                                                    scratch_ptr(s) + 1);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) g_launches++;
+      }
+      if (e == cudaSuccess) e = cudaMemcpyAsync(chk, scratch_ptr(s) + 1, sizeof(chk), cudaMemcpyDeviceToHost, st);
       if (e == cudaSuccess) e = cudaStreamSynchronize(st);
       if (e != cudaSuccess) { set_err("%s: %s", who, cudaGetErrorString(e)); r = KS_ERR_CUDA; }
+      steps0 = (long long)chk[0];
     }
+    if (r == KS_OK && chk[1] != 0) { set_err("%s: d_state does not hold valid records (a negative step counter or a price off the grid)", who); r = KS_ERR_INVALID_ARG; }
     if (r == KS_OK && (steps0 < 0 || steps0 >= 4294967296LL)) { set_err("%s: d_state does not hold a valid record (step counter)", who); r = KS_ERR_INVALID_ARG; }
     if (r == KS_OK && s->h_words[0] == 0xffffffffffffffffull) { set_err("%s: d_state holds a negative depth", who); r = KS_ERR_INVALID_ARG; }
     if (r != KS_OK) { free_sim(s); return r; }
@@ -415,12 +427,34 @@ static LaunchPlan plan_launch(const ks_sim* s) {
   return pl;
 }
 
+// cudaFuncSetAttribute is host work that used to precede every launch (1000 times in ks_run_stepwise).
+// MaxDynamicSharedMemorySize is only an upper limit, so it is raised monotonically: one cache per
+// kernel instantiation and device holding the largest value set so far (+1; 0 = never set).
+struct SmemAttrCache { std::atomic<long long> set_plus1[64]; };
+
+template <class K>
+static cudaError_t ensure_smem_attr(K kern, SmemAttrCache& c, size_t smem) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool cached = dev >= 0 && dev < 64;
+  if (cached && c.set_plus1[dev].load(std::memory_order_acquire) >= (long long)smem + 1) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e != cudaSuccess) return e;
+  if (cached) {
+    long long cur = c.set_plus1[dev].load(std::memory_order_relaxed);
+    while (cur < (long long)smem + 1 && !c.set_plus1[dev].compare_exchange_weak(cur, (long long)smem + 1)) {}
+  }
+  return cudaSuccess;
+}
+
 template <int MODEL, int ATOM, bool PACKED>
 static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
   auto kern = ks::ks_persistent_kernel<MODEL, ATOM, PACKED>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  static SmemAttrCache cache;
+  cudaError_t e = ensure_smem_attr(kern, cache, smem);
   if (e != cudaSuccess) return e;
   kern<<<P.M, T, smem, st>>>(P);
   return cudaGetLastError();
@@ -429,9 +463,8 @@ static cudaError_t launch_persistent(const ks::KernelParams& P, int T, size_t sm
 template <bool PACKED, int COLS, int NB, int MAXT, int MINB, int GROUP = 1, bool MIX = false>
 static cudaError_t launch_decoupled_as(const ks::KernelParams& P, int T, size_t smem, cudaStream_t st) {
   auto kern = ks::ks_decoupled_kernel<PACKED, COLS, NB, MAXT, MINB, GROUP, MIX>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  static SmemAttrCache cache;
+  cudaError_t e = ensure_smem_attr(kern, cache, smem);
   if (e != cudaSuccess) return e;
   kern<<<P.M, T, smem, st>>>(P);
   return cudaGetLastError();
@@ -502,7 +535,9 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
   const long double inflow = total_steps * (long double)s->inflow_per_step;
   const long double known_resting = s->bound_pending ? 0.0L : (long double)s->resting_bound;
   if (known_resting + inflow >= 2147483648.0L) { set_err("%s: per-side depth could reach 2^31", who); return KS_ERR_OVERFLOW; }
-  if (total_steps >= 4294967296.0L) { set_err("%s: the step counter would pass 2^32", who); return KS_ERR_OVERFLOW; }
+  // 8 steps of head-room: the decoupled kernel's 32-bit loop counters advance by up to 8 steps (ring
+  // depth, or twice the steps per pass) and compare `s + stride < S`
+  if (total_steps + 8.0L >= 4294967296.0L) { set_err("%s: the step counter would pass 2^32 - 8", who); return KS_ERR_OVERFLOW; }
 
   ks::KernelParams P;
   memset(&P, 0, sizeof(P));
@@ -538,6 +573,9 @@ static ks_status run_impl(ks_sim* s, int64_t S, void* stream, const char* who, i
 
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e;
+  // the kernel reads the pending check's word on the device: order it after the check even when the
+  // caller runs on another stream than ks_write_books did (asynchronous, no host wait)
+  if (s->bound_pending) KS_CUDA(cudaStreamWaitEvent(st, s->bound_event, 0));
   const bool paper = s->p.model == KS_MODEL_PAPER;
   const bool mix = !paper && (s->p.model & 1) == KS_MODEL_MIX3;
   const bool packed = !paper && s->p.model >= KS_MODEL_ZI_PACKED4;

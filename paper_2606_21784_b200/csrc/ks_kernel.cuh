@@ -432,4 +432,26 @@ __global__ void ks_depth_bound_kernel(const int32_t* books, int L, unsigned long
   }
 }
 
+// ks_attach record check: out[0] = max over markets of the step counter f[0] (atomicMax), out[1] = 1
+// when some record could not have been written by this library: f[0] < 0, last (f[12]) outside
+// [0, L), or f[13] outside [0, prev_limit) -- prev_limit = L for a previous price, 2L-1 for the
+// doubled mid of KS_MODEL_PAPER.  Such prices would reach the rules' tick arithmetic unclamped.
+__global__ void ks_attach_check_kernel(const long long* recs, int M, int L, int prev_limit, unsigned long long* out) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  long long steps = 0; int bad = 0;
+  if (m < M) {
+    const long long* r = recs + (size_t)m * 16;
+    steps = r[F_STEPS];
+    const long long last = r[F_LAST], prev = r[F_PREV];
+    bad = steps < 0 || last < 0 || last >= L || prev < 0 || prev >= prev_limit;
+    if (steps < 0) steps = 0;
+  }
+  for (int d = 16; d > 0; d >>= 1) { const long long o = __shfl_xor_sync(0xffffffffu, steps, d); steps = o > steps ? o : steps; }
+  bad = __any_sync(0xffffffffu, bad);
+  if ((threadIdx.x & 31) == 0) {
+    atomicMax(out, (unsigned long long)steps);
+    if (bad) out[1] = 1ull;
+  }
+}
+
 }  // namespace ks

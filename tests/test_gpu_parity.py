@@ -105,7 +105,8 @@ def test_decoupled_kernel_gives_identical_bytes(ks, oracle):
     import torch
     L, seed, S = 128, 2, 150
     p = zi_params(8, 10)
-    # M > #warps makes every warp index the clearing warp of some market (clearing warp = market mod #warps)
+    # (pipe = 1, ks_persistent_kernel: clearing warp = market mod #warps, so M > #warps makes every warp index a
+    # clearing warp; ks_decoupled_kernel's clearing warp is always the CTA's last warp)
     for M, A, T in [(5, 512, 512), (5, 500, 256), (3, 97, 64), (4, 33, 96), (2, 0, 128), (3, 1900, 512), (2, 1984, 1024),
                     (7, 1024, 160), (6, 1024, 128), (9, 1000, 96), (5, 3000, 224), (11, 4096, 1024), (3, 4096, 288)]:
         ids = np.arange(M)
@@ -464,6 +465,86 @@ def test_deferred_depth_check_refuses_the_run_on_the_device(ks, oracle):
         rec = sim.state[M * 8 * L: M * (8 * L + 128)].view(torch.int64).view(M, 16).cpu().numpy()
         assert np.array_equal(raw, books) and (rec[:, 0] == 0).all()     # not a byte of the run happened
         sim.ks_destroy()
+
+
+def test_attach_checks_every_markets_record(ks):
+    """ks_attach adopts per-market step counters and prices: a record that this library cannot have
+    written -- in ANY market, not only market 0 -- is refused (a price off the grid would reach the
+    rules' tick arithmetic unclamped), and the run guards continue from the largest step counter."""
+    import torch
+    M, L, A, seed, p = 6, 64, 100, 3, zi_params(8, 10)
+    sim = ks.KsSim(M, L, A, p, seed)
+    sim.ks_run(20)
+    torch.cuda.synchronize()
+    good = sim.state.clone()
+    sim.ks_destroy()
+    rec0 = M * 8 * L
+    for m, field, value in ((4, 12, L), (5, 12, -1), (3, 13, L + 5), (2, 13, -2), (1, 0, -7)):
+        state = good.clone()
+        state[rec0: rec0 + M * 128].view(torch.int64).view(M, 16)[m, field] = value
+        with pytest.raises(ks.KsError) as e:
+            ks.KsSim(M, L, A, p, seed, state=state, attach=True)
+        assert e.value.status == ks.KS_ERR_INVALID_ARG, (m, field, value)
+    # a market further along than market 0: the step guard counts from the maximum
+    state = good.clone()
+    state[rec0: rec0 + M * 128].view(torch.int64).view(M, 16)[4, 0] = 2 ** 32 - 100
+    sim = ks.KsSim(M, L, A, p, seed, state=state, attach=True)
+    with pytest.raises(ks.KsError) as e:
+        sim.ks_run(95)
+    assert e.value.status == ks.KS_ERR_OVERFLOW
+    sim.ks_destroy()
+    # KS_MODEL_PAPER keeps the doubled mid in f[13]: up to 2(L-1) is legal there
+    pp = paper_params(100, 0.15, 0.15)
+    sim = ks.KsSim(M, L, 100, pp, seed)
+    sim.ks_run(5)
+    torch.cuda.synchronize()
+    state = sim.state.clone()
+    sim.ks_destroy()
+    state[rec0: rec0 + M * 128].view(torch.int64).view(M, 16)[2, 13] = 2 * (L - 1)
+    ks.KsSim(M, L, 100, pp, seed, state=state, attach=True).ks_destroy()
+    state[rec0: rec0 + M * 128].view(torch.int64).view(M, 16)[2, 13] = 2 * L - 1
+    with pytest.raises(ks.KsError):
+        ks.KsSim(M, L, 100, pp, seed, state=state, attach=True)
+
+
+def test_step_counter_guard_leaves_headroom_for_the_kernels_lookahead(ks):
+    """The kernels count steps in 32 bits and the decoupled kernel compares `s + stride < S` with a
+    stride of up to 8: ks_run refuses a run that would bring the counter within 8 of 2^32."""
+    M, L, A, seed, p = 2, 64, 0, 1, zi_params(8, 10)
+    sim = ks.KsSim(M, L, A, p, seed)
+    for S in (2 ** 32 - 8, 2 ** 32 - 1, 2 ** 32):
+        with pytest.raises(ks.KsError) as e:
+            sim.ks_run(S)
+        assert e.value.status == ks.KS_ERR_OVERFLOW
+    sim.ks_destroy()
+
+
+def test_run_on_another_stream_than_write_books(ks, oracle):
+    """ks_run reads the pending depth check's word on the device; the library orders the launch after
+    the check with an event wait, so the run may be enqueued on a different stream than
+    ks_write_books (the books themselves are the caller's to order: done here with an event)."""
+    import torch
+    M, L, A, seed, S, p = 40, 256, 300, 6, 25, zi_params(16, 50)
+    books = random_books(M, L, seed=9, max_qty=30, fill=0.4)
+    _, er0 = oracle.init_state(M, L, -1)
+    eb, er = oracle_rows(oracle, p, L, A, seed, np.arange(M), S, books=books, recs=er0)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    d_books = torch.from_numpy(books).cuda()
+    torch.cuda.synchronize()
+    sim = ks.KsSim(M, L, A, p, seed, stream=s1)
+    filler = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+    with torch.cuda.stream(s1):
+        for _ in range(8):
+            filler.fill_(1)                             # keeps s1 busy so that the check is still pending
+    sim.ks_write_books(d_books, stream=s1)
+    ev = torch.cuda.Event()
+    ev.record(s1)
+    s2.wait_event(ev)
+    sim.ks_run(S, stream=s2)
+    s2.synchronize()
+    b, r = sim.books_to_host(), sim.stats_to_host()
+    sim.ks_destroy()
+    assert_rows_equal(b, r, np.arange(M), eb, er, "run on another stream")
 
 
 # ------------------------------------------------------------------ PACKED4 draw contract
