@@ -293,6 +293,66 @@ def time_case(ks, torch, dev, c, *, reps=3, mode="persistent", S=None, M=None, o
             "plan": plan}
 
 
+def time_state_io(ks, torch, dev, c, hbm_peak_gbs, reps=5):
+    """a0 + a7 alone (north_star: "HBM peak for the book load and store"; Eq.6): the
+    config's M x L books resident in HBM (ks_write_books of random books, so the load is not
+    skipped), no agents, ONE step -- the launch loads every book and record and stores them again.
+    Bytes = 2 * M * (8L + 128).  Median device time of `reps` launches, CUDA events."""
+    from paper_2606_21784_b200.workloads import random_books
+    M, L = c.M, c.L
+    st = torch.empty(ks.ks_state_bytes(M, L), dtype=torch.uint8, device=dev)
+    one = torch.from_numpy(random_books(64, L, seed=11, max_qty=50, fill=0.3)).to(dev)
+    books = one.repeat((M + 63) // 64, 1, 1)[:M].contiguous()
+    ts, plan = [], ""
+    for i in range(1 + reps):
+        sim = ks.KsSim(M, L, 0, c.params, c.seed, state=st)
+        try:
+            sim.ks_write_books(books)
+            torch.cuda.synchronize()
+            plan = sim.ks_plan_string()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); sim.ks_run(1); b.record()
+            torch.cuda.synchronize()
+            sim.ks_error_state()
+            ts.append(a.elapsed_time(b))
+        finally:
+            sim.ks_destroy()
+    ms = float(np.median(ts[1:]))
+    nbytes = 2 * M * (8 * L + 128)
+    return {"ms": ms, "bytes": nbytes, "GBps": nbytes / (ms * 1e-3) / 1e9, "frac_of_hbm": nbytes / (ms * 1e-3) / 1e9 / hbm_peak_gbs,
+            "plan": plan}
+
+
+def time_e2e_small(ks, torch, dev, c, reps=20):
+    """End to end through the C ABI with HOST buffers for a latency-regime config: opening books H2D
+    from pinned memory, ks_run(S), books + records D2H into pinned memory.  Host clock around the
+    calls and the final synchronize (what a caller waits), CUDA events beside it; medians."""
+    M, L = c.M, c.L
+    st = torch.empty(ks.ks_state_bytes(M, L), dtype=torch.uint8, device=dev)
+    h_open = torch.zeros((M, 2, L), dtype=torch.int32).pin_memory()
+    h_books = torch.empty((M, 2, L), dtype=torch.int32).pin_memory()
+    h_recs = torch.empty((M, 16), dtype=torch.int64).pin_memory()
+    host_ms, dev_ms = [], []
+    for i in range(3 + reps):
+        sim = ks.KsSim(M, L, c.A, c.params, c.seed, state=st)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        a.record()
+        sim.ks_write_books(h_open); sim.ks_run(c.S); sim.ks_read_books(h_books); sim.ks_read_stats(h_recs)
+        b.record()
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        sim.ks_destroy()
+        if i >= 3:
+            host_ms.append((t1 - t0) * 1e3)
+            dev_ms.append(a.elapsed_time(b))
+    hm, dm = float(np.median(host_ms)), float(np.median(dev_ms))
+    ev = float(M) * c.A * c.S
+    return {"host_ms": hm, "device_ms": dm, "events_per_s_host_clock": ev / (hm * 1e-3), "us_per_step_host_clock": hm * 1e3 / c.S,
+            "h2d_bytes": int(h_open.numel() * 4), "d2h_bytes": int(h_books.numel() * 4 + h_recs.numel() * 8)}
+
+
 def run_case(args):
     """--case: ONE timed run of a named case (after one warm-up), a small JSON line."""
     import torch
@@ -545,27 +605,25 @@ def main():
     achieved = ALG_MULTS_PER_EVENT[model] * kev / 1e12
     exec_per_event = exec_mults(cfg.params, plans[-1])
     executed = exec_per_event * kev / 1e12
-    roofline = {"bound": "alu", "kernel": plans[-1], "achieved": achieved, "peak": peak,
-                "unit": "T 32x32->64-bit integer multiplies/s", "frac": achieved / peak,
-                "frac_executed": executed / peak,
+    roofline = {"bound": "alu", "kernel": plans[-1], "achieved": executed, "peak": peak,
+                "unit": "T 32x32->64-bit integer multiplies/s", "frac": executed / peak,
+                "achieved_algorithmic": achieved, "frac_algorithmic": achieved / peak,
                 "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(cfg.name if args.rng == "literal" else cfg.name + "_packed4"),
                 "peak_source": ("measured in this process: ks_bench_int_pipe(5), a pure mul.wide.u32 stream "
                                 "(include/kineticsim_bench.h)") if mulwide_peak else
                                "derived (microbenchmarks skipped): see peak_derived_source",
-                "peak_derived": peak_derived, "frac_of_derived_peak": achieved / peak_derived,
-                "frac_executed_of_derived_peak": executed / peak_derived,
+                "peak_derived": peak_derived, "frac_of_derived_peak": executed / peak_derived,
+                "frac_algorithmic_of_derived_peak": achieved / peak_derived,
                 "peak_derived_source": "%d SMs x 4 SMSPs x 8 lanes/clk (IMAD.WIDE = 2 passes of the 16-lane fmaheavy pipe) x %.0f MHz (%s)"
                                        % (sms, sm_max_mhz, "MEASURED_PEAKS.json sm_max_mhz" if peaks else "NVML max clock"),
                 "alg_mults_per_event": ALG_MULTS_PER_EVENT[model], "executed_mults_per_event": exec_per_event,
                 "avg_launch_ms": avg_kern_s * 1e3,
-                "frac_note": "achieved/frac count the ALGORITHMIC multiplies (SURVEY.md S8(d): 22 per event); the kernel executes "
-                             "fewer (19, or 18 when two steps share a pass over the agents: hoisted / strength-reduced / shared "
-                             "rounds, w3 skipped; counted in the SASS by tests/test_library_host.py), so frac can pass 1.0 -- "
-                             "the pipe's own utilisation is frac_executed "
-                             "(ncu: sm__pipe_fmaheavy_cycles_active, profiles/)",
-                "hbm": {"algorithmic_bytes": M * (8 * L + 128), "achieved_GBps": M * (8 * L + 128) / avg_kern_s / 1e9,
-                        "peak_GBps": peaks.get("hbm_gbs", 6650.0),
-                        "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback (B200_PROFILING.md)"}}
+                "frac_note": "achieved/frac count the multiplies the kernel EXECUTES per event (counted in the SASS by "
+                             "tests/test_library_host.py): a utilisation of the multiply pipe, <= 1 (ncu: "
+                             "sm__pipe_fmaheavy_cycles_active, profiles/).  achieved_algorithmic/frac_algorithmic count SURVEY.md "
+                             "S8(d)'s ALGORITHMIC 22 per event; the kernel executes fewer (19, or 18 when two steps share a pass: "
+                             "hoisted / strength-reduced / shared rounds, w3 skipped), so that figure can pass 1.0",
+                "hbm": None}
     if micro:
         # BASELINE.json's metric names the smem-atomic roofline: keep its two fractions beside the headline
         roofline["frac_of_smem_atomic_peak"] = micro["frac_of_smem_atomic_peak"]
@@ -584,11 +642,30 @@ def main():
         "kernel_events_per_s": kev,
         "paper_context": {"events_per_s": 5.47e10, "where": "RTX 5090, M=8192 A=1024 L=128 S=500, PAPER.md:313 (other GPU, other agent model)"},
     }
-    if micro:
-        line["microbench"] = micro
+    # ---- a0/a7 against HBM: the state phase alone (A = 0, S = 1 after ks_write_books) on the C4 and C5 shapes
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    state_io = {name: time_state_io(ks, torch, dev, CONFIGS[name], hbm_peak) for name in ("C4", "C5")}
+    state_io["peak_GBps"] = hbm_peak
+    state_io["peak_source"] = "MEASURED_PEAKS.json hbm_gbs (measured)" if peaks else "fallback (B200_PROFILING.md)"
+    state_io["what"] = ("ks_run(S=1) with A=0 on resident books after ks_write_books: book + record load, book + record store, "
+                        "2*M*(8L+128) bytes, median device time of 5")
+    roofline["hbm"] = {"algorithmic_bytes": state_io["C4"]["bytes"], "achieved_GBps": state_io["C4"]["GBps"], "peak_GBps": hbm_peak,
+                       "frac": state_io["C4"]["frac_of_hbm"], "peak_source": state_io["peak_source"],
+                       "what": "the state phase (a0 + a7) of the C4 shape timed alone, see state_io; inside the 608 ms launch "
+                               "it is 0.02 % of the time"}
 
+    detail, tail = {}, {}
+    if micro:
+        detail["microbench"] = micro
+        tail["microbench"] = {"mul_wide_u32_T_per_s": micro["mul_wide_u32_thread_ops_per_s"] / 1e12,
+                              "smem_atomic_peak_T_per_s": micro["smem_atomic_peak_lane_ops_per_s"] / 1e12,
+                              "smem_atomic_pattern_T_per_s": micro["smem_atomic_pattern_lane_ops_per_s"] / 1e12,
+                              "generate_only_events_per_s": micro["generate_only_events_per_s"]}
     if not args.no_extras:
-        line.update(extras(ks, torch, dev, peak, cfg))
+        d_, t_ = extras(ks, torch, dev, peak, cfg, micro)
+        detail.update(d_)
+        tail.update(t_)
+    line["detail"] = detail
 
     if not args.no_cpu_baseline:
         n_mk = min(cfg.M, 64)
@@ -596,6 +673,9 @@ def main():
         line["cpu_baseline"] = {"value": ev_s, "unit": "events/s", "cores": 1, "kind": "oracle",
                                 "sample": "%d seeded sampled markets x S=%d steps of %s (%.3g events, %.1f s), 1 thread of %d host cores"
                                           % (n, S, cfg.name, n * A * S, dt, os.cpu_count() or 0)}
+    # compact per-config numbers LAST: the driver's record keeps the tail of the line
+    line["state_io"] = state_io
+    line.update(tail)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -609,12 +689,19 @@ PROFILED_TRAFFIC_C2 = {"persistent": {"dram_bytes": 215040 + 0, "global_load_sto
                        "source": "profiles/r2d_traffic.md (ncu; the L2 is invalidated between launches under ncu)"}
 
 
-def extras(ks, torch, dev, peak_tmults, headline_cfg):
+def compact(r):
+    """{ms, events_per_s, frac_executed, plan} of a timed case, plan shortened."""
+    return {"ms": round(r["ms"], 4), "events_per_s": float("%.4g" % r["events_per_s"]), "frac_executed": round(r["frac_executed"], 4),
+            "plan": r["plan"].replace("ks_", "").replace("_kernel", "").replace("steps_per_pass", "spp")}
+
+
+def extras(ks, torch, dev, peak_tmults, headline_cfg, micro):
     """The other BASELINE configs, the other contracts and the ablation, timed in the same process
     (each a few ms to a few hundred ms of GPU time): every number DESIGN.md quotes is in the
     driver-run line.  frac_executed = executed multiplies/s over the same measured peak as the
-    headline's roofline."""
-    out = {}
+    headline's roofline.  -> (detail, tail): the full records, and the compact ones that go LAST in
+    the JSON line."""
+    out, tail = {}, {}
 
     def with_frac(r, c):
         r["executed_mults_per_event"] = exec_mults(c.params, r["plan"])
@@ -629,12 +716,25 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
         c = CONFIGS[name]
         allc[name] = with_frac(time_case(ks, torch, dev, c, reps=5 if c.events < 5e10 else 3), c)
     out["all_configs"] = allc
+    tail["all_configs"] = {k: compact(v) for k, v in allc.items()}
+    for name in ("C1", "C3"):
+        if name in allc:
+            tail["all_configs"][name]["us_per_step"] = round(allc[name]["us_per_step"], 4)
     for key, case in (("packed4_C4", "C4_packed4"), ("model4_C4shape", "model4_C4shape")):
         c = case_config(case)
         out[key] = with_frac(time_case(ks, torch, dev, c, reps=3), c)
+        tail[key] = compact(out[key])
     out["packed4_C4"]["note"] = "PACKED4 draw contract (DESIGN.md A22): NOT the BASELINE.json contract, reported beside it"
     out["model4_C4shape"]["note"] = ("the paper's own agent model (DESIGN.md A24) on the C4 shape, alpha_mom = alpha_maker = 0.15, "
                                      "Delta = 32, q <= 100, P_mkt = 0.02 (parameter values ours: the paper gives none)")
+    if micro:
+        # PACKED4 is where the smem-atomic roofline BASELINE.json names can be approached: its fractions too
+        tail["packed4_C4"]["frac_of_smem_atomic_peak"] = round(out["packed4_C4"]["events_per_s"] / micro["smem_atomic_peak_lane_ops_per_s"], 4)
+        tail["packed4_C4"]["frac_of_smem_atomic_pattern"] = round(out["packed4_C4"]["events_per_s"] / micro["smem_atomic_pattern_lane_ops_per_s"], 4)
+
+    # end to end (host buffers, host clock) for the latency-regime configs
+    tail["e2e_small"] = {name: {k: (round(v, 4) if isinstance(v, float) and v < 1e6 else v) for k, v in
+                                time_e2e_small(ks, torch, dev, CONFIGS[name]).items()} for name in ("C1", "C3")}
 
     # a8 ablation on C2: one launch per step, book through HBM every step
     c = CONFIGS["C2"]
@@ -645,6 +745,9 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
         "slowdown_vs_persistent": sw["ms"] / pers["ms"],
         "algorithmic_hbm_bytes": float(c.S) * c.M * 2 * (8 * c.L + 128), "persistent_algorithmic_hbm_bytes": float(c.M) * (8 * c.L + 128),
         "measured_traffic": PROFILED_TRAFFIC_C2}
+    tail["ablation_launch_per_step_C2"] = {"ms": round(sw["ms"], 4), "persistent_ms": round(pers["ms"], 4), "launches": c.S,
+                                           "us_per_launch": round(sw["ms"] * 1e3 / c.S, 3),
+                                           "slowdown_vs_persistent": round(sw["ms"] / pers["ms"], 3)}
 
     # context runs in the paper's own shapes: Table IV's fixed workload and the
     # latency configuration with zero-intelligence agents -- NOT the paper's
@@ -672,7 +775,7 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
             sim = ks.KsSim(Ms, Ls, As, paper_params(As, al), 5, state=st)
             sim.ks_run_traced(Ss, tr)
             ks.ks_trace_stats(tr, Ms, Ss, K, res)
-            if record:
+            if record and al in (0.0, 0.15, 0.7):
                 o = res.cpu().numpy()
                 rows.append({"alpha_mom": al, "volatility": float(np.nanmean(o[:, 0])), "excess_kurtosis": float(np.nanmean(o[:, 1])),
                              "volume_per_step": float(np.nanmean(o[:, 2])), "acf_r_lag1": float(np.nanmean(o[:, 4])),
@@ -687,7 +790,7 @@ def extras(ks, torch, dev, peak_tmults, headline_cfg):
     out["sivj_sweep"] = {"configs": len(alphas), "M": Ms, "L": Ls, "A": As, "S": Ss, "agent_events": len(alphas) * Ms * As * Ss,
                          "ms_total_device": a.elapsed_time(b), "paper": "< 250 ms for 12.8e6 events (RTX 5090, PAPER.md:458)",
                          "mean_over_markets": rows}
-    return out
+    return out, tail
 
 
 if __name__ == "__main__":
