@@ -293,22 +293,25 @@ def time_case(ks, torch, dev, c, *, reps=3, mode="persistent", S=None, M=None, o
             "plan": plan}
 
 
-def time_state_io(ks, torch, dev, c, hbm_peak_gbs, reps=5):
+def time_state_io(ks, torch, dev, c, hbm_peak_gbs, reps=5, warm_steps=8, threads=0):
     """a0 + a7 alone (north_star: "HBM peak for the book load and store"; Eq.6): the
-    config's M x L books resident in HBM (ks_write_books of random books, so the load is not
-    skipped), no agents, ONE step -- the launch loads every book and record and stores them again.
+    config's own resting books after `warm_steps` real steps, resident in HBM; then a handle with NO
+    agents attached to that state (ks_attach) runs ONE step -- the launch loads every book and
+    record, clears an already uncrossed book (nothing trades) and stores them again.
     Bytes = 2 * M * (8L + 128).  Median device time of `reps` launches, CUDA events."""
-    from paper_2606_21784_b200.workloads import random_books
     M, L = c.M, c.L
     st = torch.empty(ks.ks_state_bytes(M, L), dtype=torch.uint8, device=dev)
-    one = torch.from_numpy(random_books(64, L, seed=11, max_qty=50, fill=0.3)).to(dev)
-    books = one.repeat((M + 63) // 64, 1, 1)[:M].contiguous()
+    sim = ks.KsSim(M, L, c.A, c.params, c.seed, state=st)
+    sim.ks_run(warm_steps)
+    torch.cuda.synchronize()
+    sim.ks_error_state()
+    sim.ks_destroy()
     ts, plan = [], ""
     for i in range(1 + reps):
-        sim = ks.KsSim(M, L, 0, c.params, c.seed, state=st)
+        sim = ks.KsSim(M, L, 0, c.params, c.seed, state=st, attach=True)      # synchronises
         try:
-            sim.ks_write_books(books)
-            torch.cuda.synchronize()
+            if threads:
+                sim.ks_set_option(ks.KS_OPT_BLOCK_THREADS, threads)
             plan = sim.ks_plan_string()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(); sim.ks_run(1); b.record()
@@ -645,10 +648,13 @@ def main():
     # ---- a0/a7 against HBM: the state phase alone (A = 0, S = 1 after ks_write_books) on the C4 and C5 shapes
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     state_io = {name: time_state_io(ks, torch, dev, CONFIGS[name], hbm_peak) for name in ("C4", "C5")}
+    # the same with the block size of the plan the config itself runs under (C4: 96, C5: 160 threads)
+    state_io["C4_T96"] = time_state_io(ks, torch, dev, CONFIGS["C4"], hbm_peak, threads=96)
+    state_io["C5_T160"] = time_state_io(ks, torch, dev, CONFIGS["C5"], hbm_peak, threads=160)
     state_io["peak_GBps"] = hbm_peak
     state_io["peak_source"] = "MEASURED_PEAKS.json hbm_gbs (measured)" if peaks else "fallback (B200_PROFILING.md)"
-    state_io["what"] = ("ks_run(S=1) with A=0 on resident books after ks_write_books: book + record load, book + record store, "
-                        "2*M*(8L+128) bytes, median device time of 5")
+    state_io["what"] = ("ks_run(S=1) of a handle with A=0 attached to the config's own resting books (8 real steps): book + record load, "
+                        "one clearing of an uncrossed book, book + record store; 2*M*(8L+128) bytes, median device time of 5")
     roofline["hbm"] = {"algorithmic_bytes": state_io["C4"]["bytes"], "achieved_GBps": state_io["C4"]["GBps"], "peak_GBps": hbm_peak,
                        "frac": state_io["C4"]["frac_of_hbm"], "peak_source": state_io["peak_source"],
                        "what": "the state phase (a0 + a7) of the C4 shape timed alone, see state_io; inside the 608 ms launch "

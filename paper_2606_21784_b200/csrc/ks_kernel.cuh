@@ -138,8 +138,42 @@ __device__ __forceinline__ bool depth_check_aborts(const KernelParams& P, int* s
   return *s_abort != 0;
 }
 
-// a0: state load (HBM -> shared) of one market's [2][L] book, skipped for a fresh (all-zero) book;
-// per-thread partial depth totals and extents of what was loaded.
+// Bulk asynchronous copies (TMA engine, no tensor map): ONE elected thread moves a whole 8*L-byte
+// book between HBM and shared memory, so the state phase does not depend on how many threads the
+// CTA has (32 for the throughput plan: 32 threads of int4 loads left the copy engine idle) and the
+// other threads hold no registers or LSU slots for it.  Sizes are multiples of 16 bytes (L >= 32),
+// both addresses 16-byte aligned (d_state is, and 8*L is a multiple of 256).
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst_smem, const void* src_gmem, uint32_t bytes, uint32_t mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst_smem), "l"(src_gmem), "r"(bytes), "r"(mbar) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* dst_gmem, uint32_t src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(src_smem), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+// the bulk stores of this thread have READ their shared-memory source (the CTA may exit)
+__device__ __forceinline__ void bulk_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// generic-proxy writes of this thread to shared memory become visible to the async proxy (the copy engine)
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// a0: state load (HBM -> shared) of one market's [2][L] book, skipped for a fresh (all-zero) book:
+// one bulk copy of 8*L bytes issued by thread 0, completion on an mbarrier every thread waits on;
+// then a pass over SHARED memory gives the per-thread partial depth totals and extents of what was
+// loaded.
 __device__ __forceinline__ void load_book(const KernelParams& P, int32_t* book, const int32_t* gbook, int L,
                                           long long& sb0, long long& sa0, int& bmax, int& amin) {
   const int tid = threadIdx.x, T = blockDim.x;
@@ -149,11 +183,18 @@ __device__ __forceinline__ void load_book(const KernelParams& P, int32_t* book, 
   if (P.fresh) {
     for (int i = tid; i < nvec; i += T) sbook4[i] = make_int4(0, 0, 0, 0);
   } else {
-    const int4* gbook4 = reinterpret_cast<const int4*>(gbook);
+    __shared__ __align__(8) unsigned long long s_load_mbar;
+    const uint32_t mbar = (uint32_t)__cvta_generic_to_shared(&s_load_mbar);
+    if (tid == 0) {
+      mbar_init(mbar, 1);
+      mbar_expect_tx(mbar, 8u * (uint32_t)L);
+      bulk_load((uint32_t)__cvta_generic_to_shared(book), gbook, 8u * (uint32_t)L, mbar);
+    }
+    __syncthreads();                                   // the barrier object exists before anybody polls it
+    mbar_wait(mbar, 0);
     const int nside = L / 4;
     for (int i = tid; i < nvec; i += T) {
-      int4 v = __ldg(gbook4 + i);
-      sbook4[i] = v;
+      const int4 v = sbook4[i];
       int vals[4] = {v.x, v.y, v.z, v.w};
       if (i < nside) {
 #pragma unroll
@@ -166,28 +207,31 @@ __device__ __forceinline__ void load_book(const KernelParams& P, int32_t* book, 
   }
 }
 
-// a7: write-back (shared -> HBM) of the book with 16-byte vectors and of the 128-byte record; the
-// depth totals give sub_buy / sub_sell by conservation: submitted = (resting after - resting
-// before) + executed during this run (the oracle counts the same quantity order by order).
-// keep[3] = resting bid total, resting ask total, executed volume at the start of the run.
+// a7: write-back (shared -> HBM) of the book with ONE bulk copy and of the 128-byte record; the
+// depth totals (a pass over shared memory) give sub_buy / sub_sell by conservation: submitted =
+// (resting after - resting before) + executed during this run (the oracle counts the same quantity
+// order by order).  keep[3] = resting bid total, resting ask total, executed volume at the start
+// of the run.  Every thread fences its own book writes towards the copy engine before the barriers
+// of the reduction; thread 0 issues the copy after them and keeps the CTA alive until the engine
+// has read the book.
 __device__ __forceinline__ void store_state(const KernelParams& P, const int32_t* book, int32_t* gbook, long long* grec, int L,
                                             long long* s_rec, const long long* keep, const int* s_ovf,
                                             long long* s_red64, int* s_red32) {
   const int tid = threadIdx.x, T = blockDim.x;
   long long sb1 = 0, sa1 = 0;
+  fence_proxy_async_smem();
   {
     const int nvec = L / 2, nside = L / 4;
     const int4* sbook4 = reinterpret_cast<const int4*>(book);
-    int4* gbook4 = reinterpret_cast<int4*>(gbook);
     for (int i = tid; i < nvec; i += T) {
-      int4 v = sbook4[i];
-      gbook4[i] = v;
+      const int4 v = sbook4[i];
       long long sum = (long long)v.x + v.y + v.z + v.w;
       if (i < nside) sb1 += sum; else sa1 += sum;
     }
   }
-  BookTotals tot1 = block_reduce_totals(sb1, sa1, -1, 0x7fffffff, s_red64, s_red32);
+  BookTotals tot1 = block_reduce_totals(sb1, sa1, -1, 0x7fffffff, s_red64, s_red32);     // has barriers
   if (tid == 0) {
+    bulk_store(gbook, (uint32_t)__cvta_generic_to_shared(book), 8u * (uint32_t)L);
     long long dvol = s_rec[F_SUMVOL] - keep[2];
     s_rec[F_SUBBUY] += (tot1.sum_bid - keep[0]) + dvol;
     s_rec[F_SUBSELL] += (tot1.sum_ask - keep[1]) + dvol;
@@ -196,6 +240,7 @@ __device__ __forceinline__ void store_state(const KernelParams& P, const int32_t
   }
   __syncthreads();
   if (tid < 16) grec[tid] = s_rec[tid];
+  if (tid == 0) bulk_store_wait_read();
 }
 
 // a3-a5 on the active window [lo, hi] of a book in this CTA's shared memory, by one warp: picks
