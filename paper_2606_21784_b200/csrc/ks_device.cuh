@@ -463,7 +463,7 @@ __device__ __forceinline__ void packed_agent(const KernelParams& P, const BookRe
 // clearing warp widens its window to that boundary.
 template <int ATOM, int KIND, bool CLAMP>
 __device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef& book, const RuleCtx& rc,
-                                            const uint32_t (&w)[4], uint32_t parity, int& sink) {
+                                            const uint32_t (&w)[4], uint32_t parity, uint32_t& mkt_seen, int& sink) {
   const uint32_t qmax = KIND == 0 ? (uint32_t)P.noise_qmax : (KIND == 1 ? (uint32_t)P.mom_qmax : (uint32_t)P.maker_qty);
   const int q = (int)hi32((uint64_t)w[2] * qmax + P.q_addend);
   const bool buy = KIND == 0 ? (int32_t)w[0] < 0
@@ -483,9 +483,13 @@ __device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef
     } else {
       addr = buy ? rc.bid_last - 4u * (uint32_t)P.maker_spread_max : rc.ask_last + 4u * (uint32_t)P.maker_spread_max;
     }
-    if (mkt) {
-      addr = buy ? book.saddr + 4u * (uint32_t)(rc.L - 1) : book.saddr + 4u * (uint32_t)rc.L;   // bid[L-1] / ask[0]
-      rc.mkt_flags[buy ? 0 : 1] = 1;
+    if (KIND != 2) {
+      // branch-free (a divergent branch per event kept ptxas from interleaving the four unrolled
+      // events): the edge address by two selects, the flag as a bit kept in a register until the
+      // thread has generated all its orders of the step (generate_step_paper stores it once)
+      const uint32_t edge = buy ? book.saddr + 4u * (uint32_t)(rc.L - 1) : book.saddr + 4u * (uint32_t)rc.L;   // bid[L-1] / ask[0]
+      addr = mkt ? edge : addr;
+      mkt_seen |= mkt ? (buy ? 1u : 2u) : 0u;
     }
     book_add_at<ATOM>(book, addr, q, sink);
   } else {
@@ -494,9 +498,9 @@ __device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef
     else if (KIND == 1) p2 = rc.mid2 + (buy ? 2 : -2);
     else                p2 = rc.mid2 + (buy ? -2 : 2) * P.maker_spread_max;
     int tick = clamp_tick((p2 + 1) >> 1, rc.L);
-    if (mkt) {
-      tick = buy ? rc.L - 1 : 0;
-      rc.mkt_flags[buy ? 0 : 1] = 1;
+    if (KIND != 2) {
+      tick = mkt ? (buy ? rc.L - 1 : 0) : tick;
+      mkt_seen |= mkt ? (buy ? 1u : 2u) : 0u;
     }
     book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
   }
@@ -750,11 +754,11 @@ __device__ __forceinline__ void generate_mix3_rel_group(const KernelParams& P, c
 template <int ATOM, int KIND, bool CLAMP>
 __device__ __forceinline__ void generate_class_paper(const KernelParams& P, const BookRef& book, const MarketUniform& mu,
                                                      const StepUniform& u, const RuleCtx& rc, const ClassPlan& pl,
-                                                     const P0Step& p0_inc, uint32_t parity, int& sink) {
+                                                     const P0Step& p0_inc, uint32_t parity, uint32_t& mkt_seen, int& sink) {
   auto one = [&](uint64_t p0) {
     uint32_t w[4];
     philox_block_from_p0(P, mu, u, p0, w);
-    paper_order<ATOM, KIND, CLAMP>(P, book, rc, w, parity, sink);
+    paper_order<ATOM, KIND, CLAMP>(P, book, rc, w, parity, mkt_seen, sink);
   };
   uint64_t p0 = pl.p0;
 #pragma unroll kGenUnroll
@@ -781,15 +785,18 @@ __device__ __forceinline__ void generate_step_paper(const KernelParams& P, const
                                                     int tid, uint32_t t, int& sink) {
   const uint32_t maker_first = (uint32_t)P.paper_n_noise + (uint32_t)P.paper_n_mom + (uint32_t)tid;
   const uint32_t par = (maker_first + t) & 1u;
+  uint32_t mkt_seen = 0;                               // bit 0: a marketable buy, bit 1: a marketable sell
   if (rc.noclamp) {
-    generate_class_paper<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, sink);
-    generate_class_paper<ATOM, 1, false>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, sink);
-    generate_class_paper<ATOM, 2, false>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, sink);
+    generate_class_paper<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, mkt_seen, sink);
+    generate_class_paper<ATOM, 1, false>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, mkt_seen, sink);
+    generate_class_paper<ATOM, 2, false>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, mkt_seen, sink);
   } else {
-    generate_class_paper<ATOM, 0, true>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, sink);
-    generate_class_paper<ATOM, 1, true>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, sink);
-    generate_class_paper<ATOM, 2, true>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, sink);
+    generate_class_paper<ATOM, 0, true>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, mkt_seen, sink);
+    generate_class_paper<ATOM, 1, true>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, mkt_seen, sink);
+    generate_class_paper<ATOM, 2, true>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, mkt_seen, sink);
   }
+  if (mkt_seen & 1u) rc.mkt_flags[0] = 1;
+  if (mkt_seen & 2u) rc.mkt_flags[1] = 1;
 }
 
 // The highest tick < `from` with bid depth (-1 if none) / the lowest tick >= `from` with ask depth
