@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
                     [--scaling weak|strong] [--rng literal|packed4] [--no-extras]
-    python bench.py --case NAME [--S n] [--M m] [--mode persistent|stepwise|traced]   # one run, for ncu
+    python bench.py --case NAME [--S n] [--M m] [--mode persistent|stepwise|traced|state_io]   # one run, for ncu
 
 A "step" is one pass of the whole hot path over one batch: ks_create (state init) + ONE ks_run of
 all S steps of the workload (a0-a7).  Workload: BASELINE.json configs[3] ("throughput scale", C4:
@@ -376,6 +376,13 @@ def run_case(args):
     if args.rel_columns:
         opts.append((ks.KS_OPT_REL_COLUMNS, args.rel_columns))
     n0 = ks.ks_launch_count()
+    if args.mode == "state_io":
+        # the state phase alone (a0 + a7): the launch bench.py's state_io key times
+        r = time_state_io(ks, torch, dev, c, 1.0, reps=1, threads=args.threads)
+        r.update({"case": c.name, "mode": args.mode, "gpu_launches": ks.ks_launch_count() - n0})
+        del r["frac_of_hbm"]
+        print(json.dumps(r), flush=True)
+        return
     r = time_case(ks, torch, dev, c, reps=1, mode=args.mode, S=args.S, M=args.M, opts=opts)
     if args.trace_stats:
         M, S = r["M"], r["S"]
@@ -412,7 +419,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs / contracts / ablation keys")
     ap.add_argument("--all-configs", action="store_true", help="(kept for compatibility: the extras are on by default)")
     ap.add_argument("--case", default=None, help="run ONE named case once and print a small JSON line (ncu / sanitizer helper)")
-    ap.add_argument("--mode", default="persistent", choices=["persistent", "stepwise", "traced"])
+    ap.add_argument("--mode", default="persistent", choices=["persistent", "stepwise", "traced", "state_io"])
     ap.add_argument("--trace-stats", action="store_true", help="--case: also launch ks_run_traced + ks_trace_stats once")
     ap.add_argument("--S", type=int, default=None, help="--case: override the number of steps")
     ap.add_argument("--M", type=int, default=None, help="--case: override the number of markets")

@@ -192,18 +192,28 @@ __device__ __forceinline__ void load_book(const KernelParams& P, int32_t* book, 
     }
     __syncthreads();                                   // the barrier object exists before anybody polls it
     mbar_wait(mbar, 0);
+    // Depths are >= 0 and a side's total stays below 2^31 (the guards of ks_run; ks_write_books and
+    // ks_attach refuse negative entries), so a thread's partial sums fit 32 bits and "this vector
+    // holds depth" is "its sum is not zero".  Per 16-byte vector: one LDS.128, the sum, one compare;
+    // the tick inside the extreme vector is found once, after the loops (with 32 threads and 4 KB of
+    // book the state phase is bound by instruction issue, not by HBM: profiles/r3_state_io.md).
     const int nside = L / 4;
-    for (int i = tid; i < nvec; i += T) {
+    int s32b = 0, s32a = 0, ib = -1, ia = -1;
+    for (int i = tid; i < nside; i += T) {             // bids: the LAST vector with depth (i increases)
       const int4 v = sbook4[i];
-      int vals[4] = {v.x, v.y, v.z, v.w};
-      if (i < nside) {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { sb0 += vals[j]; if (vals[j] > 0) bmax = max(bmax, 4 * i + j); }
-      } else {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { sa0 += vals[j]; if (vals[j] > 0) amin = min(amin, 4 * (i - nside) + j); }
-      }
+      const int sum = (v.x + v.y) + (v.z + v.w);
+      s32b += sum;
+      ib = sum != 0 ? i : ib;
     }
+    for (int i = nside + tid; i < nvec; i += T) {      // asks: the FIRST vector with depth
+      const int4 v = sbook4[i];
+      const int sum = (v.x + v.y) + (v.z + v.w);
+      s32a += sum;
+      ia = (sum != 0 && ia < 0) ? i : ia;
+    }
+    sb0 = s32b; sa0 = s32a;
+    if (ib >= 0) { const int4 v = sbook4[ib]; bmax = 4 * ib + (v.w > 0 ? 3 : v.z > 0 ? 2 : v.y > 0 ? 1 : 0); }
+    if (ia >= 0) { const int4 v = sbook4[ia]; amin = 4 * (ia - nside) + (v.x > 0 ? 0 : v.y > 0 ? 1 : v.z > 0 ? 2 : 3); }
   }
 }
 
@@ -218,18 +228,15 @@ __device__ __forceinline__ void store_state(const KernelParams& P, const int32_t
                                             long long* s_rec, const long long* keep, const int* s_ovf,
                                             long long* s_red64, int* s_red32) {
   const int tid = threadIdx.x, T = blockDim.x;
-  long long sb1 = 0, sa1 = 0;
+  int s32b = 0, s32a = 0;                              // 32 bits suffice: see load_book
   fence_proxy_async_smem();
   {
     const int nvec = L / 2, nside = L / 4;
     const int4* sbook4 = reinterpret_cast<const int4*>(book);
-    for (int i = tid; i < nvec; i += T) {
-      const int4 v = sbook4[i];
-      long long sum = (long long)v.x + v.y + v.z + v.w;
-      if (i < nside) sb1 += sum; else sa1 += sum;
-    }
+    for (int i = tid; i < nside; i += T) { const int4 v = sbook4[i]; s32b += (v.x + v.y) + (v.z + v.w); }
+    for (int i = nside + tid; i < nvec; i += T) { const int4 v = sbook4[i]; s32a += (v.x + v.y) + (v.z + v.w); }
   }
-  BookTotals tot1 = block_reduce_totals(sb1, sa1, -1, 0x7fffffff, s_red64, s_red32);     // has barriers
+  BookTotals tot1 = block_reduce_totals((long long)s32b, (long long)s32a, -1, 0x7fffffff, s_red64, s_red32);     // has barriers
   if (tid == 0) {
     bulk_store(gbook, (uint32_t)__cvta_generic_to_shared(book), 8u * (uint32_t)L);
     long long dvol = s_rec[F_SUMVOL] - keep[2];
