@@ -485,11 +485,13 @@ __device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef
     }
     if (KIND != 2) {
       // branch-free (a divergent branch per event kept ptxas from interleaving the four unrolled
-      // events): the edge address by two selects, the flag as a bit kept in a register until the
-      // thread has generated all its orders of the step (generate_step_paper stores it once)
+      // events): the edge address by two selects; whether the thread generated ANY marketable order
+      // this step is the running minimum of the 16-bit draw, one instruction per event
+      // (generate_step_paper compares it once and raises both flags: the clearing warp then reads the
+      // depth at both edge ticks, and an edge nobody hit holds none)
       const uint32_t edge = buy ? book.saddr + 4u * (uint32_t)(rc.L - 1) : book.saddr + 4u * (uint32_t)rc.L;   // bid[L-1] / ask[0]
       addr = mkt ? edge : addr;
-      mkt_seen |= mkt ? (buy ? 1u : 2u) : 0u;
+      mkt_seen = min(mkt_seen, w[3] >> 16);
     }
     book_add_at<ATOM>(book, addr, q, sink);
   } else {
@@ -500,7 +502,7 @@ __device__ __forceinline__ void paper_order(const KernelParams& P, const BookRef
     int tick = clamp_tick((p2 + 1) >> 1, rc.L);
     if (KIND != 2) {
       tick = mkt ? (buy ? rc.L - 1 : 0) : tick;
-      mkt_seen |= mkt ? (buy ? 1u : 2u) : 0u;
+      mkt_seen = min(mkt_seen, w[3] >> 16);
     }
     book_add<ATOM>(book, 4u * (uint32_t)(buy ? tick : tick + rc.L), q, sink);
   }
@@ -785,7 +787,7 @@ __device__ __forceinline__ void generate_step_paper(const KernelParams& P, const
                                                     int tid, uint32_t t, int& sink) {
   const uint32_t maker_first = (uint32_t)P.paper_n_noise + (uint32_t)P.paper_n_mom + (uint32_t)tid;
   const uint32_t par = (maker_first + t) & 1u;
-  uint32_t mkt_seen = 0;                               // bit 0: a marketable buy, bit 1: a marketable sell
+  uint32_t mkt_seen = 0x10000u;                        // smallest 16-bit marketable draw among this thread's noise / momentum agents (none: 2^16)
   if (rc.noclamp) {
     generate_class_paper<ATOM, 0, false>(P, book, mu, u, rc, g.cls[0], g.p0_inc, 0u, mkt_seen, sink);
     generate_class_paper<ATOM, 1, false>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, mkt_seen, sink);
@@ -795,8 +797,7 @@ __device__ __forceinline__ void generate_step_paper(const KernelParams& P, const
     generate_class_paper<ATOM, 1, true>(P, book, mu, u, rc, g.cls[1], g.p0_inc, 0u, mkt_seen, sink);
     generate_class_paper<ATOM, 2, true>(P, book, mu, u, rc, g.cls[2], g.p0_inc, par, mkt_seen, sink);
   }
-  if (mkt_seen & 1u) rc.mkt_flags[0] = 1;
-  if (mkt_seen & 2u) rc.mkt_flags[1] = 1;
+  if ((int)mkt_seen < P.paper_pmkt_q16) { rc.mkt_flags[0] = 1; rc.mkt_flags[1] = 1; }
 }
 
 // The highest tick < `from` with bid depth (-1 if none) / the lowest tick >= `from` with ask depth
